@@ -1,0 +1,484 @@
+// caee_oracle.cpp — CPU oracle for the CAEE per-layer MoE decode path.
+//
+// TEST INFRASTRUCTURE ONLY.  This file is the slow, plain, obviously-correct
+// restatement of what the hot path computes, written from the paper
+// (/root/reference/PAPER.md, cited as PAPER.md:<line>) and, where the paper is
+// silent, from the readings listed in DESIGN.md §3 (numbered R1..R28 after
+// SURVEY.md §8(c)).  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load it.  It shares no code, header,
+// table or helper with the CUDA path under paper_2606_29982_b200/csrc/.
+//
+// Conventions: decision logic (O1..O6) is fp32 in a fixed evaluation order, or
+// integer; this file must be compiled with -ffp-contract=off so that no
+// multiply-add is fused.  The FFN and combine (O7, O8) accumulate in fp64 with
+// operands widened exactly from their storage type; y is returned in fp64,
+// unrounded (reading R29).
+//
+// Pins (tests/test_oracle_*.py, all -m "not gpu"):
+//   O0 scores      : fp64 torch matmul + torch.sigmoid / softmax
+//   O1 route       : torch.topk reductions, brute force over C(E,k), invariants
+//                    (exact DeepSeek-style form: "parity unpinned" by PAPER.md —
+//                    the paper never defines its router; pinned by BASELINE.json
+//                    configs + invariants only)
+//   O2 importance  : sum_e I(e) = T, order independence
+//   O3 cost/F_cost : closed forms (3573 ns, 11.010 us), literal max-of-sums
+//   O4 prune       : brute force over all subsets, F_cost == F_base, maximality
+//   O5 compensate  : K_final subset of A_trans, unaffected tokens untouched
+//   O6 compact     : inverse-permutation check against idx
+//   O7/O8 FFN      : torch fp64 SwiGLU MLP, linearity, concatenation identity,
+//                    e4m3 closed-form table vs torch.float8_e4m3fn
+//   O9 fit         : exact recovery of a synthetic line, numpy.polyfit
+//   whole method vs the paper's reported latency/accuracy: parity unpinned
+//   (needs the model, suites and hardware the container lacks).
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+enum Dtype { DT_F32 = 0, DT_BF16 = 1, DT_E4M3 = 2 };
+enum ScoreFn { SCORE_SOFTMAX = 0, SCORE_SIGMOID = 1 };
+enum PruneMode { MODE_NONE = 0, MODE_THRESH = 1, MODE_CIR = 2, MODE_RANK = 3, MODE_FRAC = 4 };
+enum Flags { FLAG_COMP_ALL_TOKENS = 1, FLAG_KEEP_TOP1 = 2 };
+
+const double FIX_ONE = 1099511627776.0;  // 2^40, fixed-point unit of I_fix (reading R-fix)
+
+inline float bf16_widen(uint16_t b) {
+  uint32_t u = static_cast<uint32_t>(b) << 16;
+  float f;
+  std::memcpy(&f, &u, 4);
+  return f;
+}
+
+// OCP FP8 E4M3 ("fn": no infinities, S.1111.111 is NaN, max 448):
+// value = (-1)^s * 2^(e-7) * (1 + m/8) for e > 0; (-1)^s * 2^-6 * (m/8) for e == 0.
+inline double e4m3_value(uint8_t c) {
+  int s = c >> 7, e = (c >> 3) & 15, m = c & 7;
+  if (e == 15 && m == 7) return std::numeric_limits<double>::quiet_NaN();
+  double v = (e == 0) ? std::ldexp(m / 8.0, -6) : std::ldexp(1.0 + m / 8.0, e - 7);
+  return s ? -v : v;
+}
+
+// One stored matrix [rows, cols], row-major, with optional 128x128 block scales
+// scales[ceil(rows/128), ceil(cols/128)] (fp32) for DT_E4M3.
+struct Mat {
+  const void* p;
+  int dtype;
+  const float* scales;
+  int rows, cols;
+  inline double at(int r, int c) const {
+    size_t i = static_cast<size_t>(r) * cols + c;
+    switch (dtype) {
+      case DT_F32: return static_cast<const float*>(p)[i];
+      case DT_BF16: return bf16_widen(static_cast<const uint16_t*>(p)[i]);
+      default: {
+        int nbc = (cols + 127) / 128;
+        double sc = scales ? scales[static_cast<size_t>(r / 128) * nbc + c / 128] : 1.0;
+        return e4m3_value(static_cast<const uint8_t*>(p)[i]) * sc;
+      }
+    }
+  }
+};
+
+inline double act_at(const void* x, int dtype, size_t i) {
+  return dtype == DT_F32 ? static_cast<const float*>(x)[i]
+                         : bf16_widen(static_cast<const uint16_t*>(x)[i]);
+}
+
+// "a ranks before b" in a descending selection with ties -> lower index (reading R22).
+inline bool before(float va, int ia, float vb, int ib) { return va > vb || (va == vb && ia < ib); }
+
+// Top-k of v[0..n) by (value desc, index asc); entries with ok[i]==0 are excluded.
+// Returns the number selected (<= k).  Plain selection: repeat argmax.
+int topk_select(const float* v, const uint8_t* ok, int n, int k, int32_t* out) {
+  std::vector<uint8_t> taken(n, 0);
+  int cnt = 0;
+  for (int j = 0; j < k; ++j) {
+    int best = -1;
+    for (int i = 0; i < n; ++i) {
+      if (taken[i] || (ok && !ok[i])) continue;
+      if (best < 0 || before(v[i], i, v[best], best)) best = i;
+    }
+    if (best < 0) break;
+    taken[best] = 1;
+    out[cnt++] = best;
+  }
+  return cnt;
+}
+
+// Gates for one token's list (sum G = 1 when norm_topk): sum taken in
+// list order in fp32, then s_e / sum.  Empty slots (idx < 0) get gate 0.
+void gates_for_list(const float* s_row, const int32_t* idx, int k, int norm_topk, float* gate) {
+  float sum = 0.0f;
+  for (int j = 0; j < k; ++j)
+    if (idx[j] >= 0) sum = sum + s_row[idx[j]];
+  for (int j = 0; j < k; ++j) {
+    if (idx[j] < 0) gate[j] = 0.0f;
+    else gate[j] = norm_topk ? s_row[idx[j]] / sum : s_row[idx[j]];
+  }
+}
+
+// F_cost(X) = max_d sum_{e in E_d} x_e * w_e, with w_e = R(e,d)*C~(e,d)
+// already folded into integer ns ticks (O3).  Fills load[d] if given.
+int64_t f_cost(const uint8_t* set, const int64_t* w, const int32_t* part, int E, int D, int64_t* load) {
+  std::vector<int64_t> l(D, 0);
+  for (int e = 0; e < E; ++e)
+    if (set[e]) l[part[e]] += w[e];
+  int64_t m = 0;
+  for (int d = 0; d < D; ++d) m = std::max(m, l[d]);
+  if (load)
+    for (int d = 0; d < D; ++d) load[d] = l[d];
+  return m;
+}
+
+}  // namespace
+
+extern "C" {
+
+// ---------------------------------------------------------------------------
+// O0 router scores ("routing score G(t)_e"; functional form per
+// BASELINE.json configs, reading R1).  logit accumulated in fp64, the activation
+// evaluated in fp64, rounded once to fp32.
+int oracle_scores(const void* x, int x_dtype, const float* Wr, const float* b_logit, int T, int H,
+                  int E, int score_fn, float* s) {
+  std::vector<double> logit(E);
+  for (int t = 0; t < T; ++t) {
+    for (int e = 0; e < E; ++e) {
+      double acc = 0.0;
+      for (int h = 0; h < H; ++h)
+        acc += act_at(x, x_dtype, static_cast<size_t>(t) * H + h) * static_cast<double>(Wr[static_cast<size_t>(e) * H + h]);
+      if (b_logit) acc += b_logit[e];
+      logit[e] = acc;
+    }
+    if (score_fn == SCORE_SIGMOID) {
+      for (int e = 0; e < E; ++e) s[static_cast<size_t>(t) * E + e] = static_cast<float>(1.0 / (1.0 + std::exp(-logit[e])));
+    } else {
+      double mx = logit[0];
+      for (int e = 1; e < E; ++e) mx = std::max(mx, logit[e]);
+      double den = 0.0;
+      for (int e = 0; e < E; ++e) den += std::exp(logit[e] - mx);
+      for (int e = 0; e < E; ++e) s[static_cast<size_t>(t) * E + e] = static_cast<float>(std::exp(logit[e] - mx) / den);
+    }
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O1 route: top-k set K_t and gates; DeepSeek group-limited
+// selection is only named at PAPER.md:291, its form is reading R1:
+//   s' = s + corr_bias (selection only); group score = sum of the two largest s'
+//   in the group; keep topk_group groups; top-k of s' inside them; gate from s.
+int oracle_route(const float* s, const float* corr_bias, int T, int E, int k, int n_group,
+                 int topk_group, int norm_topk, int32_t* idx, float* gate) {
+  if (k > E || k < 1 || n_group < 1 || E % n_group) return -1;
+  int gs = E / n_group;
+  std::vector<float> sp(E), gscore(n_group);
+  std::vector<uint8_t> ok(E);
+  std::vector<int32_t> gsel(n_group);
+  for (int t = 0; t < T; ++t) {
+    const float* sr = s + static_cast<size_t>(t) * E;
+    for (int e = 0; e < E; ++e) sp[e] = corr_bias ? sr[e] + corr_bias[e] : sr[e];
+    std::fill(ok.begin(), ok.end(), 1);
+    if (n_group > 1 && topk_group < n_group) {
+      for (int g = 0; g < n_group; ++g) {
+        int32_t two[2];
+        int c = topk_select(sp.data() + g * gs, nullptr, gs, 2, two);
+        gscore[g] = (c == 2) ? sp[g * gs + two[0]] + sp[g * gs + two[1]] : sp[g * gs + two[0]];
+      }
+      int c = topk_select(gscore.data(), nullptr, n_group, topk_group, gsel.data());
+      std::fill(ok.begin(), ok.end(), 0);
+      for (int j = 0; j < c; ++j)
+        for (int i = 0; i < gs; ++i) ok[gsel[j] * gs + i] = 1;
+    }
+    int32_t* ir = idx + static_cast<size_t>(t) * k;
+    int c = topk_select(sp.data(), ok.data(), E, k, ir);
+    for (int j = c; j < k; ++j) ir[j] = -1;
+    gates_for_list(sr, ir, k, norm_topk, gate + static_cast<size_t>(t) * k);
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O2 activation set and importance: A_act = U_t K_t;
+// I(e) = sum_t G(t)_e held as I_fix = sum_t floor(G * 2^40), an
+// exact, order-independent integer.
+int oracle_importance(const int32_t* idx, const float* gate, int T, int E, int k, uint8_t* act,
+                      int64_t* I_fix) {
+  for (int e = 0; e < E; ++e) { act[e] = 0; I_fix[e] = 0; }
+  for (int t = 0; t < T; ++t)
+    for (int j = 0; j < k; ++j) {
+      int e = idx[static_cast<size_t>(t) * k + j];
+      if (e < 0) continue;
+      act[e] = 1;
+      I_fix[e] += static_cast<int64_t>(std::floor(static_cast<double>(gate[static_cast<size_t>(t) * k + j]) * FIX_ONE));
+    }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O3 costs.  w_e = R(e,d)*C~(e,d) as integer ns: resident ? ticks_resident : ticks_miss
+// (two-tier table, reading R18).
+int oracle_effective_cost(const uint8_t* resident, const int64_t* ticks_resident,
+                          const int64_t* ticks_miss, int E, int64_t* w) {
+  for (int e = 0; e < E; ++e) w[e] = resident[e] ? ticks_resident[e] : ticks_miss[e];
+  return 0;
+}
+
+int64_t oracle_f_cost(const uint8_t* set, const int64_t* w, const int32_t* part, int E, int D,
+                      int64_t* load) {
+  return f_cost(set, w, part, E, D, load);
+}
+
+// C~(e,d) = alpha_d * S_e / B_d + beta_d with slope = alpha_d/B_d in ns
+// per byte and intercept = beta_d in ns; rounded to the nearest integer ns.
+int64_t oracle_cost_ticks(double slope_ns_per_byte, double intercept_ns, int64_t bytes) {
+  return static_cast<int64_t>(std::llround(slope_ns_per_byte * static_cast<double>(bytes) + intercept_ns));
+}
+
+// ---------------------------------------------------------------------------
+// O4 cost-aware pruning.  scalars out:
+//   [0] F_base  [1] F_cost_dense = F_cost(A_act)  [2] F_cost = F_cost(A_trans)
+//   [3] F_imp_fix = sum_{e in A_act \ A_trans} I_fix(e)  [4] |A_act|  [5] |A_must| (step 1)
+//   [6] |A_trans|
+// must[] is the step-1 mandatory set, keep[] is A_trans, load[] = per-partition cost of A_trans.
+int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const float* gate, int T,
+                 int E, int k, const int64_t* w, const int32_t* part, int D, uint8_t* act,
+                 int64_t* I_fix, uint8_t* must, uint8_t* keep, int64_t* load, int64_t* scalars) {
+  oracle_importance(idx, gate, T, E, k, act, I_fix);
+  int n_act = 0;
+  for (int e = 0; e < E; ++e) n_act += act[e];
+
+  // Step 1: mandatory set by mode.
+  std::fill(must, must + E, 0);
+  if (mode == MODE_NONE) {
+    for (int e = 0; e < E; ++e) must[e] = act[e];
+  } else if (mode == MODE_THRESH) {  // I(e) >= theta
+    int64_t thr = static_cast<int64_t>(std::floor(theta * FIX_ONE));
+    for (int e = 0; e < E; ++e) must[e] = act[e] && I_fix[e] >= thr;
+  } else if (mode == MODE_CIR) {  // minimal m* with CIR(m*) >= theta_imp
+    float th = static_cast<float>(theta);
+    for (int t = 0; t < T; ++t) {
+      const int32_t* ir = idx + static_cast<size_t>(t) * k;
+      const float* gr = gate + static_cast<size_t>(t) * k;
+      float pk = 0.0f;
+      for (int j = 0; j < k; ++j)
+        if (ir[j] >= 0) pk = pk + gr[j];
+      float rhs = th * pk;
+      float pm = 0.0f;
+      for (int j = 0; j < k; ++j) {
+        if (ir[j] < 0) break;
+        must[ir[j]] = 1;
+        pm = pm + gr[j];
+        if (pm >= rhs) break;
+      }
+    }
+  } else if (mode == MODE_RANK) {  // budget b experts/token (BASELINE.json config 1)
+    int b = static_cast<int>(theta);
+    for (int t = 0; t < T; ++t)
+      for (int j = 0; j < k - b; ++j) {
+        int e = idx[static_cast<size_t>(t) * k + j];
+        if (e >= 0) must[e] = 1;
+      }
+  } else if (mode == MODE_FRAC) {  // budget p of activated experts (BASELINE.json config 4)
+    std::vector<int> a;
+    for (int e = 0; e < E; ++e)
+      if (act[e]) a.push_back(e);
+    std::sort(a.begin(), a.end(), [&](int x, int y) { return I_fix[x] < I_fix[y] || (I_fix[x] == I_fix[y] && x < y); });
+    int64_t n_cand = static_cast<int64_t>(std::floor(theta * static_cast<double>(n_act)));
+    for (size_t i = 0; i < a.size(); ++i) must[a[i]] = static_cast<int64_t>(i) >= n_cand;
+  } else {
+    return -1;
+  }
+  if ((flags & FLAG_KEEP_TOP1) && mode != MODE_NONE)
+    for (int t = 0; t < T; ++t)
+      if (idx[static_cast<size_t>(t) * k] >= 0) must[idx[static_cast<size_t>(t) * k]] = 1;
+  int n_must = 0;
+  for (int e = 0; e < E; ++e) n_must += must[e];
+
+  // Step 2: F_base = F_cost(A_must).
+  std::vector<int64_t> l(D);
+  int64_t F_base = f_cost(must, w, part, E, D, l.data());
+
+  // Step 3: cost-invariant expansion over A_cand = A_act \ A_must
+  // (reading R3), visited by descending I(e), ties -> lower id (R7), A_must updated
+  // after each promotion.  Only part(e)'s load changes (R5); "= F_base" is "<= F_base"
+  // on integer ticks (R6).
+  for (int e = 0; e < E; ++e) keep[e] = must[e];
+  std::vector<int> cand;
+  for (int e = 0; e < E; ++e)
+    if (act[e] && !must[e]) cand.push_back(e);
+  std::sort(cand.begin(), cand.end(), [&](int x, int y) { return I_fix[x] > I_fix[y] || (I_fix[x] == I_fix[y] && x < y); });
+  for (int e : cand) {
+    if (l[part[e]] + w[e] <= F_base) {
+      keep[e] = 1;
+      l[part[e]] += w[e];
+    }
+  }
+
+  // Step 4: A_trans = A_must after expansion.
+  int64_t F_cost = f_cost(keep, w, part, E, D, load);
+  int64_t F_imp = 0;
+  int n_keep = 0;
+  for (int e = 0; e < E; ++e) {
+    n_keep += keep[e];
+    if (act[e] && !keep[e]) F_imp += I_fix[e];
+  }
+  scalars[0] = F_base;
+  scalars[1] = f_cost(act, w, part, E, D, nullptr);
+  scalars[2] = F_cost;
+  scalars[3] = F_imp;
+  scalars[4] = n_act;
+  scalars[5] = n_must;
+  scalars[6] = n_keep;
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O5 compensation: mask scores outside A_trans, Top-k again.
+// Affected tokens only (reading R14) unless FLAG_COMP_ALL_TOKENS; selection score
+// s' = s + corr_bias, no group limit (R13); exclusion, not numeric zero (R17);
+// min(k, |A_trans|) survivors (R15); gates renormalised over K_final (R16).
+int oracle_compensate(const float* s, const float* corr_bias, const uint8_t* keep, int T, int E,
+                      int k, int norm_topk, int flags, int32_t* idx, float* gate) {
+  std::vector<float> sp(E);
+  for (int t = 0; t < T; ++t) {
+    int32_t* ir = idx + static_cast<size_t>(t) * k;
+    bool affected = (flags & FLAG_COMP_ALL_TOKENS) != 0;
+    for (int j = 0; j < k; ++j)
+      if (ir[j] >= 0 && !keep[ir[j]]) affected = true;
+    if (!affected) continue;
+    const float* sr = s + static_cast<size_t>(t) * E;
+    for (int e = 0; e < E; ++e) sp[e] = corr_bias ? sr[e] + corr_bias[e] : sr[e];
+    int c = topk_select(sp.data(), keep, E, k, ir);
+    for (int j = c; j < k; ++j) ir[j] = -1;
+    gates_for_list(sr, ir, k, norm_topk, gate + static_cast<size_t>(t) * k);
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O6 compaction: experts with >= 1 token in ascending id, tokens ascending inside
+// an expert (BASELINE.json north_star (1): "compacted per-expert token list").
+// tok[i], slot[i], wt[i] give token, position in that token's list, and gate.
+int oracle_compact(const int32_t* idx, const float* gate, int T, int E, int k, int32_t* n_run,
+                   int32_t* expert_ids, int32_t* offs, int32_t* tok, int32_t* slot, float* wt) {
+  int r = 0, n = 0;
+  offs[0] = 0;
+  for (int e = 0; e < E; ++e) {
+    int before_n = n;
+    for (int t = 0; t < T; ++t)
+      for (int j = 0; j < k; ++j)
+        if (idx[static_cast<size_t>(t) * k + j] == e) {
+          tok[n] = t;
+          slot[n] = j;
+          wt[n] = gate[static_cast<size_t>(t) * k + j];
+          ++n;
+        }
+    if (n > before_n) {
+      expert_ids[r] = e;
+      offs[++r] = n;
+    }
+  }
+  *n_run = r;
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O7 one expert on one token ("E_e(t)"; SwiGLU form per BASELINE.json):
+//   g = W_g x, u = W_u x, h = g / (1 + exp(-g)) * u, o = W_d h.   All fp64.
+// W_g, W_u are [I,H]; W_d is [H,I]; optional 128x128 block scales for e4m3.
+int oracle_expert_ffn(const void* x_row, int x_dtype, const void* Wg, const void* Wu, const void* Wd,
+                      int w_dtype, const float* sg, const float* su, const float* sd, int H, int I,
+                      double* o) {
+  Mat G{Wg, w_dtype, sg, I, H}, U{Wu, w_dtype, su, I, H}, Dn{Wd, w_dtype, sd, H, I};
+  std::vector<double> xv(H), hv(I);
+  for (int h = 0; h < H; ++h) xv[h] = act_at(x_row, x_dtype, h);
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < I; ++i) {
+    double g = 0.0, u = 0.0;
+    for (int h = 0; h < H; ++h) {
+      g += G.at(i, h) * xv[h];
+      u += U.at(i, h) * xv[h];
+    }
+    hv[i] = g / (1.0 + std::exp(-g)) * u;
+  }
+#pragma omp parallel for schedule(static)
+  for (int r = 0; r < H; ++r) {
+    double acc = 0.0;
+    for (int i = 0; i < I; ++i) acc += Dn.at(r, i) * hv[i];
+    o[r] = acc;
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O8 combine over a list of tokens:
+//   y_t = routed_scale * sum_{e in K_final} G(t)_e * E_e(t) + sum_{shared} E_sh(t)
+// Weight tables are arrays of E+S pointers (routed experts first, then shared);
+// a null entry may only be hit if no listed token uses that expert.  y is
+// [n_tok, H] fp64, unrounded.  Shared experts: gate 1, every token (reading R21).
+int oracle_moe_tokens(const void* x, int x_dtype, const int32_t* tokens, int n_tok, const int32_t* idx,
+                      const float* gate, int k, const void* const* Wg, const void* const* Wu,
+                      const void* const* Wd, int w_dtype, const float* const* sg,
+                      const float* const* su, const float* const* sd, int E, int S, int H, int I,
+                      double routed_scale, double* y) {
+  std::vector<double> o(H);
+  size_t xbytes = x_dtype == DT_F32 ? 4 : 2;
+  for (int n = 0; n < n_tok; ++n) {
+    int t = tokens[n];
+    const char* xr = static_cast<const char*>(x) + static_cast<size_t>(t) * H * xbytes;
+    double* yr = y + static_cast<size_t>(n) * H;
+    for (int r = 0; r < H; ++r) yr[r] = 0.0;
+    for (int j = 0; j < k; ++j) {
+      int e = idx[static_cast<size_t>(t) * k + j];
+      if (e < 0) continue;
+      if (!Wg[e] || !Wu[e] || !Wd[e]) return -2;
+      oracle_expert_ffn(xr, x_dtype, Wg[e], Wu[e], Wd[e], w_dtype, sg ? sg[e] : nullptr,
+                        su ? su[e] : nullptr, sd ? sd[e] : nullptr, H, I, o.data());
+      double g = gate[static_cast<size_t>(t) * k + j];
+      for (int r = 0; r < H; ++r) yr[r] += g * o[r];
+    }
+    for (int r = 0; r < H; ++r) yr[r] *= routed_scale;
+    for (int sh = 0; sh < S; ++sh) {
+      int e = E + sh;
+      if (!Wg[e] || !Wu[e] || !Wd[e]) return -2;
+      oracle_expert_ffn(xr, x_dtype, Wg[e], Wu[e], Wd[e], w_dtype, sg ? sg[e] : nullptr,
+                        su ? su[e] : nullptr, sd ? sd[e] : nullptr, H, I, o.data());
+      for (int r = 0; r < H; ++r) yr[r] += o[r];
+    }
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------
+// O9 calibration fit: ordinary least squares of t_i on S_i.
+int oracle_fit(const double* S, const double* t, int n, double* slope, double* intercept, double* r2) {
+  if (n < 2) return -1;
+  double ms = 0, mt = 0;
+  for (int i = 0; i < n; ++i) { ms += S[i]; mt += t[i]; }
+  ms /= n; mt /= n;
+  double sxx = 0, sxy = 0, syy = 0;
+  for (int i = 0; i < n; ++i) {
+    sxx += (S[i] - ms) * (S[i] - ms);
+    sxy += (S[i] - ms) * (t[i] - mt);
+    syy += (t[i] - mt) * (t[i] - mt);
+  }
+  if (sxx == 0) return -1;
+  *slope = sxy / sxx;
+  *intercept = mt - *slope * ms;
+  double sse = 0;
+  for (int i = 0; i < n; ++i) {
+    double r = t[i] - (*slope * S[i] + *intercept);
+    sse += r * r;
+  }
+  *r2 = syy > 0 ? 1.0 - sse / syy : 1.0;
+  return 0;
+}
+
+double oracle_e4m3_value(int code) { return e4m3_value(static_cast<uint8_t>(code)); }
+
+}  // extern "C"
