@@ -1,0 +1,221 @@
+/* caee.h — C ABI of libcaee: the CAEE (Cost-Aware Expert Execution) per-layer MoE
+ * decode hot path on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are to /root/reference/PAPER.md ("PAPER.md:<line>") and to the readings
+ * R1..R29 listed in DESIGN.md §3.  The paper's "devices" are logical expert
+ * partitions on one GPU whose costs are aggregated by max.
+ *
+ * Conventions
+ *  - "dev" pointers are CUDA device memory on the context's device; "host" pointers
+ *    are ordinary host memory read during the call; "pinned" is page-locked host memory.
+ *  - Matrices are row-major and dense.  bf16 is the upper 16 bits of an IEEE fp32;
+ *    e4m3 is OCP FP8 E4M3 (no infinities, max 448) with one fp32 scale per 128x128
+ *    block, scales stored row-major [ceil(rows/128), ceil(cols/128)].
+ *  - Ownership: the caller owns every buffer it passes.  Activations, scores and
+ *    outputs are borrowed for the duration of the enqueued work; router weights,
+ *    expert weights (unless packed, see caee_set_weights) and tables are borrowed
+ *    until caee_destroy or the next caee_set_* call for the same item.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *    caee_route, caee_route_from_scores, caee_prune, caee_moe_forward and
+ *    caee_moe_forward_from_scores only enqueue work: no host synchronisation, no
+ *    allocation.  caee_calibrate_cost and the caee_set_* calls synchronise.
+ *  - Errors: every call returns CAEE_OK (0) or a negative code; nothing throws or
+ *    aborts across the ABI.  caee_last_error gives a human-readable reason.
+ *    A CUDA failure is sticky for the context (CAEE_ECUDA from then on).
+ *  - There is no CPU fallback: on a device that is not compute capability 10.x
+ *    caee_create fails with CAEE_EUNSUPPORTED.
+ *  - Determinism: idx, gate, keep/must masks, the compacted lists and all F_* values are
+ *    deterministic functions of the fp32 scores; y is deterministic as well (the
+ *    combine sums each token's experts in list order).
+ */
+#ifndef CAEE_H_
+#define CAEE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct caee_ctx caee_ctx; /* opaque; one per MoE layer */
+typedef int32_t caee_status;
+
+enum {
+  CAEE_OK = 0,
+  CAEE_EINVAL = -1,       /* null pointer, negative size, k > E, E % n_group != 0, theta out of range ... */
+  CAEE_ESHAPE = -2,       /* T > max_tokens, shape the chosen expert kernel cannot tile */
+  CAEE_EDTYPE = -3,       /* unknown / unsupported dtype combination */
+  CAEE_ENOMEM = -4,       /* device or host allocation failed */
+  CAEE_ECUDA = -5,        /* CUDA runtime error (sticky) */
+  CAEE_ESTATE = -6,       /* call made before the state it needs was set */
+  CAEE_EUNSUPPORTED = -7  /* not an sm_100 device */
+};
+
+enum { CAEE_F32 = 0, CAEE_BF16 = 1, CAEE_E4M3 = 2 };
+enum { CAEE_SCORE_SOFTMAX = 0, CAEE_SCORE_SIGMOID = 1 };
+
+/* How the mandatory set A_must of step 1 is formed. */
+enum {
+  CAEE_PRUNE_NONE = 0,   /* A_must = A_act: nothing can be pruned                                    */
+  CAEE_PRUNE_THRESH = 1, /* I(e) = sum_t G(t)_e >= theta        (on-device setup)  */
+  CAEE_PRUNE_CIR = 2,    /* per token, minimal m* with CIR(m*) >= theta (offloading)    */
+  CAEE_PRUNE_RANK = 3,   /* per token, the first k - theta of K_t    (BASELINE.json config 1 budget) */
+  CAEE_PRUNE_FRAC = 4    /* all but the floor(theta*|A_act|) least important (config 4 budget)       */
+};
+enum {
+  CAEE_COMP_ALL_TOKENS = 1, /* re-select every token, not only those that lost an expert (R14)       */
+  CAEE_KEEP_TOP1 = 2        /* every token's first expert is mandatory (R23)                          */
+};
+enum { CAEE_KERNEL_AUTO = 0, CAEE_KERNEL_SIMT = 1, CAEE_KERNEL_UMMA = 2 };
+
+typedef struct caee_layer_desc {
+  int32_t H;             /* hidden size                                                          */
+  int32_t I;             /* SwiGLU intermediate size                                             */
+  int32_t E;             /* routed experts, 1..512                                               */
+  int32_t S;             /* shared experts (run on every token, gate 1, never pruned; R21)       */
+  int32_t k;             /* experts per token, 1..min(E,32)                                      */
+  int32_t n_group;       /* router groups, divides E; 1 = ungrouped                              */
+  int32_t topk_group;    /* groups kept per token, 1..n_group; topk_group*(E/n_group) >= k       */
+  int32_t score_fn;      /* CAEE_SCORE_*                                                         */
+  int32_t norm_topk;     /* 1: G = s/sum_{K_t} s; 0: G = s                          */
+  float routed_scale;    /* factor on the routed sum in the combine (R2)                         */
+  int32_t act_dtype;     /* CAEE_F32 or CAEE_BF16: dtype of x and y                              */
+  int32_t w_dtype;       /* CAEE_F32, CAEE_BF16 or CAEE_E4M3: dtype of expert weights            */
+  int32_t D;             /* expert partitions, 1..64                                             */
+  int32_t max_tokens;    /* largest T any call will pass; scratch is sized from it               */
+  int32_t expert_kernel; /* CAEE_KERNEL_*: AUTO = UMMA (tcgen05) for bf16/e4m3, SIMT for fp32     */
+  int32_t device;        /* CUDA device ordinal, -1 = current device                             */
+} caee_layer_desc;
+
+/* Per-expert weight pointers: host arrays of E+S entries, routed experts first, then the
+ * shared ones.  gate/up: [I,H]; down: [H,I]; *_scale (e4m3 only, else may be NULL):
+ * [ceil(rows/128), ceil(cols/128)] fp32.  Entries point to device memory, or, where
+ * resident[e] == 0 (caee_set_residency), to pinned host memory. */
+typedef struct caee_expert_weights {
+  const void* const* gate;
+  const void* const* up;
+  const void* const* down;
+  const float* const* gate_scale;
+  const float* const* up_scale;
+  const float* const* down_scale;
+} caee_expert_weights;
+
+typedef struct caee_prune_params {
+  int32_t mode;  /* CAEE_PRUNE_*                                                                  */
+  int32_t flags; /* CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1                                         */
+  double theta;  /* THRESH: theta in gate units (sum G = 1); CIR: theta_imp in (0,1];
+                    RANK: budget b in 0..k; FRAC: p in [0,1]                                     */
+} caee_prune_params;
+
+/* Optional device outputs of caee_prune; any pointer may be NULL.  scalars[8] =
+ * { F_base, F_cost_dense = F_cost(A_act), F_cost = F_cost(A_trans), F_imp (2^-40 units),
+ *   |A_act|, |A_must| after step 1, |A_trans|, n_run }. */
+typedef struct caee_prune_out {
+  uint8_t* act;         /* dev [E]   A_act                                                        */
+  uint8_t* must;        /* dev [E]   A_must of step 1                                             */
+  uint8_t* keep;        /* dev [E]   A_trans                                                      */
+  int64_t* importance;  /* dev [E]   I(e) in units of 2^-40                                       */
+  int64_t* load;        /* dev [D]   per-partition cost of A_trans                                */
+  int64_t* scalars;     /* dev [8]                                                                */
+  int32_t* n_run;       /* dev [1]   experts that receive >= 1 token after compensation           */
+  int32_t* expert_ids;  /* dev [E]   those experts, ascending                                     */
+  int32_t* offs;        /* dev [E+1] start of each expert's token list                            */
+  int32_t* tok;         /* dev [T*k] token of each list entry, ascending inside an expert         */
+  int32_t* slot;        /* dev [T*k] position of that expert in the token's K_final               */
+  float* wt;            /* dev [T*k] gate G(t)_e of the entry                                     */
+} caee_prune_out;
+
+/* Written by caee_moe_forward when stats != NULL (device memory). */
+typedef struct caee_fwd_stats {
+  int64_t F_base, F_cost_dense, F_cost, F_imp;
+  int64_t weight_bytes; /* expert-weight bytes the expert kernel streamed (surviving + shared)   */
+  int64_t h2d_bytes;    /* bytes fetched from pinned host memory for non-resident survivors      */
+  int32_t n_act, n_keep, n_run, n_fetch;
+  int64_t load[64];     /* per-partition cost of A_trans (the quantity of PAPER.md Fig. 10)       */
+} caee_fwd_stats;
+
+typedef struct caee_calib_opts {
+  int32_t n_sizes;      /* sizes to time per tier, 2..16 (0 = default 6)                          */
+  int32_t iters;        /* timed repetitions per size (0 = default 10), median is used            */
+  int64_t min_bytes;    /* smallest transfer (0 = default 4 MiB)                                  */
+  int64_t max_bytes;    /* largest transfer (0 = one expert's weight bytes)                       */
+  int32_t apply;        /* 1: fill the context's cost table from the fits                         */
+  int32_t reserved;
+} caee_calib_opts;
+
+/* t = slope*bytes + intercept, the fitted form of C~(e,d) = alpha_d*S_e/B_d + beta_d
+ * (PAPER.md:139): slope = alpha_d/B_d, intercept = beta_d. */
+typedef struct caee_cost_fit {
+  double slope_ns_per_byte;
+  double intercept_ns;
+  double r2;
+  double gbytes_per_s;  /* 1/slope, the effective bandwidth                                       */
+  int32_t n_points;
+  int32_t valid;        /* 0 if the tier could not be measured                                    */
+} caee_cost_fit;
+
+/* Lifecycle.  caee_create validates the descriptor and allocates all scratch. */
+caee_status caee_create(const caee_layer_desc* desc, caee_ctx** out);
+caee_status caee_destroy(caee_ctx* ctx);
+/* Reason for the last failure on ctx (or, with ctx == NULL, of the last failed caee_create
+ * on this thread).  The string is owned by the library and valid until the next call. */
+const char* caee_last_error(const caee_ctx* ctx);
+
+/* Router parameters (dev, fp32).  W_r [E,H]; b_logit [E] or NULL (added to the logit);
+ * corr_bias [E] or NULL (added to the score for SELECTION only, R1). */
+caee_status caee_set_router(caee_ctx* ctx, const float* W_r, const float* b_logit, const float* corr_bias);
+/* Expert weights.  pack != 0: the library repacks each expert once into its own tile-major
+ * copy (device memory for resident experts, pinned host memory otherwise) and no longer
+ * refers to the caller's buffers afterwards.  The UMMA kernel requires pack != 0.
+ * Call caee_set_residency first when some experts live in host memory. */
+caee_status caee_set_weights(caee_ctx* ctx, const caee_expert_weights* w, int32_t pack);
+/* E_d of PAPER.md:127 as part_of_expert[e] in 0..D-1 (host).  Default: contiguous blocks. */
+caee_status caee_set_partitions(caee_ctx* ctx, const int32_t* part_of_expert, int32_t D);
+/* R(e,d) of PAPER.md:129-135 as resident[e] in {0,1} (host).  Default: all resident. */
+caee_status caee_set_residency(caee_ctx* ctx, const uint8_t* resident);
+/* C~(e,d) in integer ns for each tier (host, [E] each): the cost of expert e is
+ * resident[e] ? ticks_resident[e] : ticks_miss[e]  (R18).  ticks_miss may be NULL if all
+ * experts are resident. */
+caee_status caee_set_cost_table(caee_ctx* ctx, const int64_t* ticks_resident, const int64_t* ticks_miss);
+
+/* Offline calibration: times streaming reads of HBM (fit[0]) and
+ * pinned-host -> device copies (fit[1]) at several sizes, least-squares fits
+ * t = slope*bytes + intercept, and with opts->apply fills the cost table with
+ * round(slope*S_e + intercept) ns per tier.  Blocking.  opts may be NULL (defaults, apply=1). */
+caee_status caee_calibrate_cost(caee_ctx* ctx, const caee_calib_opts* opts, caee_cost_fit out_fit[2]);
+
+/* S0+S1: scores s = act(x W_r^T + b_logit) and the top-k set K_t with gates.
+ * x dev [T,H] act dtype; scores dev [T,E] fp32 or NULL; idx dev [T,k] int32 in descending
+ * selection score; gate dev [T,k] fp32. */
+caee_status caee_route(caee_ctx* ctx, const void* x, int32_t T, float* scores, int32_t* idx, float* gate,
+                       void* stream);
+/* S1 only, on caller-supplied scores (parity entry point). */
+caee_status caee_route_from_scores(caee_ctx* ctx, const float* scores, int32_t T, int32_t* idx, float* gate,
+                                   void* stream);
+/* S2-S6: activation set, importance, cost-aware pruning, compensation
+ * and compaction.  scores dev [T,E]; idx/gate dev [T,k] in/out: on return
+ * they hold K_final and its gates (empty slots: idx -1, gate 0).  p == NULL or mode NONE
+ * prunes nothing.  out may be NULL. */
+caee_status caee_prune(caee_ctx* ctx, const caee_prune_params* p, const float* scores, int32_t T, int32_t* idx,
+                       float* gate, const caee_prune_out* out, void* stream);
+/* The whole layer: route -> prune (p != NULL) -> fetch of surviving non-resident experts on
+ * a side stream -> grouped SwiGLU FFN over the surviving experts only -> combine
+ *   y_t = routed_scale * sum_{e in K_final} G(t)_e E_e(t) + sum_shared E_sh(t).
+ * x, y dev [T,H] act dtype; stats dev or NULL. */
+caee_status caee_moe_forward(caee_ctx* ctx, const void* x, int32_t T, const caee_prune_params* p, void* y,
+                             caee_fwd_stats* stats, void* stream);
+/* Same, with the router's scores supplied by the caller (dev [T,E] fp32) instead of
+ * computed from x: used to compare against the oracle without near-tie routing flips. */
+caee_status caee_moe_forward_from_scores(caee_ctx* ctx, const void* x, const float* scores, int32_t T,
+                                         const caee_prune_params* p, void* y, caee_fwd_stats* stats,
+                                         void* stream);
+/* K_final of the last forward call on this context (dev -> dev copy, enqueued on stream). */
+caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gate, void* stream);
+
+/* Library / build identification, e.g. "caee-b200 0.1 sm_100a". */
+const char* caee_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAEE_H_ */

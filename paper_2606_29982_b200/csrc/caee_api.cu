@@ -1,0 +1,467 @@
+// caee_api.cu — the C ABI of include/caee.h: context, validation, tables, and the enqueue
+// sequences of the per-layer hot path.  No torch types, no exceptions across the boundary.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "caee_internal.cuh"
+
+static thread_local std::string g_create_err;
+
+caee_status caee_fail(caee_ctx* c, caee_status code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf;
+  else g_create_err = buf;
+  return code;
+}
+
+caee_status caee_check_cuda(caee_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return CAEE_OK;
+  if (c) c->cuda_failed = true;
+  if (e == cudaErrorMemoryAllocation) {
+    cudaGetLastError();
+    return caee_fail(c, CAEE_ENOMEM, "%s: %s", what, cudaGetErrorString(e));
+  }
+  return caee_fail(c, CAEE_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+namespace {
+
+template <typename T>
+caee_status dev_alloc(caee_ctx* c, T** p, size_t n) {
+  CAEE_CUDA(c, cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (n ? n : 1)));
+  return CAEE_OK;
+}
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    cudaGetDevice(&prev);
+    if (prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+caee_status validate_desc(const caee_layer_desc* d) {
+  if (!d) return caee_fail(nullptr, CAEE_EINVAL, "desc is NULL");
+  if (d->H < 8 || d->I < 8 || d->H % 8 || d->I % 8) return caee_fail(nullptr, CAEE_ESHAPE, "H and I must be positive multiples of 8");
+  if (d->E < 1 || d->E > CAEE_MAX_E) return caee_fail(nullptr, CAEE_EINVAL, "E must be in 1..%d", CAEE_MAX_E);
+  if (d->S < 0 || d->S > 16) return caee_fail(nullptr, CAEE_EINVAL, "S must be in 0..16");
+  if (d->k < 1 || d->k > d->E || d->k > 32) return caee_fail(nullptr, CAEE_EINVAL, "k must be in 1..min(E,32)");
+  if (d->n_group < 1 || d->n_group > 32 || d->E % d->n_group) return caee_fail(nullptr, CAEE_EINVAL, "n_group must divide E and be <= 32");
+  if (d->topk_group < 1 || d->topk_group > d->n_group) return caee_fail(nullptr, CAEE_EINVAL, "topk_group must be in 1..n_group");
+  if ((long long)d->topk_group * (d->E / d->n_group) < d->k) return caee_fail(nullptr, CAEE_EINVAL, "topk_group*(E/n_group) < k");
+  if (d->score_fn != CAEE_SCORE_SOFTMAX && d->score_fn != CAEE_SCORE_SIGMOID) return caee_fail(nullptr, CAEE_EINVAL, "unknown score_fn");
+  if (d->act_dtype != CAEE_F32 && d->act_dtype != CAEE_BF16) return caee_fail(nullptr, CAEE_EDTYPE, "act_dtype must be F32 or BF16");
+  if (d->w_dtype != CAEE_F32 && d->w_dtype != CAEE_BF16 && d->w_dtype != CAEE_E4M3) return caee_fail(nullptr, CAEE_EDTYPE, "unknown w_dtype");
+  if (d->D < 1 || d->D > CAEE_MAX_D) return caee_fail(nullptr, CAEE_EINVAL, "D must be in 1..%d", CAEE_MAX_D);
+  if (d->max_tokens < 1 || d->max_tokens > 65536) return caee_fail(nullptr, CAEE_EINVAL, "max_tokens must be in 1..65536");
+  if (d->expert_kernel < CAEE_KERNEL_AUTO || d->expert_kernel > CAEE_KERNEL_UMMA) return caee_fail(nullptr, CAEE_EINVAL, "unknown expert_kernel");
+  if (!(d->routed_scale == d->routed_scale)) return caee_fail(nullptr, CAEE_EINVAL, "routed_scale is NaN");
+  return CAEE_OK;
+}
+
+caee_status validate_prune(caee_ctx* c, const caee_prune_params* p) {
+  if (!p) return CAEE_OK;
+  switch (p->mode) {
+    case CAEE_PRUNE_NONE: break;
+    case CAEE_PRUNE_THRESH:
+      if (!(p->theta >= 0.0) || p->theta > 1e6) return caee_fail(c, CAEE_EINVAL, "THRESH: theta must be in [0, 1e6]");
+      break;
+    case CAEE_PRUNE_CIR:
+      if (!(p->theta > 0.0 && p->theta <= 1.0)) return caee_fail(c, CAEE_EINVAL, "CIR: theta_imp must be in (0,1]");
+      break;
+    case CAEE_PRUNE_RANK:
+      if (!(p->theta >= 0.0 && p->theta <= c->d.k) || p->theta != (double)(int)p->theta)
+        return caee_fail(c, CAEE_EINVAL, "RANK: budget must be an integer in 0..k");
+      break;
+    case CAEE_PRUNE_FRAC:
+      if (!(p->theta >= 0.0 && p->theta <= 1.0)) return caee_fail(c, CAEE_EINVAL, "FRAC: p must be in [0,1]");
+      break;
+    default: return caee_fail(c, CAEE_EINVAL, "unknown prune mode %d", p->mode);
+  }
+  if (p->flags & ~(CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1)) return caee_fail(c, CAEE_EINVAL, "unknown prune flags");
+  return CAEE_OK;
+}
+
+caee_status upload_costs(caee_ctx* c) {
+  const int E = c->d.E;
+  std::vector<int64_t> w(E);
+  for (int e = 0; e < E; ++e) w[e] = c->resident_h[e] ? c->ticks_res_h[e] : c->ticks_miss_h[e];
+  CAEE_CUDA(c, cudaMemcpy(c->w_eff, w.data(), sizeof(int64_t) * E, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->resident, c->resident_h.data(), E, cudaMemcpyHostToDevice));
+  return CAEE_OK;
+}
+
+caee_status check_call(caee_ctx* c, int T) {
+  if (!c) return CAEE_EINVAL;
+  if (c->cuda_failed) return CAEE_ECUDA;
+  if (T < 0) return caee_fail(c, CAEE_EINVAL, "T < 0");
+  if (T > c->d.max_tokens) return caee_fail(c, CAEE_ESHAPE, "T=%d exceeds max_tokens=%d", T, c->d.max_tokens);
+  return CAEE_OK;
+}
+
+caee_status after_launch(caee_ctx* c, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? CAEE_OK : caee_check_cuda(c, e, what);
+}
+
+void free_all(caee_ctx* c) {
+  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->scores, c->idx,
+                  c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
+                  c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
+                  c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
+                  c->packed.dev_ptrs};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  for (size_t e = 0; e < c->packed.base.size(); ++e) {
+    if (!c->packed.base[e]) continue;
+    if (c->packed.on_host[e]) cudaFreeHost(c->packed.base[e]);
+    else cudaFree(c->packed.base[e]);
+  }
+  if (c->side_stream) cudaStreamDestroy(c->side_stream);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
+}
+
+caee_status create_impl(caee_ctx* c) {
+  const caee_layer_desc& d = c->d;
+  const size_t Tm = d.max_tokens, E = d.E, k = d.k, S = d.S;
+  c->ksplit_max = d.H / 256 > 0 ? d.H / 256 : 1;
+  size_t prow = 1;
+  for (int T = 1; T <= d.max_tokens; ++T) prow = std::max(prow, (size_t)caee_router_ksplit(c, T) * T);
+  caee_status rc;
+#define A(ptr, n) if ((rc = dev_alloc(c, &(ptr), (n))) != CAEE_OK) return rc
+  A(c->part, E); A(c->resident, E); A(c->w_eff, E);
+  A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
+  A(c->partial, prow * E); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
+  A(c->act, E); A(c->must, E); A(c->keep, E); A(c->I_fix, E); A(c->load, CAEE_MAX_D); A(c->scalars, 8);
+  c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS + S * ((Tm + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS));
+  A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
+  A(c->wl.ent_tok, Tm * (k + S)); A(c->wl.ent_slot, Tm * k); A(c->wl.ent_wt, Tm * k); A(c->wl.ent_dst, Tm * (k + S));
+  A(c->wl.run_expert, c->wl.max_runs); A(c->wl.run_start, c->wl.max_runs); A(c->wl.run_n, c->wl.max_runs);
+  A(c->wl.run_hrow, c->wl.max_runs); A(c->wl.meta, 16); A(c->wl.sched, 2 + c->wl.max_runs);
+  c->h_rows_cap = Tm * k + 15 * std::min(E, Tm * k) + S * (Tm + 15) + 16;
+  if (c->kernel == CAEE_KERNEL_SIMT) { A(c->hbuf_f32, c->h_rows_cap * d.I); }
+  else { A(c->hbuf_b16, c->h_rows_cap * d.I); }
+  A(c->obuf, Tm * (k + S) * d.H);
+#undef A
+  CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
+  CAEE_CUDA(c, cudaMemset(c->scalars, 0, sizeof(int64_t) * 8));
+  CAEE_CUDA(c, cudaMemset(c->load, 0, sizeof(int64_t) * CAEE_MAX_D));
+  // defaults: contiguous partitions, everything resident, unit costs
+  c->part_h.resize(E); c->resident_h.assign(E, 1); c->ticks_res_h.assign(E, 1); c->ticks_miss_h.assign(E, 1);
+  const int per = (int)((E + d.D - 1) / d.D);
+  for (size_t e = 0; e < E; ++e) c->part_h[e] = (int32_t)(e / per);
+  CAEE_CUDA(c, cudaMemcpy(c->part, c->part_h.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  if ((rc = upload_costs(c)) != CAEE_OK) return rc;
+  CAEE_CUDA(c, cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking));
+  CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+  CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+  return CAEE_OK;
+}
+
+// route -> [prune + compensate] -> work list.  scores_in == NULL: compute scores from x.
+caee_status enqueue_decisions(caee_ctx* c, const void* x, const float* scores_in, int T, const caee_prune_params* p,
+                              int32_t* idx, float* gate, float* scores_out, bool do_route, cudaStream_t st) {
+  const float* scores = scores_in;
+  if (T > 0 && do_route) {
+    if (!scores_in) {
+      int ks = caee_router_ksplit(c, T);
+      caee_launch_router_logits(c, x, T, ks, st);
+      caee_launch_route_topk(c, nullptr, ks, T, scores_out ? scores_out : c->scores, idx, gate, st);
+      scores = scores_out ? scores_out : c->scores;
+    } else {
+      caee_launch_route_topk(c, scores_in, 0, T, nullptr, idx, gate, st);
+    }
+  }
+  const int mode = p ? p->mode : CAEE_PRUNE_NONE;
+  if (p) {
+    caee_launch_prune(c, mode, p->flags, p->theta, T, idx, gate, st);
+    if (mode != CAEE_PRUNE_NONE && T > 0) caee_launch_compensate(c, p->flags, scores, T, idx, gate, st);
+  }
+  caee_launch_worklist(c, T, idx, gate, st);
+  return after_launch(c, "decision kernels");
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* caee_version(void) { return "caee-b200 0.1 sm_100a"; }
+
+const char* caee_last_error(const caee_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+caee_status caee_create(const caee_layer_desc* desc, caee_ctx** out) {
+  if (!out) return caee_fail(nullptr, CAEE_EINVAL, "out is NULL");
+  *out = nullptr;
+  caee_status rc = validate_desc(desc);
+  if (rc != CAEE_OK) return rc;
+  int dev = desc->device;
+  if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return caee_fail(nullptr, CAEE_EUNSUPPORTED, "no CUDA device: this library has no CPU fallback");
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return caee_fail(nullptr, CAEE_EUNSUPPORTED, "cannot query CUDA device %d: this library has no CPU fallback", dev);
+  }
+  if (prop.major != 10) return caee_fail(nullptr, CAEE_EUNSUPPORTED, "device %d is sm_%d%d; libcaee is built for sm_100a only", dev, prop.major, prop.minor);
+  caee_ctx* c = new (std::nothrow) caee_ctx();
+  if (!c) return caee_fail(nullptr, CAEE_ENOMEM, "host allocation failed");
+  c->d = *desc;
+  c->d.device = dev;
+  c->device = dev;
+  c->num_sms = prop.multiProcessorCount;
+  c->wl = caee_worklist{};
+  c->kernel = desc->expert_kernel == CAEE_KERNEL_AUTO ? (desc->w_dtype == CAEE_F32 ? CAEE_KERNEL_SIMT : CAEE_KERNEL_UMMA)
+                                                       : desc->expert_kernel;
+  if (c->kernel == CAEE_KERNEL_UMMA) {
+    std::string why;
+    rc = caee_umma_supported(c, &why);
+    if (rc != CAEE_OK) {
+      g_create_err = why;
+      delete c;
+      return rc;
+    }
+  }
+  DeviceGuard g(dev);
+  rc = create_impl(c);
+  if (rc != CAEE_OK) {
+    g_create_err = c->err;
+    free_all(c);
+    delete c;
+    return rc;
+  }
+  *out = c;
+  return CAEE_OK;
+}
+
+caee_status caee_destroy(caee_ctx* c) {
+  if (!c) return CAEE_EINVAL;
+  DeviceGuard g(c->device);
+  cudaDeviceSynchronize();
+  free_all(c);
+  delete c;
+  return CAEE_OK;
+}
+
+caee_status caee_set_router(caee_ctx* c, const float* W_r, const float* b_logit, const float* corr_bias) {
+  if (!c) return CAEE_EINVAL;
+  if (!W_r) return caee_fail(c, CAEE_EINVAL, "W_r is NULL");
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  c->Wr = W_r; c->b_logit = b_logit; c->corr_bias = corr_bias; c->have_router = true;
+  return CAEE_OK;
+}
+
+caee_status caee_set_partitions(caee_ctx* c, const int32_t* part, int32_t D) {
+  if (!c) return CAEE_EINVAL;
+  if (!part) return caee_fail(c, CAEE_EINVAL, "part_of_expert is NULL");
+  if (D != c->d.D) return caee_fail(c, CAEE_EINVAL, "D=%d differs from the descriptor's D=%d", D, c->d.D);
+  for (int e = 0; e < c->d.E; ++e)
+    if (part[e] < 0 || part[e] >= D) return caee_fail(c, CAEE_EINVAL, "part_of_expert[%d]=%d out of range", e, part[e]);
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  c->part_h.assign(part, part + c->d.E);
+  CAEE_CUDA(c, cudaMemcpy(c->part, part, sizeof(int32_t) * c->d.E, cudaMemcpyHostToDevice));
+  return CAEE_OK;
+}
+
+caee_status caee_set_residency(caee_ctx* c, const uint8_t* resident) {
+  if (!c) return CAEE_EINVAL;
+  if (!resident) return caee_fail(c, CAEE_EINVAL, "resident is NULL");
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  for (int e = 0; e < c->d.E; ++e) c->resident_h[e] = resident[e] ? 1 : 0;
+  return upload_costs(c);
+}
+
+caee_status caee_set_cost_table(caee_ctx* c, const int64_t* ticks_resident, const int64_t* ticks_miss) {
+  if (!c) return CAEE_EINVAL;
+  if (!ticks_resident) return caee_fail(c, CAEE_EINVAL, "ticks_resident is NULL");
+  for (int e = 0; e < c->d.E; ++e) {
+    if (ticks_resident[e] < 0 || (ticks_miss && ticks_miss[e] < 0)) return caee_fail(c, CAEE_EINVAL, "negative cost for expert %d", e);
+    if (ticks_resident[e] > (1LL << 40) || (ticks_miss && ticks_miss[e] > (1LL << 40))) return caee_fail(c, CAEE_EINVAL, "cost for expert %d exceeds 2^40 ns", e);
+  }
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  c->ticks_res_h.assign(ticks_resident, ticks_resident + c->d.E);
+  if (ticks_miss) c->ticks_miss_h.assign(ticks_miss, ticks_miss + c->d.E);
+  else c->ticks_miss_h = c->ticks_res_h;
+  c->have_cost = true;
+  return upload_costs(c);
+}
+
+caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t pack) {
+  if (!c) return CAEE_EINVAL;
+  if (!w || !w->gate || !w->up || !w->down) return caee_fail(c, CAEE_EINVAL, "weight pointer tables are NULL");
+  const int n = c->d.E + c->d.S;
+  const bool fp8 = c->d.w_dtype == CAEE_E4M3;
+  if (fp8 && (!w->gate_scale || !w->up_scale || !w->down_scale)) return caee_fail(c, CAEE_EINVAL, "e4m3 weights need block scales");
+  for (int e = 0; e < n; ++e) {
+    if (!w->gate[e] || !w->up[e] || !w->down[e]) return caee_fail(c, CAEE_EINVAL, "expert %d has a NULL weight pointer", e);
+    if (fp8 && (!w->gate_scale[e] || !w->up_scale[e] || !w->down_scale[e])) return caee_fail(c, CAEE_EINVAL, "expert %d has a NULL scale pointer", e);
+  }
+  if (c->kernel == CAEE_KERNEL_UMMA && !pack) return caee_fail(c, CAEE_EINVAL, "the UMMA expert kernel needs pack != 0");
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  c->wg_h.assign(w->gate, w->gate + n); c->wu_h.assign(w->up, w->up + n); c->wd_h.assign(w->down, w->down + n);
+  if (fp8) { c->sg_h.assign(w->gate_scale, w->gate_scale + n); c->su_h.assign(w->up_scale, w->up_scale + n); c->sd_h.assign(w->down_scale, w->down_scale + n); }
+  else { c->sg_h.assign(n, nullptr); c->su_h.assign(n, nullptr); c->sd_h.assign(n, nullptr); }
+  const size_t pb = sizeof(void*) * n;
+  CAEE_CUDA(c, cudaMemcpy(c->wg, c->wg_h.data(), pb, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->wu, c->wu_h.data(), pb, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->wd, c->wd_h.data(), pb, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->sg, c->sg_h.data(), pb, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->su, c->su_h.data(), pb, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->sd, c->sd_h.data(), pb, cudaMemcpyHostToDevice));
+  if (c->kernel == CAEE_KERNEL_UMMA) {
+    // tile-major repack, once ("packed weight layout (done once at caee_set_weights)")
+    caee_packed& P = c->packed;
+    for (size_t e = 0; e < P.base.size(); ++e)
+      if (P.base[e]) { if (P.on_host[e]) cudaFreeHost(P.base[e]); else cudaFree(P.base[e]); }
+    P.base.assign(n, nullptr); P.on_host.assign(n, 0);
+    P.bytes_per_expert = caee_umma_packed_bytes(c);
+    if (!P.dev_ptrs) CAEE_CUDA(c, cudaMalloc((void**)&P.dev_ptrs, pb));
+    for (int e = 0; e < n; ++e) {
+      const bool res = e >= c->d.E || c->resident_h[e];
+      if (!res) return caee_fail(c, CAEE_EUNSUPPORTED, "non-resident experts are not supported by the UMMA path yet");
+      CAEE_CUDA(c, cudaMalloc((void**)&P.base[e], P.bytes_per_expert));
+      caee_launch_pack_expert(c, e, P.base[e], c->wg_h[e], c->wu_h[e], c->wd_h[e], c->sg_h[e], c->su_h[e], c->sd_h[e], 0);
+    }
+    CAEE_CUDA(c, cudaMemcpy(P.dev_ptrs, P.base.data(), pb, cudaMemcpyHostToDevice));
+    CAEE_CUDA(c, cudaDeviceSynchronize());
+  } else {
+    for (int e = 0; e < c->d.E; ++e)
+      if (!c->resident_h[e]) return caee_fail(c, CAEE_EUNSUPPORTED, "the SIMT expert kernel needs every expert in device memory");
+  }
+  c->have_weights = true;
+  return CAEE_OK;
+}
+
+caee_status caee_calibrate_cost(caee_ctx* c, const caee_calib_opts* opts, caee_cost_fit out_fit[2]) {
+  if (!c) return CAEE_EINVAL;
+  if (!out_fit) return caee_fail(c, CAEE_EINVAL, "out_fit is NULL");
+  if (c->cuda_failed) return CAEE_ECUDA;
+  DeviceGuard g(c->device);
+  caee_status rc = caee_calibrate_impl(c, opts, out_fit);
+  if (rc != CAEE_OK) return rc;
+  if (!opts || opts->apply) {
+    const int64_t bytes = 3LL * c->d.H * c->d.I * (c->d.w_dtype == CAEE_F32 ? 4 : c->d.w_dtype == CAEE_BF16 ? 2 : 1) +
+                          (c->d.w_dtype == CAEE_E4M3 ? 3LL * ((c->d.H + 127) / 128) * ((c->d.I + 127) / 128) * 4 : 0);
+    std::vector<int64_t> tr(c->d.E), tm(c->d.E);
+    for (int e = 0; e < c->d.E; ++e) {
+      tr[e] = out_fit[0].valid ? llround(out_fit[0].slope_ns_per_byte * (double)bytes + out_fit[0].intercept_ns) : c->ticks_res_h[e];
+      tm[e] = out_fit[1].valid ? llround(out_fit[1].slope_ns_per_byte * (double)bytes + out_fit[1].intercept_ns) : c->ticks_miss_h[e];
+      if (tr[e] < 0) tr[e] = 0;
+      if (tm[e] < 0) tm[e] = 0;
+    }
+    return caee_set_cost_table(c, tr.data(), tm.data());
+  }
+  return CAEE_OK;
+}
+
+caee_status caee_route(caee_ctx* c, const void* x, int32_t T, float* scores, int32_t* idx, float* gate, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if (!c->have_router) return caee_fail(c, CAEE_ESTATE, "caee_route before caee_set_router");
+  if (T == 0) return CAEE_OK;
+  if (!x || !idx || !gate) return caee_fail(c, CAEE_EINVAL, "x, idx or gate is NULL");
+  DeviceGuard g(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  int ks = caee_router_ksplit(c, T);
+  caee_launch_router_logits(c, x, T, ks, st);
+  caee_launch_route_topk(c, nullptr, ks, T, scores, idx, gate, st);
+  return after_launch(c, "caee_route");
+}
+
+caee_status caee_route_from_scores(caee_ctx* c, const float* scores, int32_t T, int32_t* idx, float* gate, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if (T == 0) return CAEE_OK;
+  if (!scores || !idx || !gate) return caee_fail(c, CAEE_EINVAL, "scores, idx or gate is NULL");
+  DeviceGuard g(c->device);
+  caee_launch_route_topk(c, scores, 0, T, nullptr, idx, gate, (cudaStream_t)stream);
+  return after_launch(c, "caee_route_from_scores");
+}
+
+caee_status caee_prune(caee_ctx* c, const caee_prune_params* p, const float* scores, int32_t T, int32_t* idx, float* gate,
+                       const caee_prune_out* out, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if ((rc = validate_prune(c, p)) != CAEE_OK) return rc;
+  if (T > 0 && (!idx || !gate)) return caee_fail(c, CAEE_EINVAL, "idx or gate is NULL");
+  const bool prunes = p && p->mode != CAEE_PRUNE_NONE;
+  if (prunes && T > 0 && !scores) return caee_fail(c, CAEE_EINVAL, "scores is NULL but compensation needs them");
+  DeviceGuard g(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  caee_prune_params none = {CAEE_PRUNE_NONE, 0, 0.0};
+  rc = enqueue_decisions(c, nullptr, scores, T, p ? p : &none, idx, gate, nullptr, false, st);
+  if (rc != CAEE_OK) return rc;
+  caee_launch_export_worklist(c, T, out, st);
+  if (out) {
+    const size_t E = c->d.E;
+    if (out->act) CAEE_CUDA(c, cudaMemcpyAsync(out->act, c->act, E, cudaMemcpyDeviceToDevice, st));
+    if (out->must) CAEE_CUDA(c, cudaMemcpyAsync(out->must, c->must, E, cudaMemcpyDeviceToDevice, st));
+    if (out->keep) CAEE_CUDA(c, cudaMemcpyAsync(out->keep, c->keep, E, cudaMemcpyDeviceToDevice, st));
+    if (out->importance) CAEE_CUDA(c, cudaMemcpyAsync(out->importance, c->I_fix, 8 * E, cudaMemcpyDeviceToDevice, st));
+    if (out->load) CAEE_CUDA(c, cudaMemcpyAsync(out->load, c->load, 8 * (size_t)c->d.D, cudaMemcpyDeviceToDevice, st));
+    if (out->scalars) CAEE_CUDA(c, cudaMemcpyAsync(out->scalars, c->scalars, 64, cudaMemcpyDeviceToDevice, st));
+  }
+  return after_launch(c, "caee_prune");
+}
+
+static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores, int32_t T, const caee_prune_params* p,
+                                void* y, caee_fwd_stats* stats, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if ((rc = validate_prune(c, p)) != CAEE_OK) return rc;
+  if (!c->have_weights) return caee_fail(c, CAEE_ESTATE, "caee_moe_forward before caee_set_weights");
+  if (!scores && !c->have_router) return caee_fail(c, CAEE_ESTATE, "caee_moe_forward before caee_set_router");
+  if (p && p->mode != CAEE_PRUNE_NONE && !c->have_cost) return caee_fail(c, CAEE_ESTATE, "pruning requested before caee_set_cost_table / caee_calibrate_cost");
+  if (T == 0) return CAEE_OK;
+  if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
+  DeviceGuard g(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);
+  if (rc != CAEE_OK) return rc;
+  if (c->kernel == CAEE_KERNEL_SIMT) caee_launch_expert_simt(c, x, T, st);
+  else caee_launch_expert_umma(c, x, T, st);
+  caee_launch_combine(c, T, c->idx, c->gate, y, st);
+  caee_launch_stats(c, stats, p != nullptr, st);
+  return after_launch(c, "caee_moe_forward");
+}
+
+caee_status caee_moe_forward(caee_ctx* c, const void* x, int32_t T, const caee_prune_params* p, void* y,
+                             caee_fwd_stats* stats, void* stream) {
+  return forward_impl(c, x, nullptr, T, p, y, stats, stream);
+}
+
+caee_status caee_moe_forward_from_scores(caee_ctx* c, const void* x, const float* scores, int32_t T,
+                                         const caee_prune_params* p, void* y, caee_fwd_stats* stats, void* stream) {
+  if (c && !scores && T > 0) return caee_fail(c, CAEE_EINVAL, "scores is NULL");
+  return forward_impl(c, x, scores, T, p, y, stats, stream);
+}
+
+caee_status caee_last_routing(caee_ctx* c, int32_t T, int32_t* idx, float* gate, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if (T == 0) return CAEE_OK;
+  DeviceGuard g(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (idx) CAEE_CUDA(c, cudaMemcpyAsync(idx, c->idx, sizeof(int32_t) * T * c->d.k, cudaMemcpyDeviceToDevice, st));
+  if (gate) CAEE_CUDA(c, cudaMemcpyAsync(gate, c->gate, sizeof(float) * T * c->d.k, cudaMemcpyDeviceToDevice, st));
+  return CAEE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,141 @@
+// caee_internal.cuh — context layout and launch declarations shared by the .cu files of
+// libcaee.  Not part of the public ABI (include/caee.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/caee.h"
+
+#define CAEE_FIX_ONE_F 1099511627776.0f /* 2^40: fixed-point unit of I(e) */
+#define CAEE_MAX_E 512
+#define CAEE_MAX_D 64
+#define CAEE_RUN_TOKENS 128 /* tokens per run: one UMMA N tile */
+
+// One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
+struct caee_worklist {
+  // experts with >= 1 token (ABI view, S6)
+  int32_t* counts;      // [E]   tokens per routed expert
+  int32_t* estart;      // [E]   first entry of expert e (exclusive scan of counts)
+  int32_t* offs;        // [E+1] exclusive scan over experts with >= 1 token (compacted)
+  int32_t* expert_ids;  // [E]
+  int32_t* ent_tok;     // [Tmax*(k+S)] token of each entry; routed entries first, shared after Tmax*k... see worklist.cu
+  int32_t* ent_slot;    // [Tmax*k]
+  float* ent_wt;        // [Tmax*k]
+  int32_t* ent_dst;     // [Tmax*(k+S)] destination row in o
+  // runs (kernel view)
+  int32_t* run_expert;  // [max_runs] expert id in 0..E+S-1
+  int32_t* run_start;   // [max_runs] first entry
+  int32_t* run_n;       // [max_runs] tokens in the run, 1..CAEE_RUN_TOKENS
+  int32_t* run_hrow;    // [max_runs] first row of the run in the h scratch (rows padded to 16 per run)
+  int32_t* meta;        // [16]: 0 n_run(ABI) 1 n_runs 2 n_entries(routed) 3 h rows total 4.. reserved
+  int32_t* sched;       // [2 + max_runs]: 0 ticket, 1 unused, 2.. per-run ready counters
+  int32_t max_runs;
+};
+
+struct caee_packed {
+  // per expert (E+S) device pointer to the packed tile image, or NULL if not packed / not resident
+  uint8_t** dev_ptrs;            // device array [E+S]
+  std::vector<uint8_t*> base;    // host copy of the pointers (device memory or pinned host)
+  std::vector<uint8_t> on_host;  // 1: base[e] is pinned host memory
+  size_t bytes_per_expert = 0;
+  size_t p1_tile_bytes = 0, p2_tile_bytes = 0;  // bytes of one phase-1 / phase-2 tile (all k-blocks)
+};
+
+struct caee_ctx {
+  caee_layer_desc d;
+  int device = 0, num_sms = 0;
+  int kernel = CAEE_KERNEL_SIMT;  // resolved expert kernel
+  std::string err;
+  bool cuda_failed = false;
+
+  // router (borrowed)
+  const float* Wr = nullptr;
+  const float* b_logit = nullptr;
+  const float* corr_bias = nullptr;
+  bool have_router = false, have_weights = false, have_cost = false;
+
+  // tables
+  std::vector<int32_t> part_h;
+  std::vector<uint8_t> resident_h;
+  std::vector<int64_t> ticks_res_h, ticks_miss_h;
+  int32_t* part = nullptr;      // dev [E]
+  uint8_t* resident = nullptr;  // dev [E]
+  int64_t* w_eff = nullptr;     // dev [E] = resident ? ticks_resident : ticks_miss
+
+  // raw weights (borrowed): device arrays of E+S pointers
+  const void** wg = nullptr;
+  const void** wu = nullptr;
+  const void** wd = nullptr;
+  const float** sg = nullptr;
+  const float** su = nullptr;
+  const float** sd = nullptr;
+  std::vector<const void*> wg_h, wu_h, wd_h;
+  std::vector<const float*> sg_h, su_h, sd_h;
+  caee_packed packed;
+
+  // scratch
+  int ksplit_max = 1;
+  float* partial = nullptr;  // [ksplit_max, Tmax, E]
+  float* scores = nullptr;   // [Tmax, E]
+  int32_t* idx = nullptr;    // [Tmax, k]
+  float* gate = nullptr;     // [Tmax, k]
+  uint8_t* act = nullptr;    // [E]
+  uint8_t* must = nullptr;
+  uint8_t* keep = nullptr;
+  int64_t* I_fix = nullptr;  // [E]
+  int64_t* load = nullptr;   // [D]
+  int64_t* scalars = nullptr;  // [8]
+  caee_worklist wl;
+  float* hbuf_f32 = nullptr;         // SIMT: h rows [rows, I] fp32
+  __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16/fp16
+  float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
+  size_t h_rows_cap = 0;
+
+  // offload
+  cudaStream_t side_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+};
+
+caee_status caee_fail(caee_ctx* c, caee_status code, const char* fmt, ...);
+caee_status caee_check_cuda(caee_ctx* c, cudaError_t e, const char* what);
+
+#define CAEE_CUDA(c, expr)                                             \
+  do {                                                                 \
+    cudaError_t _e = (expr);                                           \
+    if (_e != cudaSuccess) return caee_check_cuda((c), _e, #expr);     \
+  } while (0)
+
+static inline int caee_ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// router.cu
+int caee_router_ksplit(const caee_ctx* c, int T);
+void caee_launch_router_logits(caee_ctx* c, const void* x, int T, int ksplit, cudaStream_t s);
+void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int ksplit, int T, float* scores_out,
+                            int32_t* idx, float* gate, cudaStream_t s);
+// prune.cu
+void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx,
+                       const float* gate, cudaStream_t s);
+void caee_launch_compensate(caee_ctx* c, int flags, const float* scores, int T, int32_t* idx, float* gate,
+                            cudaStream_t s);
+// worklist.cu
+void caee_launch_worklist(caee_ctx* c, int T, const int32_t* idx, const float* gate, cudaStream_t s);
+void caee_launch_export_worklist(caee_ctx* c, int T, const caee_prune_out* out, cudaStream_t s);
+// expert_simt.cu
+void caee_launch_expert_simt(caee_ctx* c, const void* x, int T, cudaStream_t s);
+// expert_umma.cu
+caee_status caee_umma_supported(const caee_ctx* c, std::string* why);
+size_t caee_umma_packed_bytes(const caee_ctx* c);
+void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst_dev, const void* g, const void* u, const void* d,
+                             const float* sg, const float* su, const float* sd, cudaStream_t s);
+void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, cudaStream_t s);
+// combine.cu
+void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
+void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, cudaStream_t s);
+// calibrate.cu
+caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost_fit fit[2]);

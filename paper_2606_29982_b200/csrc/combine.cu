@@ -1,0 +1,74 @@
+// combine.cu — S8 weighted combine:
+//   y_t = routed_scale * sum_{j: K_final(t)_j valid} G(t)_j * o[t, j] + sum_s o[t, k+s]
+// The expert kernels leave each (token, slot) output row in o[(t*(k+S) + slot), :] (fp32), so
+// the sum runs in list order and y is deterministic.  Also fills caee_fwd_stats.
+#include "caee_internal.cuh"
+
+namespace {
+
+template <typename YT> __device__ __forceinline__ void st4(YT* p, float4 v);
+template <> __device__ __forceinline__ void st4<float>(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+template <> __device__ __forceinline__ void st4<__nv_bfloat16>(__nv_bfloat16* p, float4 v) {
+  __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+  uint2 u = {*reinterpret_cast<uint32_t*>(&a), *reinterpret_cast<uint32_t*>(&b)};
+  *reinterpret_cast<uint2*>(p) = u;
+}
+
+template <typename YT>
+__global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf, const int32_t* __restrict__ idx,
+                                                 const float* __restrict__ gate, YT* __restrict__ y, int H, int k, int S,
+                                                 float routed_scale) {
+  const int t = blockIdx.y, c = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (c >= H) return;
+  const int KS = k + S;
+  float4 acc = {0.f, 0.f, 0.f, 0.f};
+  for (int j = 0; j < k; ++j) {
+    if (idx[(size_t)t * k + j] < 0) continue;
+    const float g = gate[(size_t)t * k + j];
+    const float4 o = *reinterpret_cast<const float4*>(obuf + ((size_t)t * KS + j) * H + c);
+    acc.x = fmaf(g, o.x, acc.x); acc.y = fmaf(g, o.y, acc.y); acc.z = fmaf(g, o.z, acc.z); acc.w = fmaf(g, o.w, acc.w);
+  }
+  acc.x *= routed_scale; acc.y *= routed_scale; acc.z *= routed_scale; acc.w *= routed_scale;
+  for (int s = 0; s < S; ++s) {
+    const float4 o = *reinterpret_cast<const float4*>(obuf + ((size_t)t * KS + k + s) * H + c);
+    acc.x += o.x; acc.y += o.y; acc.z += o.z; acc.w += o.w;
+  }
+  st4<YT>(y + (size_t)t * H + c, acc);
+}
+
+__global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_t* load, const int32_t* meta, int D, int S,
+                        int pruned, long long bytes_per_expert, const int32_t* fetch_info) {
+  if (threadIdx.x == 0) {
+    st->F_base = pruned ? scalars[0] : 0;
+    st->F_cost_dense = pruned ? scalars[1] : 0;
+    st->F_cost = pruned ? scalars[2] : 0;
+    st->F_imp = pruned ? scalars[3] : 0;
+    st->n_act = pruned ? (int32_t)scalars[4] : meta[0];
+    st->n_keep = pruned ? (int32_t)scalars[6] : meta[0];
+    st->n_run = meta[0];
+    int n_sh = meta[1] > 0 ? S : 0;
+    st->weight_bytes = (long long)(meta[0] + n_sh) * bytes_per_expert;
+    st->n_fetch = fetch_info ? fetch_info[0] : 0;
+    st->h2d_bytes = (long long)st->n_fetch * bytes_per_expert;
+  }
+  for (int d = threadIdx.x; d < 64; d += blockDim.x) st->load[d] = (pruned && d < D) ? load[d] : 0;
+}
+
+}  // namespace
+
+void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t st) {
+  const caee_layer_desc& d = c->d;
+  if (T <= 0) return;
+  dim3 grid(caee_ceil_div(d.H, 1024), T);
+  if (d.act_dtype == CAEE_F32)
+    k_combine<float><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (float*)y, d.H, d.k, d.S, d.routed_scale);
+  else
+    k_combine<__nv_bfloat16><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (__nv_bfloat16*)y, d.H, d.k, d.S, d.routed_scale);
+}
+
+void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, cudaStream_t st) {
+  if (!stats) return;
+  long long bpe = 3LL * c->d.H * c->d.I * (c->d.w_dtype == CAEE_F32 ? 4 : c->d.w_dtype == CAEE_BF16 ? 2 : 1);
+  if (c->d.w_dtype == CAEE_E4M3) bpe += 3LL * ((c->d.H + 127) / 128) * ((c->d.I + 127) / 128) * 4;
+  k_stats<<<1, 64, 0, st>>>(stats, c->scalars, c->load, c->wl.meta, c->d.D, c->d.S, pruned, bpe, nullptr);
+}

@@ -1,0 +1,109 @@
+// warp_select.cuh — warp-shuffle top-k used by the router (S1) and by compensation (S5).
+// A warp holds one token's E scores, expert e = lane + 32*i in register slot i.  Every
+// comparison is "(value desc, expert id asc)" so that ties go to the lower index (R22),
+// and gates are summed in list order with round-to-nearest fp32 adds and an IEEE divide
+// so that the result is a deterministic function of the scores.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define CAEE_NONE_ID 0x7fffffff
+
+__device__ __forceinline__ bool caee_before(float va, int ia, float vb, int ib) {
+  return va > vb || (va == vb && ia < ib);
+}
+
+__device__ __forceinline__ void caee_warp_argmax(float& v, int& id) {
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    float ov = __shfl_xor_sync(0xffffffffu, v, o);
+    int oi = __shfl_xor_sync(0xffffffffu, id, o);
+    if (caee_before(ov, oi, v, id)) { v = ov; id = oi; }
+  }
+}
+
+// Group-limited routing: group score = sum of the two largest s' in the group; the
+// topk_group best groups (ties -> lower group id) stay allowed.  Returns the per-lane slot
+// mask of allowed experts.  Requires n_group <= 32.
+template <int NV>
+__device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint32_t ok, int E, int n_group,
+                                                    int topk_group, int lane) {
+  const int gs = E / n_group;
+  float my_gscore = -INFINITY;  // lane g holds the score of group g
+  for (int g = 0; g < n_group; ++g) {
+    float m1 = -INFINITY, m2 = -INFINITY;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int e = lane + 32 * i;
+      if (((ok >> i) & 1u) && e / gs == g) {
+        float v = sp[i];
+        if (v > m1) { m2 = m1; m1 = v; }
+        else if (v > m2) m2 = v;
+      }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      float o1 = __shfl_xor_sync(0xffffffffu, m1, o);
+      float o2 = __shfl_xor_sync(0xffffffffu, m2, o);
+      float hi = fmaxf(m1, o1), lo = fminf(m1, o1);
+      m2 = fmaxf(lo, fmaxf(m2, o2));
+      m1 = hi;
+    }
+    float sc = gs >= 2 ? __fadd_rn(m1, m2) : m1;
+    if (lane == g) my_gscore = sc;
+  }
+  uint32_t gsel = 0;
+  for (int j = 0; j < topk_group; ++j) {
+    float v = (lane < n_group && !((gsel >> lane) & 1u)) ? my_gscore : -INFINITY;
+    int id = (lane < n_group && !((gsel >> lane) & 1u)) ? lane : CAEE_NONE_ID;
+    caee_warp_argmax(v, id);
+    if (id != CAEE_NONE_ID) gsel |= 1u << id;
+  }
+  uint32_t m = 0;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int e = lane + 32 * i;
+    if (e < E && ((gsel >> (e / gs)) & 1u)) m |= 1u << i;
+  }
+  return m;
+}
+
+// Top-k of sp over the allowed slots, listed in descending order; gates from s.
+// Writes idx_out[0..k) (-1 for empty slots) and gate_out[0..k).  k <= 32.
+template <int NV>
+__device__ __forceinline__ void caee_warp_select(const float (&s)[NV], const float (&sp)[NV], uint32_t ok, int k,
+                                                 int norm_topk, int lane, int32_t* idx_out, float* gate_out) {
+  int sel_e = -1;
+  float sel_s = 0.f;
+  for (int j = 0; j < k; ++j) {
+    float bv = -INFINITY;
+    int bi = CAEE_NONE_ID;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int e = lane + 32 * i;
+      if (((ok >> i) & 1u) && caee_before(sp[i], e, bv, bi)) { bv = sp[i]; bi = e; }
+    }
+    caee_warp_argmax(bv, bi);
+    float ws = 0.f;
+    if (bi != CAEE_NONE_ID) {
+      int owner = bi & 31, slot = bi >> 5;
+      float mine = 0.f;
+#pragma unroll
+      for (int i = 0; i < NV; ++i)
+        if (i == slot) mine = s[i];
+      ws = __shfl_sync(0xffffffffu, mine, owner);
+      if (lane == owner) ok &= ~(1u << slot);
+    }
+    if (lane == j) { sel_e = bi == CAEE_NONE_ID ? -1 : bi; sel_s = ws; }
+  }
+  float sum = 0.f;
+  for (int j = 0; j < k; ++j) {
+    int ej = __shfl_sync(0xffffffffu, sel_e, j);
+    float sj = __shfl_sync(0xffffffffu, sel_s, j);
+    if (ej >= 0) sum = __fadd_rn(sum, sj);
+  }
+  if (lane < k) {
+    idx_out[lane] = sel_e;
+    gate_out[lane] = sel_e < 0 ? 0.f : (norm_topk ? __fdiv_rn(sel_s, sum) : sel_s);
+  }
+}

@@ -1,0 +1,113 @@
+"""Test/bench harness: builds a CAEE layer on the GPU from a workloads.LayerConfig through the
+ctypes binding, and computes the matching oracle results on the host from the same bits.
+
+The oracle side (oracle_*) only calls oracle/; the GPU side only calls the binding.
+"""
+import numpy as np
+import torch
+
+from oracle import oracle as orc
+from paper_2606_29982_b200 import binding as B
+from paper_2606_29982_b200 import workloads as wl
+
+TOL = {wl.DT_F32: 1e-4, wl.DT_BF16: 2e-2, wl.DT_E4M3: 5e-2}   # x RMS(y), BASELINE.json north_star
+
+
+class GpuLayer:
+    def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=True, device="cuda:0"):
+        self.cfg, self.seed, self.device, self.max_tokens = cfg, seed, device, max_tokens
+        self.ctx = B.caee_create(B.layer_desc(cfg, max_tokens, kernel))
+        self.Wr, self.b_logit, self.corr_bias = wl.router(cfg, seed, device)
+        B.caee_set_router(self.ctx, self.Wr, self.b_logit, self.corr_bias)
+        self.part = wl.partitions(cfg)
+        B.caee_set_partitions(self.ctx, self.part, cfg.D)
+        self.resident = wl.residency(cfg, seed)
+        self.ticks_res, self.ticks_miss = wl.cost_tables(cfg)
+        B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
+        n = cfg.E + cfg.S
+        raw = [wl.expert_weights(cfg, seed, e, device) for e in range(n)]
+        fp8 = cfg.w_dtype == wl.DT_E4M3
+        B.caee_set_weights(self.ctx, [r["gate"] for r in raw], [r["up"] for r in raw], [r["down"] for r in raw],
+                           [r["gate_scale"] for r in raw] if fp8 else None, [r["up_scale"] for r in raw] if fp8 else None,
+                           [r["down_scale"] for r in raw] if fp8 else None, pack=1)
+        torch.cuda.synchronize()
+        self.raw = raw if keep_raw else None
+        self._host = {}
+
+    def close(self):
+        if self.ctx is not None:
+            B.caee_destroy(self.ctx)
+            self.ctx = None
+            self.raw = None
+
+    # ---- host copies of exactly the bits the GPU holds
+    def host_expert(self, e):
+        if e not in self._host:
+            r = self.raw[e] if self.raw is not None else wl.expert_weights(self.cfg, self.seed, e, self.device)
+            self._host[e] = {k: wl.bits(v) for k, v in r.items()}
+        return self._host[e]
+
+    def w_eff(self):
+        return orc.effective_cost(self.resident, self.ticks_res, self.ticks_miss)
+
+    # ---- oracle pipeline on the same inputs
+    def oracle_scores(self, x):
+        return orc.scores(wl.bits(x), self.Wr.cpu().numpy(), self.b_logit.cpu().numpy(), self.cfg.score_fn)
+
+    def oracle_decisions(self, s, mode=None, theta=0.0, flags=0):
+        """route -> prune -> compensate -> compact on scores s.  mode None = dense top-k."""
+        c = self.cfg
+        cb = None if self.corr_bias is None else self.corr_bias.cpu().numpy()
+        idx, gate = orc.route(s, cb, c.k, c.n_group, c.topk_group, c.norm_topk)
+        out = dict(idx0=idx.copy(), gate0=gate.copy())
+        if mode is not None:
+            pr = orc.prune(mode, theta, flags, idx, gate, c.E, self.w_eff(), self.part, c.D)
+            if mode != 0:
+                idx, gate = orc.compensate(s, cb, pr["keep"], idx, gate, c.norm_topk, flags)
+            out["prune"] = pr
+        out["idx"], out["gate"] = idx, gate
+        out["compact"] = orc.compact(idx, gate, c.E)
+        return out
+
+    def oracle_y(self, x, idx, gate, tokens):
+        c = self.cfg
+        n = c.E + c.S
+        used = set(int(e) for t in tokens for e in idx[t] if e >= 0) | set(range(c.E, n))
+        tabs = {k: [None] * n for k in ("gate", "up", "down", "gate_scale", "up_scale", "down_scale")}
+        for e in used:
+            h = self.host_expert(e)
+            for k in h:
+                tabs[k][e] = h[k]
+        fp8 = c.w_dtype == wl.DT_E4M3
+        return orc.moe_tokens(wl.bits(x), list(tokens), idx, gate, tabs["gate"], tabs["up"], tabs["down"], c.E, c.S,
+                              c.routed_scale, tabs["gate_scale"] if fp8 else None, tabs["up_scale"] if fp8 else None,
+                              tabs["down_scale"] if fp8 else None)
+
+    # ---- GPU calls (through the C ABI)
+    def forward(self, x, params=None, scores=None, want_stats=False):
+        T = x.shape[0]
+        y = torch.empty_like(x)
+        stats = B.stats_buffer(self.device) if want_stats else None
+        if scores is None:
+            B.caee_moe_forward(self.ctx, x, T, params, y, stats)
+        else:
+            B.caee_moe_forward_from_scores(self.ctx, x, scores, T, params, y, stats)
+        torch.cuda.synchronize()
+        return (y, B.read_stats(stats)) if want_stats else y
+
+    def last_routing(self, T):
+        idx = torch.empty(T, self.cfg.k, dtype=torch.int32, device=self.device)
+        gate = torch.empty(T, self.cfg.k, dtype=torch.float32, device=self.device)
+        B.caee_last_routing(self.ctx, T, idx, gate)
+        torch.cuda.synchronize()
+        return idx.cpu().numpy(), gate.cpu().numpy()
+
+
+def check_y(y_gpu, y_ref, tokens, tol):
+    """max |y_gpu - y_oracle| <= tol * RMS(y_oracle) over the sampled tokens (oracle unrounded, R29)."""
+    got = y_gpu[list(tokens)].double().cpu().numpy()
+    rms = float(np.sqrt(np.mean(y_ref ** 2)))
+    err = float(np.abs(got - y_ref).max())
+    assert np.isfinite(got).all(), "non-finite output"
+    assert err <= tol * rms, f"max|err| {err:.3e} > {tol:g} x RMS {rms:.3e} (ratio {err / rms:.3e})"
+    return err / rms

@@ -1,0 +1,224 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu, needs a B200).
+
+Protocol: (1) GPU scores vs oracle scores <= 1e-5 relative; (2) with the
+oracle's fp32 scores injected, indices, gates, masks, lists and F_* values bit-exact;
+(3) layer output within 1e-4 / 2e-2 / 5e-2 x RMS (fp32 / bf16 / fp8) of the unrounded oracle.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_29982_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MODES = {"none": (0, 0.0), "thresh": (1, None), "cir": (2, 0.8), "rank": (3, 1), "frac": (4, 0.25)}
+
+# reduced R1-style layer: same routing structure, a few tiles in each direction
+R1S = wl.scaled(wl.C3, name="R1-small", H=1024, I=384, E=64, k=4, n_group=8, topk_group=4, D=8,
+                straggler_part=3, cost_ticks_ns=901)
+C2S = wl.scaled(wl.C2, name="C2-small", H=512, I=256, E=16, S=2, k=3, D=4)
+
+
+@pytest.fixture(scope="module")
+def H():
+    from tests import harness
+    return harness
+
+
+def _layer(H, cfg, **kw):
+    return H.GpuLayer(cfg, **kw)
+
+
+def _thresh_theta(cfg, T):
+    return 0.6 * T * cfg.k / cfg.E + 0.05      # around the mean importance of an active expert
+
+
+@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, wl.C2], ids=lambda c: c.name)
+def test_route_scores_and_selection(H, cfg):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, cfg, max_tokens=160)
+    try:
+        for T in (1, 7, 33, 160):
+            x = wl.hidden(cfg, T, 3, L.device)
+            s_gpu = torch.empty(T, cfg.E, dtype=torch.float32, device=L.device)
+            idx = torch.empty(T, cfg.k, dtype=torch.int32, device=L.device)
+            gate = torch.empty(T, cfg.k, dtype=torch.float32, device=L.device)
+            B.caee_route(L.ctx, x, T, s_gpu, idx, gate)
+            torch.cuda.synchronize()
+            s_ref = L.oracle_scores(x)
+            np.testing.assert_allclose(s_gpu.cpu().numpy(), s_ref, rtol=1e-5, atol=1e-10)
+            # injected scores: bit-exact selection and gates
+            s_dev = torch.from_numpy(s_ref).to(L.device)
+            B.caee_route_from_scores(L.ctx, s_dev, T, idx, gate)
+            torch.cuda.synchronize()
+            d = L.oracle_decisions(s_ref)
+            assert np.array_equal(idx.cpu().numpy(), d["idx0"])
+            assert np.array_equal(gate.cpu().numpy().view(np.uint32), d["gate0"].view(np.uint32))
+    finally:
+        L.close()
+
+
+@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S], ids=lambda c: c.name)
+@pytest.mark.parametrize("mode", list(MODES))
+def test_prune_compensate_compact_bit_exact(H, cfg, mode):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, cfg, max_tokens=300)
+    try:
+        for T in (1, 5, 16, 64, 300):
+            m, theta = MODES[mode]
+            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS) if mode == "thresh" else (0,)):
+                th = _thresh_theta(cfg, T) if theta is None else theta
+                x = wl.hidden(cfg, T, 11, L.device)
+                s = L.oracle_scores(x)
+                d = L.oracle_decisions(s, m, th, flags)
+                s_dev = torch.from_numpy(s).to(L.device)
+                idx = torch.from_numpy(d["idx0"]).to(L.device)
+                gate = torch.from_numpy(d["gate0"]).to(L.device)
+                out = B.PruneOut(cfg.E, cfg.D, T, cfg.k, L.device)
+                B.caee_prune(L.ctx, B.prune_params(m, th, flags), s_dev, T, idx, gate, out.struct)
+                torch.cuda.synchronize()
+                g = {k: v.cpu().numpy() for k, v in out.t.items()}
+                pr, cp = d["prune"], d["compact"]
+                for name in ("act", "must", "keep"):
+                    assert np.array_equal(g[name], pr[name]), (name, T, mode)
+                assert np.array_equal(g["importance"], pr["I_fix"])
+                assert np.array_equal(g["load"], pr["load"])
+                assert list(g["scalars"][:7]) == [pr["F_base"], pr["F_cost_dense"], pr["F_cost"], pr["F_imp_fix"],
+                                                  pr["n_act"], pr["n_must"], pr["n_keep"]]
+                assert np.array_equal(idx.cpu().numpy(), d["idx"])
+                assert np.array_equal(gate.cpu().numpy().view(np.uint32), d["gate"].view(np.uint32))
+                nr = int(g["n_run"][0])
+                assert nr == cp["n_run"] == int(g["scalars"][7])
+                assert np.array_equal(g["expert_ids"][:nr], cp["expert_ids"])
+                assert np.array_equal(g["offs"][:nr + 1], cp["offs"])
+                ne = int(cp["offs"][-1])
+                assert np.array_equal(g["tok"][:ne], cp["tok"]) and np.array_equal(g["slot"][:ne], cp["slot"])
+                assert np.array_equal(g["wt"][:ne].view(np.uint32), cp["wt"].view(np.uint32))
+                if m != 0 and T >= 16:
+                    assert pr["n_keep"] <= pr["n_act"]
+    finally:
+        L.close()
+
+
+def _forward_case(H, L, T, mode, tokens=None, seed=21):
+    from paper_2606_29982_b200 import binding as B
+    cfg = L.cfg
+    m, theta = MODES[mode]
+    th = _thresh_theta(cfg, T) if theta is None else theta
+    x = wl.hidden(cfg, T, seed, L.device)
+    s = L.oracle_scores(x)
+    d = L.oracle_decisions(s, None if mode == "dense" else m, th)
+    params = None if mode == "dense" else B.prune_params(m, th)
+    y, st = L.forward(x, params, torch.from_numpy(s).to(L.device), want_stats=True)
+    idx_g, gate_g = L.last_routing(T)
+    assert np.array_equal(idx_g, d["idx"])
+    assert np.array_equal(gate_g.view(np.uint32), d["gate"].view(np.uint32))
+    assert st.n_run == d["compact"]["n_run"]
+    if mode != "dense":
+        assert (st.F_base, st.F_cost_dense, st.F_cost) == (d["prune"]["F_base"], d["prune"]["F_cost_dense"], d["prune"]["F_cost"])
+        assert st.n_keep == d["prune"]["n_keep"]
+    tokens = list(range(T)) if tokens is None else tokens
+    y_ref = L.oracle_y(x, d["idx"], d["gate"], tokens)
+    return H.check_y(y, y_ref, tokens, H.TOL[cfg.w_dtype])
+
+
+@pytest.mark.parametrize("mode", ["dense", "none", "rank", "thresh"])
+def test_forward_c1_fp32(H, mode):
+    L = _layer(H, wl.C1, max_tokens=64)
+    try:
+        for T in (16, 1, 37):
+            _forward_case(H, L, T, mode)
+    finally:
+        L.close()
+
+
+@pytest.mark.parametrize("kernel", ["simt", "umma"])
+@pytest.mark.parametrize("cfg", [C2S, R1S], ids=lambda c: c.name)
+def test_forward_small_bf16(H, cfg, kernel):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, cfg, max_tokens=200, kernel=B.CAEE_KERNEL_SIMT if kernel == "simt" else B.CAEE_KERNEL_UMMA)
+    try:
+        for T, mode in ((1, "dense"), (8, "thresh"), (32, "cir"), (128, "frac"), (200, "dense"), (19, "rank")):
+            _forward_case(H, L, T, mode)
+    finally:
+        L.close()
+
+
+def test_forward_hot_expert_spans_several_runs(H):
+    """All tokens on the same experts: one expert gets T > 128 tokens (two runs, ragged tail)."""
+    from paper_2606_29982_b200 import binding as B
+    cfg = C2S
+    L = _layer(H, cfg, max_tokens=300, kernel=B.CAEE_KERNEL_UMMA)
+    try:
+        T = 283
+        x = wl.hidden(cfg, T, 5, L.device)
+        s = np.full((T, cfg.E), 0.01, np.float32)
+        s[:, [2, 5, 11]] = [0.5, 0.3, 0.14]
+        s[::7, 9] = 0.4                                   # a few tokens take another expert
+        d = L.oracle_decisions(s)
+        y = L.forward(x, None, torch.from_numpy(s).to(L.device))
+        toks = list(range(0, T, 9)) + [T - 1]
+        H.check_y(y, L.oracle_y(x, d["idx"], d["gate"], toks), toks, H.TOL[cfg.w_dtype])
+    finally:
+        L.close()
+
+
+def test_forward_edge_cases(H):
+    from paper_2606_29982_b200 import binding as B
+    cfg = R1S
+    L = _layer(H, cfg, max_tokens=32)
+    try:
+        # T = 0 is a no-op
+        B.caee_moe_forward(L.ctx, None, 0, None, None)
+        # a threshold nobody reaches empties A_trans: routed part is 0, shared expert still runs (R15)
+        T = 4
+        x = wl.hidden(cfg, T, 9, L.device)
+        s = L.oracle_scores(x)
+        d = L.oracle_decisions(s, 1, 1e3)
+        assert d["prune"]["n_keep"] == 0 and (d["idx"] == -1).all()
+        y, st = L.forward(x, B.prune_params(1, 1e3), torch.from_numpy(s).to(L.device), want_stats=True)
+        assert st.n_run == 0 and st.n_keep == 0
+        H.check_y(y, L.oracle_y(x, d["idx"], d["gate"], range(T)), range(T), H.TOL[cfg.w_dtype])
+        # T beyond max_tokens is refused, not truncated
+        with pytest.raises(B.CaeeError) as ei:
+            B.caee_moe_forward(L.ctx, x, 33, None, x)
+        assert ei.value.code == B.CAEE_ESHAPE
+        with pytest.raises(B.CaeeError) as ei:
+            B.caee_moe_forward(L.ctx, x, T, B.prune_params(2, 1.5), x)
+        assert ei.value.code == B.CAEE_EINVAL
+    finally:
+        L.close()
+
+
+def test_forward_end_to_end_routing_flips(H):
+    """Own scores (no injection): routing may flip on near-ties; flips must be rare and the
+    output must match the oracle evaluated on the GPU's own K_final."""
+    cfg = R1S
+    L = _layer(H, cfg, max_tokens=128)
+    try:
+        T = 128
+        x = wl.hidden(cfg, T, 31, L.device)
+        y = L.forward(x, None)
+        idx_g, gate_g = L.last_routing(T)
+        d = L.oracle_decisions(L.oracle_scores(x))
+        flips = int((idx_g != d["idx"]).sum())
+        assert flips <= 0.01 * idx_g.size, f"{flips} routing flips of {idx_g.size}"
+        toks = list(range(0, T, 8))
+        H.check_y(y, L.oracle_y(x, idx_g, gate_g, toks), toks, H.TOL[cfg.w_dtype])
+    finally:
+        L.close()
+
+
+def test_calibrate_cost(H):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, C2S, max_tokens=8)
+    try:
+        f_hbm, f_h2d = B.caee_calibrate_cost(L.ctx, B.caee_calib_opts(5, 5, 8 << 20, 96 << 20, 1, 0))
+        assert f_hbm.valid and 1000 < f_hbm.gbytes_per_s < 9000 and f_hbm.r2 > 0.9
+        assert f_h2d.valid and 5 < f_h2d.gbytes_per_s < 200 and f_h2d.r2 > 0.9
+        # the fit agrees with the oracle's least squares on synthetic points
+        from oracle import oracle as orc
+        assert orc.cost_ticks(f_hbm.slope_ns_per_byte, f_hbm.intercept_ns, 3 * C2S.H * C2S.I * 2) > 0
+    finally:
+        L.close()
