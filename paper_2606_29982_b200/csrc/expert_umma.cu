@@ -401,12 +401,13 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, cudaStream_t st)
   const int ncap = std::min(CAEE_RUN_TOKENS, (T + 15) & ~15);
   p.b_stage_bytes = ncap * kKBlock * 2;
   p.stage_bytes = kAStageBytes + p.b_stage_bytes;
-  const int smem_budget = 227 * 1024 - 1024 - 512;  // alignment slack + static barriers
+  const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers block
+  const int smem_budget = max_dyn - 1024;           // alignment slack
   p.n_stages = std::min(kMaxStages, smem_budget / p.stage_bytes);
   const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(k_expert_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 512);
+    cudaFuncSetAttribute(k_expert_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
     attr_set = true;
   }
   k_expert_umma<<<c->num_sms, kThreads, dyn, st>>>(p);

@@ -104,7 +104,7 @@ def test_prune_compensate_compact_bit_exact(H, cfg, mode):
 def _forward_case(H, L, T, mode, tokens=None, seed=21):
     from paper_2606_29982_b200 import binding as B
     cfg = L.cfg
-    m, theta = MODES[mode]
+    m, theta = MODES.get(mode, (0, 0.0))
     th = _thresh_theta(cfg, T) if theta is None else theta
     x = wl.hidden(cfg, T, seed, L.device)
     s = L.oracle_scores(x)
