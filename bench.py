@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py — CAEE MoE-layer decode throughput on B200 (one JSON line on stdout).
+
+A "step" is one pass of the whole hot path (router -> cost lookup -> cost-aware prune ->
+compensation -> compaction -> grouped SwiGLU FFN over the surviving experts -> combine) over
+one batch of synthetic tokens, through the C ABI (caee_moe_forward).  Default workload:
+BASELINE.json config 3, the DeepSeek-R1-shaped bf16 layer (H 7168, 256+1 experts, top-8,
+I 2048, 22.5 GB of expert weights in HBM) at a 128-token decode batch.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--tokens 128]
+                    [--prune thresh:0.6] [--impl caee|reference]
+
+N > 1 (under torchrun) runs N independent replicas ("replicas only").
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "moe_layer_decode_tokens_per_s"
+UNIT = "tokens/s"
+MODE_IDS = {"none": 0, "thresh": 1, "cir": 2, "rank": 3, "frac": 4}
+
+
+def parse_prune(s):
+    if s in ("dense", "off"):
+        return None
+    name, _, val = s.partition(":")
+    return MODE_IDS[name], float(val or 0)
+
+
+def workload_name(cfg, T, prune):
+    p = "dense top-k" if prune is None else f"CAEE prune {prune}"
+    return (f"{cfg.name}: H={cfg.H} I={cfg.I} E={cfg.E}+{cfg.S} top-{cfg.k} groups {cfg.n_group}/{cfg.topk_group} "
+            f"D={cfg.D}, decode batch T={T}, {p}")
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out = self.p.communicate(timeout=5)[0]
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out = self.p.communicate()[0]
+        sm, mx, reasons = [], [], set()
+        for line in out.strip().splitlines():
+            f = [v.strip() for v in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# --------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample_run(cfg, T, prune, seed, n_sample, device_for_inputs, layer=None):
+    """Times the oracle as it stands on the host cores: decisions on all T tokens, FFN + combine on
+    n_sample of them; returns (tokens_per_s extrapolated to T, seconds of CPU work, cores)."""
+    import numpy as np
+    from oracle import oracle as orc
+    from paper_2606_29982_b200 import workloads as wl
+    cores = len(os.sched_getaffinity(0))
+    x = wl.hidden(cfg, T, seed + 100, device_for_inputs)
+    Wr, b_logit, cb = (layer.Wr, layer.b_logit, layer.corr_bias) if layer is not None else wl.router(cfg, seed, device_for_inputs)
+    xb, Wr_h, b_h = wl.bits(x), Wr.cpu().numpy(), b_logit.cpu().numpy()
+    cb_h = None if cb is None else cb.cpu().numpy()
+    part = wl.partitions(cfg)
+    w_eff = orc.effective_cost(wl.residency(cfg, seed), *wl.cost_tables(cfg))
+    t0 = time.perf_counter()
+    s = orc.scores(xb, Wr_h, b_h, cfg.score_fn)
+    idx, gate = orc.route(s, cb_h, cfg.k, cfg.n_group, cfg.topk_group, cfg.norm_topk)
+    if prune is not None:
+        pr = orc.prune(prune[0], prune[1], 0, idx, gate, cfg.E, w_eff, part, cfg.D)
+        if prune[0] != 0:
+            idx, gate = orc.compensate(s, cb_h, pr["keep"], idx, gate, cfg.norm_topk, 0)
+    orc.compact(idx, gate, cfg.E)
+    t_dec = time.perf_counter() - t0
+    tokens = list(range(0, T, max(1, T // n_sample)))[:n_sample]
+    n = cfg.E + cfg.S
+    used = sorted(set(int(e) for t in tokens for e in idx[t] if e >= 0) | set(range(cfg.E, n)))
+    tabs = {k: [None] * n for k in ("gate", "up", "down", "gate_scale", "up_scale", "down_scale")}
+    for e in used:                                   # untimed: fetch the exact bits of the needed experts
+        r = wl.expert_weights(cfg, seed, e, device_for_inputs)
+        for k_, v in r.items():
+            tabs[k_][e] = wl.bits(v)
+    fp8 = cfg.w_dtype == wl.DT_E4M3
+    t0 = time.perf_counter()
+    orc.moe_tokens(xb, tokens, idx, gate, tabs["gate"], tabs["up"], tabs["down"], cfg.E, cfg.S, cfg.routed_scale,
+                   tabs["gate_scale"] if fp8 else None, tabs["up_scale"] if fp8 else None,
+                   tabs["down_scale"] if fp8 else None)
+    t_ffn = time.perf_counter() - t0
+    total = t_dec + t_ffn * T / len(tokens)
+    return T / total, t_dec + t_ffn, cores, len(tokens)
+
+
+def run_reference(args, cfg, prune):
+    """--impl reference: the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    T = args.tokens
+    n_sample = 1
+    vals, secs = [], []
+    for i in range(args.warmup + args.steps):
+        v, sec, cores, ns = oracle_sample_run(cfg, T, prune, 0, n_sample, "cpu")
+        if i >= args.warmup:
+            vals.append(v)
+            secs.append(sec)
+    value = statistics.mean(vals)
+    sample = (f"per step: oracle decisions on all {T} tokens + FFN/combine on {n_sample} token(s), extrapolated linearly "
+              f"to {T} tokens; inputs drawn on the CPU generator")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * T / value, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, T, args.prune)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# --------------------------------------------------------------------------- the CUDA arm
+def run_caee(args, cfg, prune):
+    import torch
+    from paper_2606_29982_b200 import binding as B
+    from paper_2606_29982_b200 import workloads as wl
+    from paper_2606_29982_b200.layer import Layer
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libcaee has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    T, K, W = args.tokens, args.steps, max(args.warmup, 3)
+    L = Layer(cfg, seed=rank, max_tokens=max(T, 128), device=dev)
+    params = None if prune is None else B.prune_params(prune[0], prune[1])
+    xs = [wl.hidden(cfg, T, rank * 1000 + 100 + i, dev) for i in range(4)]      # rotate a few batches
+    y = torch.empty_like(xs[0])
+    stats = B.stats_buffer(dev)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(steps):
+            fn(i)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    step = lambda i: L.forward(xs[i % len(xs)], params, y=y, stats=stats)
+    for i in range(W):
+        step(i)
+    torch.cuda.synchronize()
+    # --- device-resident timing, with the expert kernel timed by its own event pair
+    B.caee_profile(L.ctx, K)
+    clocks = ClockSampler(local)
+    ms_total = timed(step, K)
+    clk = clocks.stop()
+    expert_ms = B.caee_profile_read(L.ctx, K)
+    B.caee_profile(L.ctx, 0)
+    st = B.read_stats(stats)
+    ms_step = ms_total / K
+    value = world * T / (ms_step * 1e-3)
+
+    # --- end to end through the public call with HOST buffers (pinned), copies inside the timed region
+    xh = [x.cpu().pin_memory() for x in xs]
+    yh = torch.empty_like(xh[0]).pin_memory()
+    xd = torch.empty_like(xs[0])
+
+    def e2e_step(i):
+        xd.copy_(xh[i % len(xh)], non_blocking=True)
+        L.forward(xd, params, y=y)
+        yh.copy_(y, non_blocking=True)
+
+    for i in range(3):
+        e2e_step(i)
+    ms_e2e = timed(e2e_step, K) / K
+    e2e_value = world * T / (ms_e2e * 1e-3)
+    nbytes = xs[0].numel() * xs[0].element_size()
+
+    # --- dense (no pruning) beside it, same batches
+    dense_ms = timed(lambda i: L.forward(xs[i % len(xs)], None, y=y, stats=stats), K) / K
+    st_dense = B.read_stats(stats)
+
+    if rank != 0:
+        L.close()
+        return
+    peak, peak_src = peaks()
+    k_ms = float(statistics.mean(expert_ms)) if len(expert_ms) else None
+    achieved = st.weight_bytes / (k_ms * 1e-3) / 1e9 if k_ms else None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"{cfg.name}/T{T}/{args.prune}")
+    launches_per_step = 2 + (2 if prune is not None and prune[0] != 0 else (1 if prune is not None else 0)) + 3 + 1 + 1 + 1
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.w_dtype], "data": "synthetic",
+        "config": {"workload": workload_name(cfg, T, args.prune), "l2": "inputs larger than L2: each step streams "
+                   f"{st.weight_bytes / 1e9:.2f} GB of expert weights (L2 is 126 MB)", "parallelism": "replicas only",
+                   "seed": 0},
+        "clocks": clk,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "ms_per_step": ms_e2e},
+        "gpu_launches": launches_per_step * K,
+        "roofline": {"bound": "hbm", "kernel": "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak if achieved else None, "traffic": traffic, "peak_source": peak_src,
+                     "bytes_per_launch": st.weight_bytes, "kernel_ms": k_ms,
+                     "frac_of_8TBps_nominal": achieved / 8000.0 if achieved else None},
+        "latency_us": {"pruned": ms_step * 1e3, "dense": dense_ms * 1e3, "expert_kernel": k_ms * 1e3 if k_ms else None},
+        "pruning": {"n_act": st.n_act, "n_keep": st.n_keep, "n_run": st.n_run, "F_cost_dense": st.F_cost_dense,
+                    "F_cost": st.F_cost, "bytes_pruned": st.weight_bytes, "bytes_dense": st_dense.weight_bytes,
+                    "n_run_dense": st_dense.n_run},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        try:
+            import psutil
+            ram_gb = psutil.virtual_memory().available / 2 ** 30
+        except Exception:
+            ram_gb = 16.0
+        n_sample = max(1, min(16, int((ram_gb * 0.4) / (cfg.expert_bytes * cfg.k / 2 ** 30 + 1e-9))))
+        L.close()
+        torch.cuda.empty_cache()
+        v, sec, cores, ns = oracle_sample_run(cfg, T, prune, 0, n_sample, dev)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"oracle decisions on all {T} tokens + FFN/combine on {ns} of them "
+                                         f"({sec:.1f} s of CPU work), extrapolated linearly to {T} tokens"}
+    else:
+        L.close()
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="caee", choices=["caee", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--tokens", type=int, default=128)
+    ap.add_argument("--prune", default="thresh:0.6", help="dense | none | thresh:θ | cir:θ_imp | rank:b | frac:p")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2606_29982_b200 import workloads as wl
+    cfg = wl.CONFIGS[args.workload.upper()]
+    prune = parse_prune(args.prune)
+    if args.impl == "reference":
+        run_reference(args, cfg, prune)
+    else:
+        run_caee(args, cfg, prune)
+
+
+if __name__ == "__main__":
+    main()

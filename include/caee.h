@@ -83,7 +83,7 @@ typedef struct caee_layer_desc {
   int32_t w_dtype;       /* CAEE_F32, CAEE_BF16 or CAEE_E4M3: dtype of expert weights            */
   int32_t D;             /* expert partitions, 1..64                                             */
   int32_t max_tokens;    /* largest T any call will pass; scratch is sized from it               */
-  int32_t expert_kernel; /* CAEE_KERNEL_*: AUTO = UMMA (tcgen05) for bf16/e4m3, SIMT for fp32     */
+  int32_t expert_kernel; /* CAEE_KERNEL_*: AUTO = UMMA (tcgen05) where it applies, else SIMT     */
   int32_t device;        /* CUDA device ordinal, -1 = current device                             */
 } caee_layer_desc;
 
@@ -211,6 +211,15 @@ caee_status caee_moe_forward_from_scores(caee_ctx* ctx, const void* x, const flo
                                          void* stream);
 /* K_final of the last forward call on this context (dev -> dev copy, enqueued on stream). */
 caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gate, void* stream);
+
+/* Optional per-kernel timing for measurement (bench.py's roofline): with n_slots > 0 every
+ * following caee_moe_forward* records a CUDA-event pair around its expert kernel on the
+ * call's stream, into slot 0, 1, ... (further calls are not recorded once the slots are
+ * used up); n_slots == 0 switches it off.  caee_profile_read synchronises on the recorded
+ * events and writes the expert kernel's duration of each recorded call in ms to
+ * expert_ms (host, [n_slots]) and their number to n_out (host), then rewinds to slot 0. */
+caee_status caee_profile(caee_ctx* ctx, int32_t n_slots);
+caee_status caee_profile_read(caee_ctx* ctx, float* expert_ms, int32_t* n_out);
 
 /* Library / build identification, e.g. "caee-b200 0.1 sm_100a". */
 const char* caee_version(void);

@@ -27,7 +27,7 @@ CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",
            "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_route",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
-           "caee_last_routing", "caee_version"]
+           "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version"]
 
 
 class caee_layer_desc(C.Structure):
@@ -87,6 +87,8 @@ _lib.caee_moe_forward.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.POINTER(caee_
 _lib.caee_moe_forward_from_scores.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(caee_prune_params),
                                               C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_last_routing.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.caee_profile.argtypes = [_ctx_p, C.c_int32]
+_lib.caee_profile_read.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
 for _n in EXPORTS:
     if _n not in ("caee_last_error", "caee_version"):
         getattr(_lib, _n).restype = C.c_int32
@@ -208,12 +210,29 @@ def caee_last_routing(ctx, T, idx, gate, stream=None):
     _check(_lib.caee_last_routing(ctx, int(T), _ptr(idx), _ptr(gate), _stream(stream)), ctx)
 
 
+def caee_profile(ctx, n_slots):
+    _check(_lib.caee_profile(ctx, int(n_slots)), ctx)
+
+
+def caee_profile_read(ctx, n_slots):
+    ms = np.zeros(max(int(n_slots), 1), np.float32)
+    n = C.c_int32(0)
+    _check(_lib.caee_profile_read(ctx, _ptr(ms), C.addressof(n)), ctx)
+    return ms[:n.value].copy()
+
+
 # ---- small conveniences for tests / bench (marshalling only) -----------------------------
 def layer_desc(cfg, max_tokens, expert_kernel=CAEE_KERNEL_AUTO, device=-1):
     """caee_layer_desc from a workloads.LayerConfig."""
     return caee_layer_desc(cfg.H, cfg.I, cfg.E, cfg.S, cfg.k, cfg.n_group, cfg.topk_group, cfg.score_fn,
                            int(cfg.norm_topk), cfg.routed_scale, cfg.act_dtype, cfg.w_dtype, cfg.D, int(max_tokens),
                            expert_kernel, device)
+
+
+def caee_kernel_is_simt(cfg, kernel):
+    """Mirror of caee_create's AUTO rule: which expert kernel a descriptor resolves to."""
+    umma_ok = cfg.w_dtype == CAEE_BF16 and cfg.act_dtype == CAEE_BF16 and cfg.H % 256 == 0 and cfg.I % 128 == 0
+    return kernel == CAEE_KERNEL_SIMT or (kernel == CAEE_KERNEL_AUTO and not umma_ok)
 
 
 def prune_params(mode, theta=0.0, flags=0):

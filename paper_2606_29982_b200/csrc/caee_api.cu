@@ -127,6 +127,8 @@ void free_all(caee_ctx* c) {
     if (c->packed.on_host[e]) cudaFreeHost(c->packed.base[e]);
     else cudaFree(c->packed.base[e]);
   }
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+  c->prof_ev.clear();
   if (c->side_stream) cudaStreamDestroy(c->side_stream);
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
@@ -223,8 +225,11 @@ caee_status caee_create(const caee_layer_desc* desc, caee_ctx** out) {
   c->device = dev;
   c->num_sms = prop.multiProcessorCount;
   c->wl = caee_worklist{};
-  c->kernel = desc->expert_kernel == CAEE_KERNEL_AUTO ? (desc->w_dtype == CAEE_F32 ? CAEE_KERNEL_SIMT : CAEE_KERNEL_UMMA)
-                                                       : desc->expert_kernel;
+  c->kernel = desc->expert_kernel;
+  if (c->kernel == CAEE_KERNEL_AUTO) {
+    std::string why;
+    c->kernel = caee_umma_supported(c, &why) == CAEE_OK ? CAEE_KERNEL_UMMA : CAEE_KERNEL_SIMT;
+  }
   if (c->kernel == CAEE_KERNEL_UMMA) {
     std::string why;
     rc = caee_umma_supported(c, &why);
@@ -435,8 +440,11 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   cudaStream_t st = (cudaStream_t)stream;
   rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);
   if (rc != CAEE_OK) return rc;
+  const bool prof = (size_t)c->prof_used * 2 + 1 < c->prof_ev.size();
+  if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
   if (c->kernel == CAEE_KERNEL_SIMT) caee_launch_expert_simt(c, x, T, st);
   else caee_launch_expert_umma(c, x, T, st);
+  if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);
   caee_launch_combine(c, T, c->idx, c->gate, y, st);
   caee_launch_stats(c, stats, p != nullptr, st);
   return after_launch(c, "caee_moe_forward");
@@ -451,6 +459,31 @@ caee_status caee_moe_forward_from_scores(caee_ctx* c, const void* x, const float
                                          const caee_prune_params* p, void* y, caee_fwd_stats* stats, void* stream) {
   if (c && !scores && T > 0) return caee_fail(c, CAEE_EINVAL, "scores is NULL");
   return forward_impl(c, x, scores, T, p, y, stats, stream);
+}
+
+caee_status caee_profile(caee_ctx* c, int32_t n_slots) {
+  if (!c) return CAEE_EINVAL;
+  if (n_slots < 0 || n_slots > 65536) return caee_fail(c, CAEE_EINVAL, "n_slots must be in 0..65536");
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+  c->prof_ev.assign((size_t)n_slots * 2, nullptr);
+  c->prof_used = 0;
+  for (auto& e : c->prof_ev) CAEE_CUDA(c, cudaEventCreate(&e));
+  return CAEE_OK;
+}
+
+caee_status caee_profile_read(caee_ctx* c, float* expert_ms, int32_t* n_out) {
+  if (!c) return CAEE_EINVAL;
+  if (!expert_ms || !n_out) return caee_fail(c, CAEE_EINVAL, "expert_ms or n_out is NULL");
+  DeviceGuard g(c->device);
+  for (int i = 0; i < c->prof_used; ++i) {
+    CAEE_CUDA(c, cudaEventSynchronize(c->prof_ev[2 * i + 1]));
+    CAEE_CUDA(c, cudaEventElapsedTime(&expert_ms[i], c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+  }
+  *n_out = c->prof_used;
+  c->prof_used = 0;
+  return CAEE_OK;
 }
 
 caee_status caee_last_routing(caee_ctx* c, int32_t T, int32_t* idx, float* gate, void* stream) {

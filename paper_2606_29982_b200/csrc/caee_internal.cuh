@@ -97,6 +97,10 @@ struct caee_ctx {
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
+  // optional expert-kernel timing (caee_profile)
+  std::vector<cudaEvent_t> prof_ev;  // 2 per slot
+  int prof_used = 0;
+
   // offload
   cudaStream_t side_stream = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;

@@ -25,9 +25,9 @@
 // Roles (256 threads, 1 CTA per SM):  warp 0 = weight producer (one lane issues bulk copies),
 // warp 1 = MMA issuer (one lane), warps 2-3 = token-operand loaders (warp 2 also owns TMEM
 // alloc/free), warps 4-7 = epilogue (TMEM -> registers -> SwiGLU -> h, or -> o rows).
-// Tiles are dealt round-robin: all phase-1 tiles precede all phase-2 tiles in every CTA's
-// order, and a phase-2 tile only waits (per-run counter) for phase-1 tiles, which never wait,
-// so the schedule cannot deadlock while the grid is co-resident (grid = #SMs, 1 CTA/SM).
+// Tiles are claimed dynamically (one atomic ticket per tile, phase-1 tickets first); a
+// phase-2 tile only waits (per-run counter) for phase-1 tiles, which never wait, so the
+// schedule cannot deadlock and CTAs that finish early simply claim more tiles.
 #include "caee_internal.cuh"
 
 namespace {
@@ -116,12 +116,6 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ uint4 ld_cg16(const void* p) {
-  uint4 v;
-  asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-  return v;
-}
-
 struct Tile {
   int phase, run, sub;  // sub = ft (phase 1) or op (phase 2)
 };
@@ -134,16 +128,40 @@ __device__ __forceinline__ bool tile_at(int i, int n_runs, int P1, int P2, Tile&
 }
 
 // ------------------------------------------------------------------ the kernel
+constexpr int kQueue = 4;      // tile-queue depth (producer runs at most this many tiles ahead)
+constexpr int kLag = 3;        // token-operand stages each loader warp keeps in flight (cp.async groups)
+
+// Next tile index for a role.  The weight producer claims tiles with one atomic ticket per
+// tile and broadcasts them through a small shared-memory queue; every other role pops the
+// same sequence.  Tickets are claimed in increasing order, phase-1 tiles have the lower
+// tickets, and a phase-1 tile never waits on another tile: a phase-2 tile's wait for its
+// run's h therefore always ends (the CTAs holding those phase-1 tickets are running).
+struct TileQueue {
+  uint32_t full0, empty0;  // mbarrier addresses
+  int* slots;
+  int q, ph;
+  __device__ __forceinline__ int pop() {
+    mbar_wait(full0 + 8 * q, ph);
+    const int t = slots[q];
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(empty0 + 8 * q);
+    if (++q == kQueue) { q = 0; ph ^= 1; }
+    return t;
+  }
+};
+
 __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 4];
+  __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 4 + 2 * kQueue];
   __shared__ uint32_t tmem_base_s;
+  __shared__ int tq_slots[kQueue];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kMaxStages]);
   const uint32_t tfull0 = smem_u32(&bars[2 * kMaxStages]), tempty0 = smem_u32(&bars[2 * kMaxStages + 2]);
+  const uint32_t qfull0 = smem_u32(&bars[2 * kMaxStages + 4]), qempty0 = smem_u32(&bars[2 * kMaxStages + 4 + kQueue]);
   const int n_runs = p.wl.meta[1];
 
   if (threadIdx.x == 0) {
@@ -154,6 +172,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull0 + 8 * a, 1);   // tcgen05.commit
       mbar_init(tempty0 + 8 * a, 4);  // one lane of each epilogue warp
+    }
+    for (int q = 0; q < kQueue; ++q) {
+      mbar_init(qfull0 + 8 * q, 1);   // producer
+      mbar_init(qempty0 + 8 * q, 7);  // MMA warp + 2 loader warps + 4 epilogue warps
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -166,13 +188,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
+  Tile t;
 
   if (warp == 0) {
-    // ===== weight producer: one 32 KB bulk copy per stage, straight from the packed image
+    // ===== weight producer: claims tiles; one 32 KB bulk copy per stage from the packed image
     if (lane == 0) {
-      int stage = 0, ph = 0;
-      Tile t;
-      for (int i = blockIdx.x; tile_at(i, n_runs, p.P1, p.P2, t); i += gridDim.x) {
+      int stage = 0, ph = 0, q = 0, qph = 0;
+      for (;;) {
+        mbar_wait(qempty0 + 8 * q, qph ^ 1);
+        const int i = atomicAdd(p.wl.sched, 1);
+        tq_slots[q] = i;
+        mbar_arrive(qfull0 + 8 * q);
+        if (++q == kQueue) { q = 0; qph ^= 1; }
+        if (!tile_at(i, n_runs, p.P1, p.P2, t)) break;
         const int e = p.wl.run_expert[t.run];
         const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
         const uint8_t* src = p.packed[e] + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes;
@@ -185,11 +214,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer
-    if (lane == 0) {
-      int stage = 0, ph = 0, it = 0;
-      Tile t;
-      for (int i = blockIdx.x; tile_at(i, n_runs, p.P1, p.P2, t); i += gridDim.x, ++it) {
+    // ===== MMA issuer (the whole warp pops the queue; one lane issues)
+    int stage = 0, ph = 0;
+    for (int it = 0; tile_at(tq.pop(), n_runs, p.P1, p.P2, t); ++it) {
+      if (lane == 0) {
         const int as = it & 1;
         const int npad = (p.wl.run_n[t.run] + 15) & ~15;
         const uint32_t idesc = make_idesc(npad);
@@ -212,19 +240,33 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
           if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
         }
         tc_commit(tfull0 + 8 * as);
+      } else {
+        // keep the ring position in step with lane 0
+        const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+        stage = (stage + nkb) % p.n_stages;
       }
+      __syncwarp();
     }
   } else if (warp == 2 || warp == 3) {
-    // ===== token-operand loaders: gather B rows (x or h) into the canonical K-major layout
+    // ===== token-operand loaders: gather B rows (x or h) into the canonical K-major layout with
+    // cp.async, kLag stages in flight per warp so that L2 latency is off the critical path
     const int wq = warp - 2;
     const int r8 = lane & 7, c4 = lane >> 3;  // row in 8-row group, 16-byte chunk (c4 and c4+4)
-    int stage = 0, ph = 0;
-    Tile t;
-    for (int i = blockIdx.x; tile_at(i, n_runs, p.P1, p.P2, t); i += gridDim.x) {
+    int stage = 0, ph = 0, pend_stage = 0, pending = 0;
+    auto publish = [&](int count) {  // the oldest `count` in-flight stages have landed
+      fence_proxy_async_smem();
+      __syncwarp();
+      for (int j = 0; j < count; ++j) {
+        if (lane == 0) mbar_arrive(full0 + 8 * pend_stage);
+        if (++pend_stage == p.n_stages) pend_stage = 0;
+      }
+      pending -= count;
+    };
+    while (tile_at(tq.pop(), n_runs, p.P1, p.P2, t)) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       const int ngroups = (n + 15) / 16 * 2;  // 8-row groups in the padded tile
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-      const uint8_t* rowp[8];  // this lane's source row in each of its groups
+      const uint8_t* rowp[8];  // this lane's source row in each of its groups (nullptr: zero fill)
 #pragma unroll
       for (int g = 0; g < 8; ++g) {
         const int row = (2 * g + wq) * 8 + r8;
@@ -245,39 +287,32 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty0 + 8 * stage, ph ^ 1);
         const uint32_t b_addr = smem_base + stage * p.stage_bytes + kAStageBytes;
-        uint4 v[8][2];
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          if (2 * g + wq < ngroups) {
-            if (rowp[g]) {
-              v[g][0] = ld_cg16(rowp[g] + (size_t)kb * 128 + c4 * 16);
-              v[g][1] = ld_cg16(rowp[g] + (size_t)kb * 128 + (c4 + 4) * 16);
-            } else {
-              v[g][0] = make_uint4(0, 0, 0, 0);
-              v[g][1] = make_uint4(0, 0, 0, 0);
-            }
-          }
-        }
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
           if (2 * g + wq < ngroups) {
             const uint32_t a = b_addr + (2 * g + wq) * 1024 + r8 * 16;
-            asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a + c4 * 128), "r"(v[g][0].x), "r"(v[g][0].y), "r"(v[g][0].z), "r"(v[g][0].w) : "memory");
-            asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a + (c4 + 4) * 128), "r"(v[g][1].x), "r"(v[g][1].y), "r"(v[g][1].z), "r"(v[g][1].w) : "memory");
+            const uint8_t* src = rowp[g] ? rowp[g] + (size_t)kb * 128 + c4 * 16 : reinterpret_cast<const uint8_t*>(p.x);
+            const uint32_t sz = rowp[g] ? 16u : 0u;  // src-size 0: zero fill
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + c4 * 128), "l"(src), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + (c4 + 4) * 128), "l"(src + (rowp[g] ? 64 : 0)), "r"(sz) : "memory");
           }
         }
-        fence_proxy_async_smem();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(full0 + 8 * stage);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        ++pending;
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+        if (pending > kLag) {
+          asm volatile("cp.async.wait_group %0;" ::"n"(kLag) : "memory");
+          publish(1);
+        }
       }
+      // flush at the tile boundary: nothing of this tile may wait behind a later tile's dependency
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      publish(pending);
     }
   } else {
     // ===== epilogue: TMEM -> registers -> SwiGLU -> h (phase 1) or -> o rows (phase 2)
     const int q = warp - 4;  // TMEM lane quadrant of this warp (warp % 4)
-    int it = 0;
-    Tile t;
-    for (int i = blockIdx.x; tile_at(i, n_runs, p.P1, p.P2, t); i += gridDim.x, ++it) {
+    for (int it = 0; tile_at(tq.pop(), n_runs, p.P1, p.P2, t); ++it) {
       const int as = it & 1;
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       mbar_wait(tfull0 + 8 * as, (it >> 1) & 1);

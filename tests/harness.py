@@ -8,37 +8,16 @@ import torch
 
 from oracle import oracle as orc
 from paper_2606_29982_b200 import binding as B
+from paper_2606_29982_b200.layer import Layer
 from paper_2606_29982_b200 import workloads as wl
 
 TOL = {wl.DT_F32: 1e-4, wl.DT_BF16: 2e-2, wl.DT_E4M3: 5e-2}   # x RMS(y), BASELINE.json north_star
 
 
-class GpuLayer:
+class GpuLayer(Layer):
     def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=True, device="cuda:0"):
-        self.cfg, self.seed, self.device, self.max_tokens = cfg, seed, device, max_tokens
-        self.ctx = B.caee_create(B.layer_desc(cfg, max_tokens, kernel))
-        self.Wr, self.b_logit, self.corr_bias = wl.router(cfg, seed, device)
-        B.caee_set_router(self.ctx, self.Wr, self.b_logit, self.corr_bias)
-        self.part = wl.partitions(cfg)
-        B.caee_set_partitions(self.ctx, self.part, cfg.D)
-        self.resident = wl.residency(cfg, seed)
-        self.ticks_res, self.ticks_miss = wl.cost_tables(cfg)
-        B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
-        n = cfg.E + cfg.S
-        raw = [wl.expert_weights(cfg, seed, e, device) for e in range(n)]
-        fp8 = cfg.w_dtype == wl.DT_E4M3
-        B.caee_set_weights(self.ctx, [r["gate"] for r in raw], [r["up"] for r in raw], [r["down"] for r in raw],
-                           [r["gate_scale"] for r in raw] if fp8 else None, [r["up_scale"] for r in raw] if fp8 else None,
-                           [r["down_scale"] for r in raw] if fp8 else None, pack=1)
-        torch.cuda.synchronize()
-        self.raw = raw if keep_raw else None
+        super().__init__(cfg, seed, max_tokens, kernel, keep_raw, device)
         self._host = {}
-
-    def close(self):
-        if self.ctx is not None:
-            B.caee_destroy(self.ctx)
-            self.ctx = None
-            self.raw = None
 
     # ---- host copies of exactly the bits the GPU holds
     def host_expert(self, e):
@@ -85,22 +64,10 @@ class GpuLayer:
 
     # ---- GPU calls (through the C ABI)
     def forward(self, x, params=None, scores=None, want_stats=False):
-        T = x.shape[0]
-        y = torch.empty_like(x)
         stats = B.stats_buffer(self.device) if want_stats else None
-        if scores is None:
-            B.caee_moe_forward(self.ctx, x, T, params, y, stats)
-        else:
-            B.caee_moe_forward_from_scores(self.ctx, x, scores, T, params, y, stats)
+        y = super().forward(x, params, scores, stats=stats)
         torch.cuda.synchronize()
         return (y, B.read_stats(stats)) if want_stats else y
-
-    def last_routing(self, T):
-        idx = torch.empty(T, self.cfg.k, dtype=torch.int32, device=self.device)
-        gate = torch.empty(T, self.cfg.k, dtype=torch.float32, device=self.device)
-        B.caee_last_routing(self.ctx, T, idx, gate)
-        torch.cuda.synchronize()
-        return idx.cpu().numpy(), gate.cpu().numpy()
 
 
 def check_y(y_gpu, y_ref, tokens, tol):

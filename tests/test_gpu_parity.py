@@ -222,3 +222,30 @@ def test_calibrate_cost(H):
         assert orc.cost_ticks(f_hbm.slope_ns_per_byte, f_hbm.intercept_ns, 3 * C2S.H * C2S.I * 2) > 0
     finally:
         L.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# Full-size configurations of BASELINE.json, in the launch configuration bench.py times.
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_forward_c2_full(H, seed):
+    """Config 2 (mid bf16 layer, 64+2 experts): every decode batch, every token, all seeds."""
+    L = H.GpuLayer(wl.C2, seed=seed, max_tokens=128)
+    try:
+        for T, mode in ((1, "dense"), (8, "cir"), (32, "thresh"), (128, "frac")):
+            toks = None if T <= 32 else list(range(0, T, 8))
+            _forward_case(H, L, T, mode, tokens=toks, seed=40 + seed)
+    finally:
+        L.close()
+
+
+@pytest.mark.parametrize("T,mode", [(128, "thresh"), (128, "dense"), (8, "cir"), (1, "dense"), (32, "frac")])
+def test_forward_c3_full_size_sampled(H, T, mode):
+    """Config 3 (DeepSeek-R1-shaped bf16, 22.5 GB of experts): K_final and F_* for the whole batch
+    bit-exact, y on sampled tokens the oracle computes one by one."""
+    L = H.GpuLayer(wl.C3, seed=0, max_tokens=128, keep_raw=False)
+    try:
+        toks = sorted(set([0, T // 3, T - 1]))
+        r = _forward_case(H, L, T, mode, tokens=toks, seed=100)
+        print(f"C3 T={T} {mode}: max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
