@@ -210,6 +210,13 @@ def run_caee(args, cfg, prune):
     for i in range(W):
         step(i)
     torch.cuda.synchronize()
+    # the batches rotate and each keeps a different number of experts: note, per batch, the
+    # weight bytes its expert-kernel launch streams (untimed; caee_fwd_stats.weight_bytes)
+    batch_bytes = []
+    for i in range(len(xs)):
+        step(i)
+        torch.cuda.synchronize()
+        batch_bytes.append(B.read_stats(stats).weight_bytes)
     # --- device-resident timing, with the expert kernel timed by its own event pair
     B.caee_profile(L.ctx, K)
     clocks = ClockSampler(local)
@@ -246,12 +253,16 @@ def run_caee(args, cfg, prune):
         return
     peak, peak_src = peaks()
     k_ms = float(statistics.mean(expert_ms)) if len(expert_ms) else None
-    achieved = st.weight_bytes / (k_ms * 1e-3) / 1e9 if k_ms else None
+    launch_bytes = [batch_bytes[i % len(xs)] for i in range(len(expert_ms))]     # launch i ran batch i % 4
+    bytes_per_launch = float(statistics.mean(launch_bytes)) if launch_bytes else None
+    achieved = bytes_per_launch / (k_ms * 1e-3) / 1e9 if k_ms else None
+    # dram bytes per launch from the committed ncu --set full capture of this same command
+    # (profiles/traffic.json, written from the .ncu-rep by hand; null when not captured)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(f"{cfg.name}/T{T}/{args.prune}")
+            traffic = json.load(f).get(f"{cfg.name}/T{T}/{args.prune}", {}).get("dram_bytes_per_launch")
     launches_per_step = 2 + (2 if prune is not None and prune[0] != 0 else (1 if prune is not None else 0)) + 3 + 1 + 1 + 1
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -266,7 +277,8 @@ def run_caee(args, cfg, prune):
         "gpu_launches": launches_per_step * K,
         "roofline": {"bound": "hbm", "kernel": "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if achieved else None, "traffic": traffic, "peak_source": peak_src,
-                     "bytes_per_launch": st.weight_bytes, "kernel_ms": k_ms,
+                     "bytes_per_launch": bytes_per_launch, "kernel_ms": k_ms,
+                     "bytes_by_batch": batch_bytes,
                      "frac_of_8TBps_nominal": achieved / 8000.0 if achieved else None},
         "latency_us": {"pruned": ms_step * 1e3, "dense": dense_ms * 1e3, "expert_kernel": k_ms * 1e3 if k_ms else None},
         "pruning": {"n_act": st.n_act, "n_keep": st.n_keep, "n_run": st.n_run, "F_cost_dense": st.F_cost_dense,
