@@ -18,7 +18,10 @@
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *    caee_route, caee_route_from_scores, caee_prune, caee_moe_forward and
  *    caee_moe_forward_from_scores only enqueue work: no host synchronisation, no
- *    allocation.  caee_calibrate_cost and the caee_set_* calls synchronise.
+ *    allocation.  One exception: when some experts are non-resident (caee_set_residency),
+ *    caee_moe_forward* waits once for its own decision kernels, because the host must learn
+ *    which non-resident experts survived pruning before it can issue their copies
+ *    ("transfer engine").  caee_calibrate_cost and the caee_set_* calls synchronise.
  *  - Errors: every call returns CAEE_OK (0) or a negative code; nothing throws or
  *    aborts across the ABI.  caee_last_error gives a human-readable reason.
  *    A CUDA failure is sticky for the context (CAEE_ECUDA from then on).
@@ -89,8 +92,10 @@ typedef struct caee_layer_desc {
 
 /* Per-expert weight pointers: host arrays of E+S entries, routed experts first, then the
  * shared ones.  gate/up: [I,H]; down: [H,I]; *_scale (e4m3 only, else may be NULL):
- * [ceil(rows/128), ceil(cols/128)] fp32.  Entries point to device memory, or, where
- * resident[e] == 0 (caee_set_residency), to pinned host memory. */
+ * [ceil(rows/128), ceil(cols/128)] fp32.  Entries point to device memory or to pinned
+ * (device-accessible) host memory; with pack != 0 the library's own image of an expert with
+ * resident[e] == 0 (caee_set_residency) is kept in pinned host memory wherever the caller's
+ * copy was. */
 typedef struct caee_expert_weights {
   const void* const* gate;
   const void* const* up;
@@ -165,9 +170,14 @@ const char* caee_last_error(const caee_ctx* ctx);
  * corr_bias [E] or NULL (added to the score for SELECTION only, R1). */
 caee_status caee_set_router(caee_ctx* ctx, const float* W_r, const float* b_logit, const float* corr_bias);
 /* Expert weights.  pack != 0: the library repacks each expert once into its own tile-major
- * copy (device memory for resident experts, pinned host memory otherwise) and no longer
- * refers to the caller's buffers afterwards.  The UMMA kernel requires pack != 0.
- * Call caee_set_residency first when some experts live in host memory. */
+ * copy (device memory for resident experts; pinned host memory plus a device staging slot of
+ * the same size for non-resident ones) and no longer refers to the caller's buffers
+ * afterwards.  The UMMA kernel (bf16 or e4m3 weights with bf16 activations) requires
+ * pack != 0; the SIMT kernel reads the caller's buffers in place and needs every expert in
+ * device memory.  The e4m3 UMMA kernel contracts in fp16 (fp32 accumulate): |x| and the
+ * SwiGLU intermediate must stay below 65504.
+ * Call caee_set_residency first when some experts live in host memory (changing the
+ * residency afterwards invalidates the weights: set them again). */
 caee_status caee_set_weights(caee_ctx* ctx, const caee_expert_weights* w, int32_t pack);
 /* E_d of PAPER.md:127 as part_of_expert[e] in 0..D-1 (host).  Default: contiguous blocks. */
 caee_status caee_set_partitions(caee_ctx* ctx, const int32_t* part_of_expert, int32_t D);
@@ -199,7 +209,9 @@ caee_status caee_route_from_scores(caee_ctx* ctx, const float* scores, int32_t T
 caee_status caee_prune(caee_ctx* ctx, const caee_prune_params* p, const float* scores, int32_t T, int32_t* idx,
                        float* gate, const caee_prune_out* out, void* stream);
 /* The whole layer: route -> prune (p != NULL) -> fetch of surviving non-resident experts on
- * a side stream -> grouped SwiGLU FFN over the surviving experts only -> combine
+ * a side stream (one cudaMemcpyAsync per surviving miss, overlapped with the resident experts'
+ * compute; stats->n_fetch / h2d_bytes count them) -> grouped SwiGLU FFN over the surviving
+ * experts only -> combine
  *   y_t = routed_scale * sum_{e in K_final} G(t)_e E_e(t) + sum_shared E_sh(t).
  * x, y dev [T,H] act dtype; stats dev or NULL. */
 caee_status caee_moe_forward(caee_ctx* ctx, const void* x, int32_t T, const caee_prune_params* p, void* y,

@@ -231,7 +231,8 @@ def layer_desc(cfg, max_tokens, expert_kernel=CAEE_KERNEL_AUTO, device=-1):
 
 def caee_kernel_is_simt(cfg, kernel):
     """Mirror of caee_create's AUTO rule: which expert kernel a descriptor resolves to."""
-    umma_ok = cfg.w_dtype == CAEE_BF16 and cfg.act_dtype == CAEE_BF16 and cfg.H % 256 == 0 and cfg.I % 128 == 0
+    umma_ok = (cfg.w_dtype in (CAEE_BF16, CAEE_E4M3) and cfg.act_dtype == CAEE_BF16 and cfg.H % 256 == 0
+               and cfg.I % 128 == 0)
     return kernel == CAEE_KERNEL_SIMT or (kernel == CAEE_KERNEL_AUTO and not umma_ok)
 
 

@@ -119,7 +119,7 @@ void free_all(caee_ctx* c) {
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
-                  c->packed.dev_ptrs};
+                  c->packed.dev_ptrs, c->x16};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (size_t e = 0; e < c->packed.base.size(); ++e) {
@@ -127,6 +127,10 @@ void free_all(caee_ctx* c) {
     if (c->packed.on_host[e]) cudaFreeHost(c->packed.base[e]);
     else cudaFree(c->packed.base[e]);
   }
+  for (uint8_t* p : c->stage_slot)
+    if (p) cudaFree(p);
+  for (cudaEvent_t e : c->fetch_ev) cudaEventDestroy(e);
+  if (c->host_meta) cudaFreeHost(c->host_meta);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   c->prof_ev.clear();
   if (c->side_stream) cudaStreamDestroy(c->side_stream);
@@ -150,10 +154,13 @@ caee_status create_impl(caee_ctx* c) {
   A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
   A(c->wl.ent_tok, Tm * (k + S)); A(c->wl.ent_slot, Tm * k); A(c->wl.ent_wt, Tm * k); A(c->wl.ent_dst, Tm * (k + S));
   A(c->wl.run_expert, c->wl.max_runs); A(c->wl.run_start, c->wl.max_runs); A(c->wl.run_n, c->wl.max_runs);
-  A(c->wl.run_hrow, c->wl.max_runs); A(c->wl.meta, 16); A(c->wl.sched, 2 + c->wl.max_runs);
+  c->wl.n_tickets = (int)E + 2;
+  A(c->wl.run_hrow, c->wl.max_runs); A(c->wl.meta, 16); A(c->wl.sched, c->wl.n_tickets + c->wl.max_runs);
+  c->wl.ready = c->wl.sched + c->wl.n_tickets;
   c->h_rows_cap = Tm * k + 15 * std::min(E, Tm * k) + S * (Tm + 15) + 16;
   if (c->kernel == CAEE_KERNEL_SIMT) { A(c->hbuf_f32, c->h_rows_cap * d.I); }
   else { A(c->hbuf_b16, c->h_rows_cap * d.I); }
+  if (c->kernel == CAEE_KERNEL_UMMA && d.w_dtype == CAEE_E4M3) { A(c->x16, Tm * d.H); }
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
@@ -168,6 +175,7 @@ caee_status create_impl(caee_ctx* c) {
   CAEE_CUDA(c, cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking));
   CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
   CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+  CAEE_CUDA(c, cudaMallocHost((void**)&c->host_meta, sizeof(int32_t) * (16 + c->wl.max_runs)));
   return CAEE_OK;
 }
 
@@ -287,7 +295,12 @@ caee_status caee_set_residency(caee_ctx* c, const uint8_t* resident) {
   if (!resident) return caee_fail(c, CAEE_EINVAL, "resident is NULL");
   DeviceGuard g(c->device);
   CAEE_CUDA(c, cudaDeviceSynchronize());
-  for (int e = 0; e < c->d.E; ++e) c->resident_h[e] = resident[e] ? 1 : 0;
+  bool changed = false;
+  for (int e = 0; e < c->d.E; ++e) {
+    changed |= c->resident_h[e] != (resident[e] ? 1 : 0);
+    c->resident_h[e] = resident[e] ? 1 : 0;
+  }
+  if (changed) c->have_weights = false;  // where an expert's image lives follows its residency: set the weights again
   return upload_costs(c);
 }
 
@@ -338,13 +351,39 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     P.base.assign(n, nullptr); P.on_host.assign(n, 0);
     P.bytes_per_expert = caee_umma_packed_bytes(c);
     if (!P.dev_ptrs) CAEE_CUDA(c, cudaMalloc((void**)&P.dev_ptrs, pb));
+    for (uint8_t* q : c->stage_slot)
+      if (q) cudaFree(q);
+    for (cudaEvent_t ev : c->fetch_ev) cudaEventDestroy(ev);
+    c->stage_slot.assign(n, nullptr);
+    c->fetch_ev.clear();
+    c->any_offload = false;
+    std::vector<uint8_t*> dptr(n, nullptr);
+    uint8_t* tmp = nullptr;  // device scratch for packing a host-resident expert
     for (int e = 0; e < n; ++e) {
       const bool res = e >= c->d.E || c->resident_h[e];
-      if (!res) return caee_fail(c, CAEE_EUNSUPPORTED, "non-resident experts are not supported by the UMMA path yet");
-      CAEE_CUDA(c, cudaMalloc((void**)&P.base[e], P.bytes_per_expert));
-      caee_launch_pack_expert(c, e, P.base[e], c->wg_h[e], c->wu_h[e], c->wd_h[e], c->sg_h[e], c->su_h[e], c->sd_h[e], 0);
+      if (res) {
+        CAEE_CUDA(c, cudaMalloc((void**)&P.base[e], P.bytes_per_expert));
+        caee_launch_pack_expert(c, e, P.base[e], c->wg_h[e], c->wu_h[e], c->wd_h[e], c->sg_h[e], c->su_h[e], c->sd_h[e], 0);
+        dptr[e] = P.base[e];
+      } else {
+        // S9: the image of a non-resident expert stays in pinned host memory; it is copied into
+        // its device staging slot by caee_moe_forward only when the expert survives pruning
+        if (!tmp) CAEE_CUDA(c, cudaMalloc((void**)&tmp, P.bytes_per_expert));
+        caee_launch_pack_expert(c, e, tmp, c->wg_h[e], c->wu_h[e], c->wd_h[e], c->sg_h[e], c->su_h[e], c->sd_h[e], 0);
+        CAEE_CUDA(c, cudaMallocHost((void**)&P.base[e], P.bytes_per_expert));
+        P.on_host[e] = 1;
+        CAEE_CUDA(c, cudaMemcpy(P.base[e], tmp, P.bytes_per_expert, cudaMemcpyDeviceToHost));
+        CAEE_CUDA(c, cudaMalloc((void**)&c->stage_slot[e], P.bytes_per_expert));
+        dptr[e] = c->stage_slot[e];
+        cudaEvent_t ev;
+        CAEE_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        c->fetch_ev.push_back(ev);
+        c->any_offload = true;
+      }
     }
-    CAEE_CUDA(c, cudaMemcpy(P.dev_ptrs, P.base.data(), pb, cudaMemcpyHostToDevice));
+    CAEE_CUDA(c, cudaDeviceSynchronize());
+    if (tmp) cudaFree(tmp);
+    CAEE_CUDA(c, cudaMemcpy(P.dev_ptrs, dptr.data(), pb, cudaMemcpyHostToDevice));
     CAEE_CUDA(c, cudaDeviceSynchronize());
   } else {
     for (int e = 0; e < c->d.E; ++e)
@@ -441,12 +480,49 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);
   if (rc != CAEE_OK) return rc;
   const bool prof = (size_t)c->prof_used * 2 + 1 < c->prof_ev.size();
-  if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
-  if (c->kernel == CAEE_KERNEL_SIMT) caee_launch_expert_simt(c, x, T, st);
-  else caee_launch_expert_umma(c, x, T, st);
+  int n_fetch = 0;
+  if (c->kernel == CAEE_KERNEL_SIMT) {
+    if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
+    caee_launch_expert_simt(c, x, T, st);
+  } else if (!c->any_offload) {
+    caee_launch_umma_prepare(c, x, T, st);
+    if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
+    caee_launch_expert_umma(c, x, T, 0, -1, 0, st);
+  } else {
+    // S9 (Fig. 8): only the non-resident experts that survived pruning are
+    // fetched, one cudaMemcpyAsync each on the side stream, while the resident experts (first
+    // in the run list) are already computing on the caller's stream.  The host has to learn
+    // which experts survived: this is the one host synchronisation of an offloading step.
+    caee_launch_umma_prepare(c, x, T, st);
+    CAEE_CUDA(c, cudaMemcpyAsync(c->host_meta, c->wl.meta, sizeof(int32_t) * 16, cudaMemcpyDeviceToHost, st));
+    CAEE_CUDA(c, cudaMemcpyAsync(c->host_meta + 16, c->wl.run_expert, sizeof(int32_t) * c->wl.max_runs, cudaMemcpyDeviceToHost, st));
+    CAEE_CUDA(c, cudaStreamSynchronize(st));
+    const int n_runs = c->host_meta[1], n_res = c->host_meta[4];
+    const int32_t* run_expert = c->host_meta + 16;
+    CAEE_CUDA(c, cudaEventRecord(c->ev_fork, st));                 // staging slots may still be read by the previous step
+    CAEE_CUDA(c, cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0));
+    struct Seg { int e, begin, count; };
+    std::vector<Seg> segs;
+    for (int r = n_res; r < n_runs; ++r) {
+      if (!segs.empty() && segs.back().e == run_expert[r]) ++segs.back().count;
+      else segs.push_back({run_expert[r], r, 1});
+    }
+    for (size_t i = 0; i < segs.size(); ++i) {
+      const int e = segs[i].e;
+      CAEE_CUDA(c, cudaMemcpyAsync(c->stage_slot[e], c->packed.base[e], c->packed.bytes_per_expert, cudaMemcpyHostToDevice, c->side_stream));
+      CAEE_CUDA(c, cudaEventRecord(c->fetch_ev[i], c->side_stream));
+    }
+    n_fetch = (int)segs.size();
+    if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
+    if (n_res > 0) caee_launch_expert_umma(c, x, T, 0, n_res, 0, st);
+    for (size_t i = 0; i < segs.size(); ++i) {
+      CAEE_CUDA(c, cudaStreamWaitEvent(st, c->fetch_ev[i], 0));
+      caee_launch_expert_umma(c, x, T, segs[i].begin, segs[i].count, 1 + (int)i, st);
+    }
+  }
   if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);
   caee_launch_combine(c, T, c->idx, c->gate, y, st);
-  caee_launch_stats(c, stats, p != nullptr, st);
+  caee_launch_stats(c, stats, p != nullptr, n_fetch, st);
   return after_launch(c, "caee_moe_forward");
 }
 

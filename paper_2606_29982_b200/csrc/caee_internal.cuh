@@ -33,9 +33,11 @@ struct caee_worklist {
   int32_t* run_start;   // [max_runs] first entry
   int32_t* run_n;       // [max_runs] tokens in the run, 1..CAEE_RUN_TOKENS
   int32_t* run_hrow;    // [max_runs] first row of the run in the h scratch (rows padded to 16 per run)
-  int32_t* meta;        // [16]: 0 n_run(ABI) 1 n_runs 2 n_entries(routed) 3 h rows total 4.. reserved
-  int32_t* sched;       // [2 + max_runs]: 0 ticket, 1 unused, 2.. per-run ready counters
-  int32_t max_runs;
+  int32_t* meta;        // [16]: 0 n_run(ABI) 1 n_runs 2 n_entries(routed) 3 h rows total
+                        //       4 runs of resident + shared experts (they come first) 5.. reserved
+  int32_t* sched;       // [n_tickets + max_runs]: tile-ticket counters (one per expert-kernel launch of a step),
+  int32_t* ready;       //   then (= sched + n_tickets) per-run "h complete" counters; zeroed every step
+  int32_t max_runs, n_tickets;
 };
 
 struct caee_packed {
@@ -93,7 +95,8 @@ struct caee_ctx {
   int64_t* scalars = nullptr;  // [8]
   caee_worklist wl;
   float* hbuf_f32 = nullptr;         // SIMT: h rows [rows, I] fp32
-  __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16/fp16
+  __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16 (bf16 weights) / fp16 (e4m3 weights)
+  __half* x16 = nullptr;             // UMMA e4m3: fp16 copy of x [Tmax, H]
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
@@ -101,9 +104,15 @@ struct caee_ctx {
   std::vector<cudaEvent_t> prof_ev;  // 2 per slot
   int prof_used = 0;
 
-  // offload
+  // offload (S9): packed images of non-resident experts live in pinned host memory
+  // (packed.base[e], on_host) and are copied into their staging slot (stage_slot[e], device)
+  // on the side stream, only when they survive pruning
   cudaStream_t side_stream = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  std::vector<uint8_t*> stage_slot;      // [E+S] device staging slot of a non-resident expert, else NULL
+  std::vector<cudaEvent_t> fetch_ev;     // one per non-resident expert
+  int32_t* host_meta = nullptr;          // pinned: meta[16] then run_expert[max_runs]
+  bool any_offload = false;
 };
 
 caee_status caee_fail(caee_ctx* c, caee_status code, const char* fmt, ...);
@@ -137,9 +146,10 @@ caee_status caee_umma_supported(const caee_ctx* c, std::string* why);
 size_t caee_umma_packed_bytes(const caee_ctx* c);
 void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst_dev, const void* g, const void* u, const void* d,
                              const float* sg, const float* su, const float* sd, cudaStream_t s);
-void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, cudaStream_t s);
+void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
+void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
-void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, cudaStream_t s);
+void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);
 // calibrate.cu
 caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost_fit fit[2]);

@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf,
 }
 
 __global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_t* load, const int32_t* meta, int D, int S,
-                        int pruned, long long bytes_per_expert, const int32_t* fetch_info) {
+                        int pruned, long long bytes_per_expert, int n_fetch) {
   if (threadIdx.x == 0) {
     st->F_base = pruned ? scalars[0] : 0;
     st->F_cost_dense = pruned ? scalars[1] : 0;
@@ -48,7 +48,7 @@ __global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_
     st->n_run = meta[0];
     int n_sh = meta[1] > 0 ? S : 0;
     st->weight_bytes = (long long)(meta[0] + n_sh) * bytes_per_expert;
-    st->n_fetch = fetch_info ? fetch_info[0] : 0;
+    st->n_fetch = n_fetch;
     st->h2d_bytes = (long long)st->n_fetch * bytes_per_expert;
   }
   for (int d = threadIdx.x; d < 64; d += blockDim.x) st->load[d] = (pruned && d < D) ? load[d] : 0;
@@ -66,9 +66,9 @@ void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* ga
     k_combine<__nv_bfloat16><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (__nv_bfloat16*)y, d.H, d.k, d.S, d.routed_scale);
 }
 
-void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, cudaStream_t st) {
+void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t st) {
   if (!stats) return;
   long long bpe = 3LL * c->d.H * c->d.I * (c->d.w_dtype == CAEE_F32 ? 4 : c->d.w_dtype == CAEE_BF16 ? 2 : 1);
   if (c->d.w_dtype == CAEE_E4M3) bpe += 3LL * ((c->d.H + 127) / 128) * ((c->d.I + 127) / 128) * 4;
-  k_stats<<<1, 64, 0, st>>>(stats, c->scalars, c->load, c->wl.meta, c->d.D, c->d.S, pruned, bpe, nullptr);
+  k_stats<<<1, 64, 0, st>>>(stats, c->scalars, c->load, c->wl.meta, c->d.D, c->d.S, pruned, bpe, n_fetch);
 }

@@ -25,15 +25,17 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 }
 
 // One warp: scans over experts -> compact ids/offsets, per-expert entry starts, runs.
-__global__ void k_wl_scan(caee_worklist wl, int T, int E, int S, int k) {
+// Run order: resident routed experts (ascending id), then the shared experts, then the
+// non-resident routed experts (ascending id) — so that an offloading step can launch the
+// resident part while the misses are still being fetched (meta[4] = runs in the first two groups).
+__global__ void k_wl_scan(caee_worklist wl, const uint8_t* __restrict__ resident, int T, int E, int S, int k) {
   const int lane = threadIdx.x;
-  int n_nz = 0, n_ent = 0, n_runs = 0, n_rows = 0;
+  int n_nz = 0, n_ent = 0;
   for (int e0 = 0; e0 < E; e0 += 32) {
     int e = e0 + lane;
     int c = e < E ? wl.counts[e] : 0;
-    int nz = c > 0, nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
+    int nz = c > 0;
     int s_nz = warp_incl_scan(nz, lane), s_c = warp_incl_scan(c, lane);
-    int s_ch = warp_incl_scan(nch, lane), s_rows = warp_incl_scan(rows, lane);
     if (e < E) {
       int start = n_ent + s_c - c;
       wl.estart[e] = start;
@@ -41,6 +43,20 @@ __global__ void k_wl_scan(caee_worklist wl, int T, int E, int S, int k) {
         int pos = n_nz + s_nz - 1;
         wl.expert_ids[pos] = e;
         wl.offs[pos] = start;
+      }
+    }
+    n_nz += __shfl_sync(0xffffffffu, s_nz, 31);
+    n_ent += __shfl_sync(0xffffffffu, s_c, 31);
+  }
+  int n_runs = 0, n_rows = 0;
+  for (int pass = 0; pass < 2; ++pass) {
+    for (int e0 = 0; e0 < E; e0 += 32) {
+      int e = e0 + lane;
+      int c = (e < E && (resident[e] != 0) == (pass == 0)) ? wl.counts[e] : 0;
+      int nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
+      int s_ch = warp_incl_scan(nch, lane), s_rows = warp_incl_scan(rows, lane);
+      if (c > 0) {
+        int start = wl.estart[e];
         int r0 = n_runs + s_ch - nch, h0 = n_rows + s_rows - rows;
         for (int j = 0; j < nch; ++j) {
           wl.run_expert[r0 + j] = e;
@@ -49,31 +65,34 @@ __global__ void k_wl_scan(caee_worklist wl, int T, int E, int S, int k) {
           wl.run_hrow[r0 + j] = h0 + j * CAEE_RUN_TOKENS;
         }
       }
+      n_runs += __shfl_sync(0xffffffffu, s_ch, 31);
+      n_rows += __shfl_sync(0xffffffffu, s_rows, 31);
     }
-    n_nz += __shfl_sync(0xffffffffu, s_nz, 31);
-    n_ent += __shfl_sync(0xffffffffu, s_c, 31);
-    n_runs += __shfl_sync(0xffffffffu, s_ch, 31);
-    n_rows += __shfl_sync(0xffffffffu, s_rows, 31);
+    if (pass == 0) {
+      if (lane == 0 && T > 0) {
+        const int TK = T * k;
+        for (int s = 0; s < S; ++s)
+          for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) {
+            int n = min(CAEE_RUN_TOKENS, T - t0);
+            wl.run_expert[n_runs] = E + s;
+            wl.run_start[n_runs] = TK + s * T + t0;
+            wl.run_n[n_runs] = n;
+            wl.run_hrow[n_runs] = n_rows;
+            n_rows += (n + 15) & ~15;
+            ++n_runs;
+          }
+      }
+      n_runs = __shfl_sync(0xffffffffu, n_runs, 0);
+      n_rows = __shfl_sync(0xffffffffu, n_rows, 0);
+      if (lane == 0) wl.meta[4] = n_runs;
+    }
   }
   if (lane == 0) {
     wl.offs[n_nz] = n_ent;
     wl.meta[0] = n_nz;
     wl.meta[2] = n_ent;
-    const int TK = T * k;
-    int r = n_runs, h = n_rows;
-    if (T > 0)
-      for (int s = 0; s < S; ++s)
-        for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) {
-          int n = min(CAEE_RUN_TOKENS, T - t0);
-          wl.run_expert[r] = E + s;
-          wl.run_start[r] = TK + s * T + t0;
-          wl.run_n[r] = n;
-          wl.run_hrow[r] = h;
-          h += (n + 15) & ~15;
-          ++r;
-        }
-    wl.meta[1] = r;
-    wl.meta[3] = h;
+    wl.meta[1] = n_runs;
+    wl.meta[3] = n_rows;
   }
 }
 
@@ -131,10 +150,10 @@ __global__ void k_wl_export(caee_worklist wl, caee_prune_out out, int E, int64_t
 void caee_launch_worklist(caee_ctx* c, int T, const int32_t* idx, const float* gate, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   cudaMemsetAsync(c->wl.counts, 0, sizeof(int32_t) * d.E, st);
-  cudaMemsetAsync(c->wl.sched, 0, sizeof(int32_t) * (2 + c->wl.max_runs), st);
+  cudaMemsetAsync(c->wl.sched, 0, sizeof(int32_t) * (c->wl.n_tickets + c->wl.max_runs), st);
   int n = T * d.k;
   if (n > 0) k_wl_count<<<caee_ceil_div(n, 256), 256, 0, st>>>(idx, n, c->wl.counts);
-  k_wl_scan<<<1, 32, 0, st>>>(c->wl, T, d.E, d.S, d.k);
+  k_wl_scan<<<1, 32, 0, st>>>(c->wl, c->resident, T, d.E, d.S, d.k);
   k_wl_fill<<<d.E + d.S, 32, 0, st>>>(c->wl, idx, gate, T, d.E, d.S, d.k);
 }
 

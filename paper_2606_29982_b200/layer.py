@@ -18,6 +18,7 @@ class Layer:
         self.part = wl.partitions(cfg)
         B.caee_set_partitions(self.ctx, self.part, cfg.D)
         self.resident = wl.residency(cfg, seed)
+        B.caee_set_residency(self.ctx, self.resident)          # before the weights: it decides where images live
         self.ticks_res, self.ticks_miss = wl.cost_tables(cfg)
         B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
         n = cfg.E + cfg.S

@@ -249,3 +249,89 @@ def test_forward_c3_full_size_sampled(H, T, mode):
         print(f"C3 T={T} {mode}: max|err|/RMS = {r:.3e}")
     finally:
         L.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# FP8 E4M3 weights with 128x128 block scales (BASELINE.json config 4) and the offload path (config 5)
+C4S = wl.scaled(wl.C4, name="C4-small", H=1024, I=384, E=64, k=4, n_group=8, topk_group=4, D=8,
+                straggler_part=3, cost_ticks_ns=600)
+C5S = wl.scaled(wl.C5, name="C5-small", H=1024, I=384, E=64, k=4, n_group=8, topk_group=4, D=8,
+                straggler_part=3, cost_ticks_ns=901, n_resident=16, miss_ticks_ns=40_000)
+
+
+@pytest.mark.parametrize("kernel", ["simt", "umma"])
+def test_forward_small_fp8(H, kernel):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, C4S, max_tokens=300, kernel=B.CAEE_KERNEL_SIMT if kernel == "simt" else B.CAEE_KERNEL_UMMA)
+    try:
+        for T, mode in ((1, "dense"), (8, "frac"), (32, "cir"), (128, "frac"), (300, "dense"), (19, "rank")):
+            r = _forward_case(H, L, T, mode)
+            print(f"fp8 {kernel} T={T} {mode}: max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
+
+
+def test_forward_fp8_uneven_block_scales(H):
+    """Block scales spread over three decades inside one tile row: the ratio/ref folding of the
+    UMMA path must still match the oracle's exact dequantisation."""
+    from paper_2606_29982_b200 import binding as B
+    cfg = C4S
+    L = _layer(H, cfg, max_tokens=32, kernel=B.CAEE_KERNEL_UMMA)
+    try:
+        g = torch.Generator(device=L.device)
+        g.manual_seed(5)
+        for r in L.raw:
+            for name in ("gate_scale", "up_scale", "down_scale"):
+                f = torch.exp(torch.empty_like(r[name]).uniform_(-3.5, 3.5, generator=g))
+                r[name].mul_(f)
+        B.caee_set_weights(L.ctx, [r["gate"] for r in L.raw], [r["up"] for r in L.raw], [r["down"] for r in L.raw],
+                           [r["gate_scale"] for r in L.raw], [r["up_scale"] for r in L.raw],
+                           [r["down_scale"] for r in L.raw], pack=1)
+        L._host.clear()
+        r = _forward_case(H, L, 24, "dense")
+        print(f"fp8 uneven scales: max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
+
+
+@pytest.mark.parametrize("mode", ["dense", "cir", "thresh"])
+def test_forward_offload_small(H, mode):
+    """Config-5-style residency: 16 of 64 experts in HBM, the rest fetched from pinned host memory
+    only when they survive pruning; output and decisions must match the all-resident oracle."""
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, C5S, max_tokens=64, kernel=B.CAEE_KERNEL_UMMA)
+    try:
+        assert int(L.resident.sum()) == 16
+        for T in (1, 8, 32, 64):
+            m, theta = MODES.get(mode, (0, 0.0))
+            th = _thresh_theta(L.cfg, T) if theta is None else theta
+            x = wl.hidden(L.cfg, T, 77, L.device)
+            s = L.oracle_scores(x)
+            d = L.oracle_decisions(s, None if mode == "dense" else m, th)
+            params = None if mode == "dense" else B.prune_params(m, th)
+            y, st = L.forward(x, params, torch.from_numpy(s).to(L.device), want_stats=True)
+            idx_g, _ = L.last_routing(T)
+            assert np.array_equal(idx_g, d["idx"])
+            run = set(int(e) for e in d["compact"]["expert_ids"])
+            want_fetch = sum(1 for e in run if not L.resident[e])
+            assert st.n_fetch == want_fetch and st.h2d_bytes == want_fetch * L.cfg.expert_bytes
+            if mode != "dense":
+                assert st.F_cost == d["prune"]["F_cost"] and st.n_keep == d["prune"]["n_keep"]
+            H.check_y(y, L.oracle_y(x, d["idx"], d["gate"], range(T)), range(T), H.TOL[L.cfg.w_dtype])
+            # a second step reuses the staging slots
+            y2 = L.forward(x, params, torch.from_numpy(s).to(L.device))
+            assert torch.equal(y, y2)
+    finally:
+        L.close()
+
+
+@pytest.mark.parametrize("T,mode", [(128, "frac"), (8, "dense"), (1, "frac")])
+def test_forward_c4_full_size_sampled(H, T, mode):
+    """Config 4 (DeepSeek-R1-shaped, FP8 E4M3 weights + 128x128 block scales, 11.3 GB)."""
+    L = H.GpuLayer(wl.C4, seed=0, max_tokens=128, keep_raw=False)
+    try:
+        toks = sorted(set([0, T // 3, T - 1]))
+        r = _forward_case(H, L, T, mode, tokens=toks, seed=100)
+        print(f"C4 T={T} {mode}: max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
