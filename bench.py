@@ -309,7 +309,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="caee", choices=["caee", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--tokens", type=int, default=128)
     ap.add_argument("--prune", default="thresh:0.6", help="dense | none | thresh:θ | cir:θ_imp | rank:b | frac:p")
     ap.add_argument("--no-cpu-baseline", action="store_true")
