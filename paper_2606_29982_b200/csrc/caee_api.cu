@@ -115,7 +115,7 @@ caee_status after_launch(caee_ctx* c, const char* what) {
 }
 
 void free_all(caee_ctx* c) {
-  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->scores, c->idx,
+  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->logits, c->tile_ctr, c->scores, c->idx,
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
@@ -141,14 +141,18 @@ void free_all(caee_ctx* c) {
 caee_status create_impl(caee_ctx* c) {
   const caee_layer_desc& d = c->d;
   const size_t Tm = d.max_tokens, E = d.E, k = d.k, S = d.S;
-  c->ksplit_max = d.H / 256 > 0 ? d.H / 256 : 1;
-  size_t prow = 1;
-  for (int T = 1; T <= d.max_tokens; ++T) prow = std::max(prow, (size_t)caee_router_ksplit(c, T) * T);
+  size_t prow = 1, ntile = 1;
+  for (int T = 1; T <= d.max_tokens; ++T) {
+    int tt, ks;
+    caee_router_shape(c, T, &tt, &ks);
+    prow = std::max(prow, (size_t)ks * T);
+    ntile = std::max(ntile, (size_t)caee_ceil_div(d.E, 64) * caee_ceil_div(T, tt));
+  }
   caee_status rc;
 #define A(ptr, n) if ((rc = dev_alloc(c, &(ptr), (n))) != CAEE_OK) return rc
   A(c->part, E); A(c->resident, E); A(c->w_eff, E);
   A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
-  A(c->partial, prow * E); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
+  A(c->partial, prow * E); A(c->logits, Tm * E); A(c->tile_ctr, ntile); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
   A(c->act, E); A(c->must, E); A(c->keep, E); A(c->I_fix, E); A(c->load, CAEE_MAX_D); A(c->scalars, 8);
   c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS + S * ((Tm + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS));
   A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
@@ -164,6 +168,7 @@ caee_status create_impl(caee_ctx* c) {
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
+  CAEE_CUDA(c, cudaMemset(c->tile_ctr, 0, sizeof(int32_t) * ntile));
   CAEE_CUDA(c, cudaMemset(c->scalars, 0, sizeof(int64_t) * 8));
   CAEE_CUDA(c, cudaMemset(c->load, 0, sizeof(int64_t) * CAEE_MAX_D));
   // defaults: contiguous partitions, everything resident, unit costs
@@ -185,12 +190,11 @@ caee_status enqueue_decisions(caee_ctx* c, const void* x, const float* scores_in
   const float* scores = scores_in;
   if (T > 0 && do_route) {
     if (!scores_in) {
-      int ks = caee_router_ksplit(c, T);
-      caee_launch_router_logits(c, x, T, ks, st);
-      caee_launch_route_topk(c, nullptr, ks, T, scores_out ? scores_out : c->scores, idx, gate, st);
+      caee_launch_router_logits(c, x, T, st);
+      caee_launch_route_topk(c, nullptr, T, scores_out ? scores_out : c->scores, idx, gate, st);
       scores = scores_out ? scores_out : c->scores;
     } else {
-      caee_launch_route_topk(c, scores_in, 0, T, nullptr, idx, gate, st);
+      caee_launch_route_topk(c, scores_in, T, nullptr, idx, gate, st);
     }
   }
   const int mode = p ? p->mode : CAEE_PRUNE_NONE;
@@ -423,9 +427,8 @@ caee_status caee_route(caee_ctx* c, const void* x, int32_t T, float* scores, int
   if (!x || !idx || !gate) return caee_fail(c, CAEE_EINVAL, "x, idx or gate is NULL");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  int ks = caee_router_ksplit(c, T);
-  caee_launch_router_logits(c, x, T, ks, st);
-  caee_launch_route_topk(c, nullptr, ks, T, scores, idx, gate, st);
+  caee_launch_router_logits(c, x, T, st);
+  caee_launch_route_topk(c, nullptr, T, scores, idx, gate, st);
   return after_launch(c, "caee_route");
 }
 
@@ -435,7 +438,7 @@ caee_status caee_route_from_scores(caee_ctx* c, const float* scores, int32_t T, 
   if (T == 0) return CAEE_OK;
   if (!scores || !idx || !gate) return caee_fail(c, CAEE_EINVAL, "scores, idx or gate is NULL");
   DeviceGuard g(c->device);
-  caee_launch_route_topk(c, scores, 0, T, nullptr, idx, gate, (cudaStream_t)stream);
+  caee_launch_route_topk(c, scores, T, nullptr, idx, gate, (cudaStream_t)stream);
   return after_launch(c, "caee_route_from_scores");
 }
 
@@ -477,8 +480,16 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);
-  if (rc != CAEE_OK) return rc;
+  const bool fused = caee_decide_fits(c, T);
+  if (fused) {
+    // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
+    if (!scores) caee_launch_router_logits(c, x, T, st);
+    caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st);
+    if ((rc = after_launch(c, "decision kernel")) != CAEE_OK) return rc;
+  } else {
+    rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);
+    if (rc != CAEE_OK) return rc;
+  }
   const bool prof = (size_t)c->prof_used * 2 + 1 < c->prof_ev.size();
   int n_fetch = 0;
   if (c->kernel == CAEE_KERNEL_SIMT) {
@@ -522,7 +533,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   }
   if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);
   caee_launch_combine(c, T, c->idx, c->gate, y, st);
-  caee_launch_stats(c, stats, p != nullptr, n_fetch, st);
+  if (!fused || c->any_offload) caee_launch_stats(c, stats, p != nullptr, n_fetch, st);
   return after_launch(c, "caee_moe_forward");
 }
 

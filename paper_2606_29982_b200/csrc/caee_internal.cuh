@@ -16,6 +16,7 @@
 #define CAEE_MAX_E 512
 #define CAEE_MAX_D 64
 #define CAEE_RUN_TOKENS 128 /* tokens per run: one UMMA N tile */
+#define CAEE_DECIDE_MAX_ENTRIES 2048 /* T*k up to which one CTA takes the whole decision step (decide.cu) */
 
 // One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
 struct caee_worklist {
@@ -82,8 +83,9 @@ struct caee_ctx {
   caee_packed packed;
 
   // scratch
-  int ksplit_max = 1;
-  float* partial = nullptr;  // [ksplit_max, Tmax, E]
+  float* partial = nullptr;  // [ksplit, T, E] split-K partial logits (sized for the worst T)
+  float* logits = nullptr;   // [Tmax, E] x W_r^T
+  int32_t* tile_ctr = nullptr;  // per output tile of the router GEMM: CTAs finished (self-resetting)
   float* scores = nullptr;   // [Tmax, E]
   int32_t* idx = nullptr;    // [Tmax, k]
   float* gate = nullptr;     // [Tmax, k]
@@ -127,10 +129,14 @@ caee_status caee_check_cuda(caee_ctx* c, cudaError_t e, const char* what);
 static inline int caee_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 // router.cu
-int caee_router_ksplit(const caee_ctx* c, int T);
-void caee_launch_router_logits(caee_ctx* c, const void* x, int T, int ksplit, cudaStream_t s);
-void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int ksplit, int T, float* scores_out,
-                            int32_t* idx, float* gate, cudaStream_t s);
+void caee_router_shape(const caee_ctx* c, int T, int* token_tile, int* ksplit);
+void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t s);
+void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate,
+                            cudaStream_t s);
+// decide.cu
+bool caee_decide_fits(const caee_ctx* c, int T);
+void caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* p, caee_fwd_stats* stats,
+                        cudaStream_t s);
 // prune.cu
 void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx,
                        const float* gate, cudaStream_t s);
@@ -151,5 +157,6 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);
+long long caee_expert_bytes(const caee_ctx* c);
 // calibrate.cu
 caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost_fit fit[2]);

@@ -3,6 +3,7 @@
 // The expert kernels leave each (token, slot) output row in o[(t*(k+S) + slot), :] (fp32), so
 // the sum runs in list order and y is deterministic.  Also fills caee_fwd_stats.
 #include "caee_internal.cuh"
+#include "worklist_dev.cuh"
 
 namespace {
 
@@ -38,20 +39,7 @@ __global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf,
 
 __global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_t* load, const int32_t* meta, int D, int S,
                         int pruned, long long bytes_per_expert, int n_fetch) {
-  if (threadIdx.x == 0) {
-    st->F_base = pruned ? scalars[0] : 0;
-    st->F_cost_dense = pruned ? scalars[1] : 0;
-    st->F_cost = pruned ? scalars[2] : 0;
-    st->F_imp = pruned ? scalars[3] : 0;
-    st->n_act = pruned ? (int32_t)scalars[4] : meta[0];
-    st->n_keep = pruned ? (int32_t)scalars[6] : meta[0];
-    st->n_run = meta[0];
-    int n_sh = meta[1] > 0 ? S : 0;
-    st->weight_bytes = (long long)(meta[0] + n_sh) * bytes_per_expert;
-    st->n_fetch = n_fetch;
-    st->h2d_bytes = (long long)st->n_fetch * bytes_per_expert;
-  }
-  for (int d = threadIdx.x; d < 64; d += blockDim.x) st->load[d] = (pruned && d < D) ? load[d] : 0;
+  caee_stats_fill(st, scalars, load, meta, D, S, pruned, bytes_per_expert, n_fetch, threadIdx.x, blockDim.x);
 }
 
 }  // namespace
@@ -66,9 +54,14 @@ void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* ga
     k_combine<__nv_bfloat16><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (__nv_bfloat16*)y, d.H, d.k, d.S, d.routed_scale);
 }
 
-void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t st) {
-  if (!stats) return;
+long long caee_expert_bytes(const caee_ctx* c) {
   long long bpe = 3LL * c->d.H * c->d.I * (c->d.w_dtype == CAEE_F32 ? 4 : c->d.w_dtype == CAEE_BF16 ? 2 : 1);
   if (c->d.w_dtype == CAEE_E4M3) bpe += 3LL * ((c->d.H + 127) / 128) * ((c->d.I + 127) / 128) * 4;
+  return bpe;
+}
+
+void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t st) {
+  if (!stats) return;
+  const long long bpe = caee_expert_bytes(c);
   k_stats<<<1, 64, 0, st>>>(stats, c->scalars, c->load, c->wl.meta, c->d.D, c->d.S, pruned, bpe, n_fetch);
 }

@@ -29,13 +29,15 @@ template <int NV>
 __device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint32_t ok, int E, int n_group,
                                                     int topk_group, int lane) {
   const int gs = E / n_group;
+  int grp[NV];  // group of this lane's expert in slot i (-1: not allowed)
+#pragma unroll
+  for (int i = 0; i < NV; ++i) grp[i] = ((ok >> i) & 1u) ? (lane + 32 * i) / gs : -1;
   float my_gscore = -INFINITY;  // lane g holds the score of group g
   for (int g = 0; g < n_group; ++g) {
     float m1 = -INFINITY, m2 = -INFINITY;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      int e = lane + 32 * i;
-      if (((ok >> i) & 1u) && e / gs == g) {
+      if (grp[i] == g) {
         float v = sp[i];
         if (v > m1) { m2 = m1; m1 = v; }
         else if (v > m2) m2 = v;
@@ -61,10 +63,8 @@ __device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint3
   }
   uint32_t m = 0;
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    int e = lane + 32 * i;
-    if (e < E && ((gsel >> (e / gs)) & 1u)) m |= 1u << i;
-  }
+  for (int i = 0; i < NV; ++i)
+    if (grp[i] >= 0 && ((gsel >> grp[i]) & 1u)) m |= 1u << i;
   return m;
 }
 
@@ -106,4 +106,88 @@ __device__ __forceinline__ void caee_warp_select(const float (&s)[NV], const flo
     idx_out[lane] = sel_e;
     gate_out[lane] = sel_e < 0 ? 0.f : (norm_topk ? __fdiv_rn(sel_s, sum) : sel_s);
   }
+}
+
+// One token's post-activation scores s (S0 tail): either loaded (scores_row) or computed from
+// the token's logits row + b_logit: sigmoid, or softmax over the E experts (R1).
+template <int NV>
+__device__ __forceinline__ void caee_token_scores(const float* __restrict__ scores_row, const float* __restrict__ logits_row,
+                                                  const float* __restrict__ b_logit, int E, int score_fn, int lane,
+                                                  float (&s)[NV]) {
+  if (scores_row) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int e = lane + 32 * i;
+      s[i] = e < E ? scores_row[e] : 0.f;
+    }
+    return;
+  }
+  float l[NV];
+  float mx = -INFINITY;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int e = lane + 32 * i;
+    l[i] = e < E ? logits_row[e] : 0.f;
+  }
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int e = lane + 32 * i;
+    if (e < E) {
+      if (b_logit) l[i] += b_logit[e];
+      mx = fmaxf(mx, l[i]);
+    }
+  }
+  if (score_fn == 1 /* CAEE_SCORE_SIGMOID */) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) s[i] = 1.0f / (1.0f + expf(-l[i]));
+  } else {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    float den = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int e = lane + 32 * i;
+      s[i] = e < E ? expf(l[i] - mx) : 0.f;
+      den += s[i];
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) den += __shfl_xor_sync(0xffffffffu, den, o);
+#pragma unroll
+    for (int i = 0; i < NV; ++i) s[i] = s[i] / den;
+  }
+}
+
+// S1 for one token: selection score s' = s + corr_bias, group limit, top-k, gates.
+template <int NV>
+__device__ __forceinline__ void caee_route_token(const float (&s)[NV], const float* __restrict__ corr_bias, int E, int k,
+                                                 int n_group, int topk_group, int norm_topk, int lane, int32_t* idx_out,
+                                                 float* gate_out) {
+  float sp[NV];
+  uint32_t ok = 0;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int e = lane + 32 * i;
+    sp[i] = (corr_bias && e < E) ? __fadd_rn(s[i], corr_bias[e]) : s[i];
+    if (e < E) ok |= 1u << i;
+  }
+  if (n_group > 1 && topk_group < n_group) ok &= caee_group_mask<NV>(sp, ok, E, n_group, topk_group, lane);
+  caee_warp_select<NV>(s, sp, ok, k, norm_topk, lane, idx_out, gate_out);
+}
+
+// S5 for one token: top-k of s' over the experts of A_trans only, no group limit (R13).
+template <int NV>
+__device__ __forceinline__ void caee_compensate_token(const float* __restrict__ scores_row, const float* __restrict__ corr_bias,
+                                                      const uint8_t* keep, int E, int k, int norm_topk, int lane,
+                                                      int32_t* idx_out, float* gate_out) {
+  float s[NV], sp[NV];
+  uint32_t ok = 0;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int e = lane + 32 * i;
+    s[i] = e < E ? scores_row[e] : 0.f;
+    sp[i] = (corr_bias && e < E) ? __fadd_rn(s[i], corr_bias[e]) : s[i];
+    if (e < E && keep[e]) ok |= 1u << i;
+  }
+  __syncwarp();
+  caee_warp_select<NV>(s, sp, ok, k, norm_topk, lane, idx_out, gate_out);
 }

@@ -4,6 +4,7 @@
 // appended as runs over all tokens).  Integer work only; the result is unique: experts
 // ascending, tokens ascending inside an expert.
 #include "caee_internal.cuh"
+#include "worklist_dev.cuh"
 
 namespace {
 
@@ -15,116 +16,13 @@ __global__ void k_wl_count(const int32_t* __restrict__ idx, int n, int32_t* __re
   }
 }
 
-__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    int n = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= o) v += n;
-  }
-  return v;
-}
-
-// One warp: scans over experts -> compact ids/offsets, per-expert entry starts, runs.
-// Run order: resident routed experts (ascending id), then the shared experts, then the
-// non-resident routed experts (ascending id) — so that an offloading step can launch the
-// resident part while the misses are still being fetched (meta[4] = runs in the first two groups).
 __global__ void k_wl_scan(caee_worklist wl, const uint8_t* __restrict__ resident, int T, int E, int S, int k) {
-  const int lane = threadIdx.x;
-  int n_nz = 0, n_ent = 0;
-  for (int e0 = 0; e0 < E; e0 += 32) {
-    int e = e0 + lane;
-    int c = e < E ? wl.counts[e] : 0;
-    int nz = c > 0;
-    int s_nz = warp_incl_scan(nz, lane), s_c = warp_incl_scan(c, lane);
-    if (e < E) {
-      int start = n_ent + s_c - c;
-      wl.estart[e] = start;
-      if (nz) {
-        int pos = n_nz + s_nz - 1;
-        wl.expert_ids[pos] = e;
-        wl.offs[pos] = start;
-      }
-    }
-    n_nz += __shfl_sync(0xffffffffu, s_nz, 31);
-    n_ent += __shfl_sync(0xffffffffu, s_c, 31);
-  }
-  int n_runs = 0, n_rows = 0;
-  for (int pass = 0; pass < 2; ++pass) {
-    for (int e0 = 0; e0 < E; e0 += 32) {
-      int e = e0 + lane;
-      int c = (e < E && (resident[e] != 0) == (pass == 0)) ? wl.counts[e] : 0;
-      int nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
-      int s_ch = warp_incl_scan(nch, lane), s_rows = warp_incl_scan(rows, lane);
-      if (c > 0) {
-        int start = wl.estart[e];
-        int r0 = n_runs + s_ch - nch, h0 = n_rows + s_rows - rows;
-        for (int j = 0; j < nch; ++j) {
-          wl.run_expert[r0 + j] = e;
-          wl.run_start[r0 + j] = start + j * CAEE_RUN_TOKENS;
-          wl.run_n[r0 + j] = min(CAEE_RUN_TOKENS, c - j * CAEE_RUN_TOKENS);
-          wl.run_hrow[r0 + j] = h0 + j * CAEE_RUN_TOKENS;
-        }
-      }
-      n_runs += __shfl_sync(0xffffffffu, s_ch, 31);
-      n_rows += __shfl_sync(0xffffffffu, s_rows, 31);
-    }
-    if (pass == 0) {
-      if (lane == 0 && T > 0) {
-        const int TK = T * k;
-        for (int s = 0; s < S; ++s)
-          for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) {
-            int n = min(CAEE_RUN_TOKENS, T - t0);
-            wl.run_expert[n_runs] = E + s;
-            wl.run_start[n_runs] = TK + s * T + t0;
-            wl.run_n[n_runs] = n;
-            wl.run_hrow[n_runs] = n_rows;
-            n_rows += (n + 15) & ~15;
-            ++n_runs;
-          }
-      }
-      n_runs = __shfl_sync(0xffffffffu, n_runs, 0);
-      n_rows = __shfl_sync(0xffffffffu, n_rows, 0);
-      if (lane == 0) wl.meta[4] = n_runs;
-    }
-  }
-  if (lane == 0) {
-    wl.offs[n_nz] = n_ent;
-    wl.meta[0] = n_nz;
-    wl.meta[2] = n_ent;
-    wl.meta[1] = n_runs;
-    wl.meta[3] = n_rows;
-  }
+  caee_wl_scan_warp(wl, wl.counts, wl.estart, resident, T, E, S, k, threadIdx.x);
 }
 
-// Block e < E: one warp lists expert e's (token, slot) pairs in ascending entry order.
-// Blocks E..E+S-1: shared expert entries (every token).
 __global__ void k_wl_fill(caee_worklist wl, const int32_t* __restrict__ idx, const float* __restrict__ gate, int T, int E,
                           int S, int k) {
-  const int lane = threadIdx.x, e = blockIdx.x, KS = k + S, TK = T * k;
-  if (e >= E) {
-    int s = e - E;
-    for (int t = lane; t < T; t += 32) {
-      wl.ent_tok[TK + s * T + t] = t;
-      wl.ent_dst[TK + s * T + t] = t * KS + k + s;
-    }
-    return;
-  }
-  if (wl.counts[e] == 0) return;
-  int pos = wl.estart[e];
-  for (int i0 = 0; i0 < TK; i0 += 32) {
-    int i = i0 + lane;
-    bool hit = i < TK && idx[i] == e;
-    unsigned b = __ballot_sync(0xffffffffu, hit);
-    if (hit) {
-      int p = pos + __popc(b & ((1u << lane) - 1));
-      int t = i / k, j = i - t * k;
-      wl.ent_tok[p] = t;
-      wl.ent_slot[p] = j;
-      wl.ent_wt[p] = gate[i];
-      wl.ent_dst[p] = t * KS + j;
-    }
-    pos += __popc(b);
-  }
+  caee_wl_fill_expert(wl, wl.counts, wl.estart, idx, gate, T, E, S, k, blockIdx.x, threadIdx.x);
 }
 
 __global__ void k_wl_export(caee_worklist wl, caee_prune_out out, int E, int64_t* scalars) {

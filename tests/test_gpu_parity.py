@@ -101,6 +101,38 @@ def test_prune_compensate_compact_bit_exact(H, cfg, mode):
         L.close()
 
 
+@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, wl.scaled(wl.C3, name="R1-router", H=256, I=128)], ids=lambda c: c.name)
+@pytest.mark.parametrize("mode", ["dense"] + list(MODES))
+def test_forward_decisions_bit_exact_fused_and_standalone(H, cfg, mode):
+    """caee_moe_forward takes the one-kernel decision path (decide.cu) up to T*k = 2048 entries and
+    the stand-alone kernels above; both must give the oracle's K_final, gates, F_* and loads."""
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, cfg, max_tokens=2048 // cfg.k + 44)
+    try:
+        for T in (1, 7, 32, 129, 2048 // cfg.k, 2048 // cfg.k + 1, 2048 // cfg.k + 44):
+            m, theta = MODES.get(mode, (0, 0.0))
+            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS) if mode == "thresh" else (0,)):
+                th = _thresh_theta(cfg, T) if theta is None else theta
+                x = wl.hidden(cfg, T, 13, L.device)
+                s = L.oracle_scores(x)
+                d = L.oracle_decisions(s, None if mode == "dense" else m, th, flags)
+                params = None if mode == "dense" else B.prune_params(m, th, flags)
+                _, st = L.forward(x, params, torch.from_numpy(s).to(L.device), want_stats=True)
+                idx_g, gate_g = L.last_routing(T)
+                assert np.array_equal(idx_g, d["idx"]), (T, mode, flags)
+                assert np.array_equal(gate_g.view(np.uint32), d["gate"].view(np.uint32)), (T, mode, flags)
+                assert st.n_run == d["compact"]["n_run"]
+                assert st.weight_bytes == (st.n_run + cfg.S) * cfg.expert_bytes
+                if mode != "dense":
+                    pr = d["prune"]
+                    assert (st.F_base, st.F_cost_dense, st.F_cost, st.F_imp) == (pr["F_base"], pr["F_cost_dense"], pr["F_cost"],
+                                                                                pr["F_imp_fix"]), (T, mode, flags)
+                    assert (st.n_act, st.n_keep) == (pr["n_act"], pr["n_keep"])
+                    assert list(st.load[:cfg.D]) == list(pr["load"])
+    finally:
+        L.close()
+
+
 def _forward_case(H, L, T, mode, tokens=None, seed=21):
     from paper_2606_29982_b200 import binding as B
     cfg = L.cfg
