@@ -37,7 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(HERE, "build", os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
         cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler",
-               "-fPIC", "-Xcompiler", "-Wall", "-c", src, "-o", obj]
+               "-fPIC", "-Xcompiler", "-Wall", "-c", src, "-o", obj] + os.environ.get("CAEE_NVCC_EXTRA", "").split()
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))

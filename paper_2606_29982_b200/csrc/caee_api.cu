@@ -115,7 +115,7 @@ caee_status after_launch(caee_ctx* c, const char* what) {
 }
 
 void free_all(caee_ctx* c) {
-  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->logits, c->tile_ctr, c->scores, c->idx,
+  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->logits, c->tile_ctr, c->decide_scratch, c->scores, c->idx,
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
@@ -152,7 +152,7 @@ caee_status create_impl(caee_ctx* c) {
 #define A(ptr, n) if ((rc = dev_alloc(c, &(ptr), (n))) != CAEE_OK) return rc
   A(c->part, E); A(c->resident, E); A(c->w_eff, E);
   A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
-  A(c->partial, prow * E); A(c->logits, Tm * E); A(c->tile_ctr, ntile); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
+  A(c->partial, prow * E); A(c->logits, Tm * E); A(c->tile_ctr, ntile); A(c->decide_scratch, caee_decide_scratch_bytes(c)); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
   A(c->act, E); A(c->must, E); A(c->keep, E); A(c->I_fix, E); A(c->load, CAEE_MAX_D); A(c->scalars, 8);
   c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS + S * ((Tm + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS));
   A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
@@ -169,6 +169,7 @@ caee_status create_impl(caee_ctx* c) {
 #undef A
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
   CAEE_CUDA(c, cudaMemset(c->tile_ctr, 0, sizeof(int32_t) * ntile));
+  CAEE_CUDA(c, cudaMemset(c->decide_scratch, 0, caee_decide_scratch_bytes(c)));
   CAEE_CUDA(c, cudaMemset(c->scalars, 0, sizeof(int64_t) * 8));
   CAEE_CUDA(c, cudaMemset(c->load, 0, sizeof(int64_t) * CAEE_MAX_D));
   // defaults: contiguous partitions, everything resident, unit costs
@@ -484,7 +485,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
     if (!scores) caee_launch_router_logits(c, x, T, st);
-    caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st);
+    CAEE_CUDA(c, caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st));
     if ((rc = after_launch(c, "decision kernel")) != CAEE_OK) return rc;
   } else {
     rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);

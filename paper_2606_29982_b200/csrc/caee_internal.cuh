@@ -16,7 +16,7 @@
 #define CAEE_MAX_E 512
 #define CAEE_MAX_D 64
 #define CAEE_RUN_TOKENS 128 /* tokens per run: one UMMA N tile */
-#define CAEE_DECIDE_MAX_ENTRIES 2048 /* T*k up to which one CTA takes the whole decision step (decide.cu) */
+#define CAEE_DECIDE_MAX_TOKENS 256 /* largest step the one-kernel decision path takes (decide.cu) */
 
 // One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
 struct caee_worklist {
@@ -85,6 +85,7 @@ struct caee_ctx {
   // scratch
   float* partial = nullptr;  // [ksplit, T, E] split-K partial logits (sized for the worst T)
   float* logits = nullptr;   // [Tmax, E] x W_r^T
+  uint8_t* decide_scratch = nullptr;  // k_decide's self-cleaning accumulators, membership matrix, barriers
   int32_t* tile_ctr = nullptr;  // per output tile of the router GEMM: CTAs finished (self-resetting)
   float* scores = nullptr;   // [Tmax, E]
   int32_t* idx = nullptr;    // [Tmax, k]
@@ -135,8 +136,9 @@ void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* s
                             cudaStream_t s);
 // decide.cu
 bool caee_decide_fits(const caee_ctx* c, int T);
-void caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* p, caee_fwd_stats* stats,
-                        cudaStream_t s);
+size_t caee_decide_scratch_bytes(const caee_ctx* c);
+cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* p, caee_fwd_stats* stats,
+                               cudaStream_t s);
 // prune.cu
 void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx,
                        const float* gate, cudaStream_t s);

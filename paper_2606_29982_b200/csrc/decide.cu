@@ -1,25 +1,46 @@
-// decide.cu — the decode-size decision step as ONE kernel: S1 top-k + gates, S2 activation set
-// and importance, S3 cost lookup / F_cost, S4 cost-aware pruning, S5 compensation, S6
-// compaction into the expert kernel's work list, and the step's caee_fwd_stats
-// (BASELINE.json north_star subsystem (1)).
+// decide.cu — the decode-size decision step as ONE cooperative kernel: S1 top-k + gates, S2
+// activation set and importance, S3 cost lookup / F_cost, S4 cost-aware pruning, S5
+// compensation, S6 compaction into the expert kernel's work list, and the step's
+// caee_fwd_stats (BASELINE.json north_star subsystem (1)).
 //
-// Why one CTA.  The pruning decision is batch-global: x_e is one bit per expert for the whole
-// batch, so every token's top-k must be known before any expert can be
-// pruned, and every expert's fate before any token can be compensated.  At decode sizes
-// (T*k <= 2048 entries, E <= 512) the whole state fits one CTA's shared memory, so the grid-wide
-// dependencies become __syncthreads and the five launches (plus two memsets) of the
-// stand-alone path collapse into this one; each stage runs exactly the device code of the
-// stand-alone kernels (warp_select.cuh, prune_dev.cuh, worklist_dev.cuh), so both paths give
-// bit-identical decisions.  Larger steps (prefill) use the stand-alone kernels.
+// Shape.  One warp per token (a token's E scores live in the warp's registers; selection is
+// warp shuffles, warp_select.cuh), 16 tokens per CTA, ceil(T/16) <= 16 CTAs, launched
+// cooperatively.  The pruning decision is batch-global — x_e is one bit per expert for the
+// whole batch — so there are two grid-wide dependencies:
+//   A  route own token; add its gates to the global importance accumulators, set A_act /
+//      per-token must bits                                         ── grid barrier 1 ──
+//   B  EVERY CTA takes the (deterministic, integer) pruning decision redundantly from the
+//      accumulators in its own shared memory (prune_dev.cuh): cheaper than a second barrier
+//   C  compensate own token if it lost an expert; publish K_final as bits of the E x T
+//      membership matrix M                                         ── grid barrier 2 ──
+//   D  every CTA scans the per-expert counts (popcounts of M) itself; each warp places its
+//      token's entries (position = popcount prefix in M); CTA 0 writes runs, meta, stats.
+// The last CTA to leave clears the accumulators, M and the barrier counters for the next
+// step.  Each stage runs the device code of the stand-alone kernels (router.cu, prune.cu,
+// worklist.cu), so both paths give bit-identical decisions; steps with more than 256 tokens
+// (prefill) use the stand-alone kernels.
+#include <cooperative_groups.h>
+
 #include "caee_internal.cuh"
 #include "prune_dev.cuh"
 #include "warp_select.cuh"
 #include "worklist_dev.cuh"
 
+#ifdef CAEE_DECIDE_TIMING
+__device__ long long g_decide_clk[16];
+#define STAMP(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) g_decide_clk[i] = clock64(); } while (0)
+extern "C" void caee_debug_decide_clocks(long long* out) { cudaMemcpyFromSymbol(out, g_decide_clk, sizeof(long long) * 16); }
+extern "C" void caee_debug_route_clocks(long long* out) { cudaMemcpyFromSymbol(out, g_route_clk, sizeof(long long) * 16); }
+extern "C" void caee_debug_prune_clocks(long long* out) { cudaMemcpyFromSymbol(out, g_prune_clk, sizeof(long long) * 16); }
+#else
+#define STAMP(i)
+#endif
+
 namespace {
 
-constexpr int kDecideThreads = 1024;
-constexpr int kMaxEnt = CAEE_DECIDE_MAX_ENTRIES;
+constexpr int kThreads = CAEE_MAX_E;          // 512: thread e owns expert e in the batch-global stages
+constexpr int kWarps = kThreads / 32;         // tokens per CTA
+constexpr int kWords = CAEE_DECIDE_MAX_TOKENS / 32;
 
 struct DecideParams {
   const float* logits;     // [T,E] x W_r^T (k_router_logits), or NULL with scores_in
@@ -41,77 +62,151 @@ struct DecideParams {
   int n_sched;             // ints of wl.sched to zero (tile tickets + per-run counters)
   caee_fwd_stats* stats;   // or NULL
   long long bytes_per_expert;
+  // self-cleaning global scratch (zero between steps)
+  unsigned long long* acc_I;  // [E]
+  unsigned char* acc_act;     // [E]
+  unsigned char* acc_must;    // [E]
+  uint32_t* M;                // [E, kWords]
+  int* bar;                   // [4]: barrier 1, barrier 2, exit ticket
 };
 
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// All CTAs of the (co-resident, cooperative) grid arrive; nobody leaves before everyone has.
+__device__ __forceinline__ void grid_barrier(int* ctr, int G) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(ctr, 1);
+    while (ld_acquire_gpu(ctr) < G) {}
+    __threadfence();
+  }
+  __syncthreads();
+}
+
 template <int NV>
-__global__ void __launch_bounds__(kDecideThreads, 1) k_decide(const DecideParams p) {
+__global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   __shared__ caee_prune_smem sm;
-  __shared__ int32_t s_idx[kMaxEnt];
-  __shared__ float s_gate[kMaxEnt];
-  __shared__ int32_t s_cnt[CAEE_MAX_E], s_est[CAEE_MAX_E];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kDecideThreads / 32;
+  __shared__ int32_t s_idx[kWarps][32];
+  __shared__ float s_gate[kWarps][32];
+  __shared__ int32_t s_est[CAEE_MAX_E];
+  __shared__ int s_scan[33 * 6];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x;
   const int T = p.T, E = p.E, k = p.k;
+  const int t = blockIdx.x * kWarps + warp;   // this warp's token
+  const bool live = t < T;
+  const bool prunes = p.has_prune && p.mode != CAEE_PRUNE_NONE;
+  int32_t* ir = s_idx[warp];
+  float* gr = s_gate[warp];
 
-  for (int i = tid; i < p.n_sched; i += kDecideThreads) p.wl.sched[i] = 0;
-  for (int e = tid; e < E; e += kDecideThreads) s_cnt[e] = 0;
+  STAMP(0);
+  float bl[NV], cb[NV];
+  caee_load_vec<NV>(p.scores_in ? nullptr : p.b_logit, E, lane, bl);
+  caee_load_vec<NV>(p.corr_bias, E, lane, cb);
+  if (blockIdx.x == 0)
+    for (int i = tid; i < p.n_sched; i += kThreads) p.wl.sched[i] = 0;
 
-  // S0 tail + S1: one warp per token
-  for (int t = warp; t < T; t += nwarps) {
+  // ---- A: S0 tail + S1 for this warp's token; S2 + per-token rules into the accumulators
+  if (live) {
     float s[NV];
     caee_token_scores<NV>(p.scores_in ? p.scores_in + (size_t)t * E : nullptr, p.logits ? p.logits + (size_t)t * E : nullptr,
-                          p.b_logit, E, p.score_fn, lane, s);
-    if (!p.scores_in) {
+                          p.b_logit != nullptr, bl, E, p.score_fn, lane, s);
+    if (!p.scores_in && prunes) {
 #pragma unroll
       for (int i = 0; i < NV; ++i) {
         const int e = lane + 32 * i;
         if (e < E) p.scores[(size_t)t * E + e] = s[i];
       }
     }
-    caee_route_token<NV>(s, p.corr_bias, E, k, p.n_group, p.topk_group, p.norm_topk, lane, s_idx + t * k, s_gate + t * k);
+    caee_route_token<NV>(s, p.corr_bias != nullptr, cb, E, k, p.n_group, p.topk_group, p.norm_topk, lane, ir, gr);
+    __syncwarp();
+    if (p.has_prune) caee_prune_token(p.mode, p.flags, p.theta, k, ir, gr, lane, p.acc_I, p.acc_act, p.acc_must);
   }
-  __syncthreads();
-
-  // S2-S4
-  const bool prunes = p.has_prune && p.mode != CAEE_PRUNE_NONE;
+  STAMP(1);
   if (p.has_prune) {
-    caee_prune_block(sm, p.mode, p.flags, p.theta, T, E, k, p.D, s_idx, s_gate, p.w_eff, p.part, p.act, p.must, p.keep,
-                     p.I_fix, p.load, p.scalars);
+    grid_barrier(p.bar + 0, G);
+    STAMP(2);
+    // ---- B: S2-S4 for the batch, redundantly per CTA; CTA 0 writes the result arrays
+    for (int e = tid; e < E; e += kThreads) {
+      sm.I[e] = __ldcg(p.acc_I + e);
+      sm.act[e] = __ldcg(p.acc_act + e);
+      sm.must[e] = __ldcg(p.acc_must + e);
+    }
     __syncthreads();
-  }
-  // S5: tokens that lost an expert re-select inside A_trans
-  if (prunes) {
-    const float* sc = p.scores_in ? p.scores_in : p.scores;
-    for (int t = warp; t < T; t += nwarps) {
-      int32_t* ir = s_idx + t * k;
+    caee_prune_decide(sm, p.mode, p.theta, E, p.D, p.w_eff, p.part, blockIdx.x == 0, p.act, p.must, p.keep, p.I_fix, p.load,
+                      p.scalars);
+    STAMP(3);
+    // ---- C: S5 — a token that lost an expert re-selects inside A_trans
+    if (live && prunes) {
       bool bad = false;
       if (lane < k) { const int e = ir[lane]; bad = e >= 0 && !sm.keep[e]; }
       const bool affected = __any_sync(0xffffffffu, bad) || (p.flags & CAEE_COMP_ALL_TOKENS);
-      if (affected) caee_compensate_token<NV>(sc + (size_t)t * E, p.corr_bias, sm.keep, E, k, p.norm_topk, lane, ir, s_gate + t * k);
+      if (affected) {
+        const float* sc = p.scores_in ? p.scores_in : p.scores;
+        caee_compensate_token<NV>(sc + (size_t)t * E, p.corr_bias != nullptr, cb, sm.keep, E, k, p.norm_topk, lane, ir, gr);
+        __syncwarp();
+      }
     }
-    __syncthreads();
   }
+  // publish K_final: global idx/gate rows and the membership bits
+  if (live && lane < k) {
+    const int e = ir[lane];
+    p.idx[(size_t)t * k + lane] = e;
+    p.gate[(size_t)t * k + lane] = gr[lane];
+    if (e >= 0) atomicOr(p.M + (size_t)e * kWords + (t >> 5), 1u << (t & 31));
+  }
+  STAMP(4);
+  grid_barrier(p.bar + 1, G);
+  STAMP(5);
 
-  // S6: counts -> scan -> fill; K_final to global
-  for (int i = tid; i < T * k; i += kDecideThreads) {
-    const int e = s_idx[i];
-    p.idx[i] = e;
-    p.gate[i] = s_gate[i];
-    if (e >= 0) atomicAdd(&s_cnt[e], 1);
+  // ---- D: S6 — counts and scans per CTA, entries per token, runs/meta/stats by CTA 0
+  int cnt = 0;
+  if (tid < E) {
+    const uint4* row = reinterpret_cast<const uint4*>(p.M + (size_t)tid * kWords);
+#pragma unroll
+    for (int q = 0; q < kWords / 4; ++q) {
+      const uint4 v = __ldcg(row + q);
+      cnt += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
+    }
+  }
+  caee_wl_scan_block(p.wl, cnt, s_est, p.resident, T, E, p.S, k, blockIdx.x == 0, s_scan);
+  __syncthreads();
+  STAMP(6);
+  if (live) caee_wl_fill_token(p.wl, p.M, kWords, s_est, ir, gr, t, T, E, p.S, k, lane);
+  if (blockIdx.x == 0 && p.stats && tid < 64)
+    caee_stats_fill(p.stats, p.scalars, p.load, p.wl.meta, p.D, p.S, p.has_prune, p.bytes_per_expert, 0, tid, 64);
+
+  // ---- exit: the last CTA out clears the scratch for the next step
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = atomicAdd(p.bar + 2, 1) == G - 1;
   }
   __syncthreads();
-  if (warp == 0) caee_wl_scan_warp(p.wl, s_cnt, s_est, p.resident, T, E, p.S, k, lane);
-  __syncthreads();
-  for (int e = warp; e < E + p.S; e += nwarps) caee_wl_fill_expert(p.wl, s_cnt, s_est, s_idx, s_gate, T, E, p.S, k, e, lane);
-  if (p.stats && tid < 64)
-    caee_stats_fill(p.stats, p.scalars, p.load, p.wl.meta, p.D, p.S, p.has_prune, p.bytes_per_expert, 0, tid, 64);
+  if (s_last) {
+    for (int e = tid; e < E; e += kThreads) { p.acc_I[e] = 0; p.acc_act[e] = 0; p.acc_must[e] = 0; }
+    for (int i = tid; i < E * kWords; i += kThreads) p.M[i] = 0;
+    if (tid < 4) p.bar[tid] = 0;
+  }
+  STAMP(7);
 }
 
 }  // namespace
 
-bool caee_decide_fits(const caee_ctx* c, int T) { return T > 0 && (long long)T * c->d.k <= kMaxEnt; }
+bool caee_decide_fits(const caee_ctx* c, int T) { (void)c; return T > 0 && T <= CAEE_DECIDE_MAX_TOKENS; }
 
-void caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* pp, caee_fwd_stats* stats,
-                        cudaStream_t st) {
+size_t caee_decide_scratch_bytes(const caee_ctx* c) {
+  const size_t E = c->d.E;
+  return E * 8 + E + E + 16 /* align */ + E * kWords * 4 + 64;
+}
+
+cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* pp, caee_fwd_stats* stats,
+                               cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   DecideParams p;
   p.logits = scores_in ? nullptr : c->logits;
@@ -125,10 +220,20 @@ void caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_p
   p.act = c->act; p.must = c->must; p.keep = c->keep; p.I_fix = c->I_fix; p.load = c->load; p.scalars = c->scalars;
   p.wl = c->wl; p.n_sched = c->wl.n_tickets + c->wl.max_runs;
   p.stats = stats; p.bytes_per_expert = caee_expert_bytes(c);
+  const size_t E = d.E;
+  uint8_t* z = c->decide_scratch;
+  p.acc_I = reinterpret_cast<unsigned long long*>(z);
+  p.acc_act = z + E * 8;
+  p.acc_must = z + E * 9;
+  const size_t m_off = (E * 10 + 15) & ~(size_t)15;
+  p.M = reinterpret_cast<uint32_t*>(z + m_off);
+  p.bar = reinterpret_cast<int*>(z + m_off + E * kWords * 4);
   const int nv = caee_ceil_div(d.E, 32);
-  if (nv <= 1) k_decide<1><<<1, kDecideThreads, 0, st>>>(p);
-  else if (nv <= 2) k_decide<2><<<1, kDecideThreads, 0, st>>>(p);
-  else if (nv <= 4) k_decide<4><<<1, kDecideThreads, 0, st>>>(p);
-  else if (nv <= 8) k_decide<8><<<1, kDecideThreads, 0, st>>>(p);
-  else k_decide<16><<<1, kDecideThreads, 0, st>>>(p);
+  const void* fn = nv <= 1   ? (const void*)k_decide<1>
+                   : nv <= 2 ? (const void*)k_decide<2>
+                   : nv <= 4 ? (const void*)k_decide<4>
+                   : nv <= 8 ? (const void*)k_decide<8>
+                             : (const void*)k_decide<16>;
+  void* args[] = {&p};
+  return cudaLaunchCooperativeKernel(fn, dim3(caee_ceil_div(T, kWarps)), dim3(kThreads), args, 0, st);
 }

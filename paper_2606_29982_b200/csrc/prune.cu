@@ -20,7 +20,13 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, do
                                                          uint8_t* __restrict__ keep_o, int64_t* __restrict__ I_o,
                                                          int64_t* __restrict__ load_o, int64_t* __restrict__ scalars) {
   __shared__ caee_prune_smem sm;
-  caee_prune_block(sm, mode, flags, theta, T, E, k, D, idx, gate, w_eff, part, act_o, must_o, keep_o, I_o, load_o, scalars);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int e = tid; e < E; e += PRUNE_THREADS) { sm.I[e] = 0; sm.act[e] = 0; sm.must[e] = 0; }
+  __syncthreads();
+  for (int t = warp; t < T; t += PRUNE_THREADS / 32)
+    caee_prune_token(mode, flags, theta, k, idx + (size_t)t * k, gate + (size_t)t * k, lane, sm.I, sm.act, sm.must);
+  __syncthreads();
+  caee_prune_decide(sm, mode, theta, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
 template <int NV>
@@ -35,7 +41,10 @@ __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ sc
   if (lane < k) { int e = ir[lane]; bad = e >= 0 && !keep[e]; }
   bool affected = __any_sync(0xffffffffu, bad) || (flags & CAEE_COMP_ALL_TOKENS);
   if (!affected) return;
-  caee_compensate_token<NV>(scores + (size_t)t * E, corr_bias, keep, E, k, norm_topk, lane, ir, gate + (size_t)t * k);
+  float cb[NV];
+  caee_load_vec<NV>(corr_bias, E, lane, cb);
+  caee_compensate_token<NV>(scores + (size_t)t * E, corr_bias != nullptr, cb, keep, E, k, norm_topk, lane, ir,
+                            gate + (size_t)t * k);
 }
 
 }  // namespace

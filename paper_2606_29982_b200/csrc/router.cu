@@ -143,9 +143,11 @@ __global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ lo
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (t >= T) return;
-  float s[NV];
-  caee_token_scores<NV>(scores_in ? scores_in + (size_t)t * E : nullptr, logits ? logits + (size_t)t * E : nullptr, b_logit,
-                        E, score_fn, lane, s);
+  float s[NV], bl[NV], cb[NV];
+  caee_load_vec<NV>(b_logit, E, lane, bl);
+  caee_load_vec<NV>(corr_bias, E, lane, cb);
+  caee_token_scores<NV>(scores_in ? scores_in + (size_t)t * E : nullptr, logits ? logits + (size_t)t * E : nullptr,
+                        b_logit != nullptr, bl, E, score_fn, lane, s);
   if (scores_out) {
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
@@ -153,7 +155,7 @@ __global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ lo
       if (e < E) scores_out[(size_t)t * E + e] = s[i];
     }
   }
-  caee_route_token<NV>(s, corr_bias, E, k, n_group, topk_group, norm_topk, lane, idx + (size_t)t * k, gate + (size_t)t * k);
+  caee_route_token<NV>(s, corr_bias != nullptr, cb, E, k, n_group, topk_group, norm_topk, lane, idx + (size_t)t * k, gate + (size_t)t * k);
 }
 
 template <int NV>

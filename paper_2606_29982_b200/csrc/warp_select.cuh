@@ -8,6 +8,12 @@
 #include <stdint.h>
 
 #define CAEE_NONE_ID 0x7fffffff
+#ifdef CAEE_DECIDE_TIMING
+__device__ long long g_route_clk[16];
+#define RSTAMP(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) g_route_clk[i] = clock64(); } while (0)
+#else
+#define RSTAMP(i)
+#endif
 
 __device__ __forceinline__ bool caee_before(float va, int ia, float vb, int ib) {
   return va > vb || (va == vb && ia < ib);
@@ -33,34 +39,78 @@ __device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint3
 #pragma unroll
   for (int i = 0; i < NV; ++i) grp[i] = ((ok >> i) & 1u) ? (lane + 32 * i) / gs : -1;
   float my_gscore = -INFINITY;  // lane g holds the score of group g
-  for (int g = 0; g < n_group; ++g) {
+  // top-2 merge of two (m1 >= m2) pairs
+#define CAEE_TOP2_MERGE(m1, m2, o1, o2)                   \
+  do {                                                    \
+    const float hi_ = fmaxf(m1, o1), lo_ = fminf(m1, o1); \
+    m2 = fmaxf(lo_, fmaxf(m2, o2));                       \
+    m1 = hi_;                                             \
+  } while (0)
+  if ((gs & 31) == 0) {
+    // a register slot lies inside one group: NV independent butterflies, then merge a group's slots
+    const int sg = gs >> 5;
+    float a1[NV], a2[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) { a1[i] = grp[i] >= 0 ? sp[i] : -INFINITY; a2[i] = -INFINITY; }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        const float o1 = __shfl_xor_sync(0xffffffffu, a1[i], o), o2 = __shfl_xor_sync(0xffffffffu, a2[i], o);
+        CAEE_TOP2_MERGE(a1[i], a2[i], o1, o2);
+      }
+    }
     float m1 = -INFINITY, m2 = -INFINITY;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      if (grp[i] == g) {
-        float v = sp[i];
-        if (v > m1) { m2 = m1; m1 = v; }
-        else if (v > m2) m2 = v;
+      if (i * 32 < E) {
+        if (i % sg == 0) { m1 = -INFINITY; m2 = -INFINITY; }
+        CAEE_TOP2_MERGE(m1, m2, a1[i], a2[i]);
+        if (i % sg == sg - 1 && lane == i / sg) my_gscore = __fadd_rn(m1, m2);
       }
     }
+  } else if (gs < 32 && (gs & (gs - 1)) == 0) {
+    // a group is an aligned segment of gs lanes of one slot: segmented butterflies
+    const int per = 32 / gs;   // groups per slot
 #pragma unroll
-    for (int o = 16; o; o >>= 1) {
-      float o1 = __shfl_xor_sync(0xffffffffu, m1, o);
-      float o2 = __shfl_xor_sync(0xffffffffu, m2, o);
-      float hi = fmaxf(m1, o1), lo = fminf(m1, o1);
-      m2 = fmaxf(lo, fmaxf(m2, o2));
-      m1 = hi;
+    for (int i = 0; i < NV; ++i) {
+      float m1 = grp[i] >= 0 ? sp[i] : -INFINITY, m2 = -INFINITY;
+      for (int o = gs >> 1; o; o >>= 1) {
+        const float o1 = __shfl_xor_sync(0xffffffffu, m1, o), o2 = __shfl_xor_sync(0xffffffffu, m2, o);
+        CAEE_TOP2_MERGE(m1, m2, o1, o2);
+      }
+      const float sc = gs >= 2 ? __fadd_rn(m1, m2) : m1;
+      const float v = __shfl_sync(0xffffffffu, sc, (lane % per) * gs);
+      if (lane / per == i) my_gscore = v;
     }
-    float sc = gs >= 2 ? __fadd_rn(m1, m2) : m1;
-    if (lane == g) my_gscore = sc;
+  } else {
+    for (int g = 0; g < n_group; ++g) {
+      float m1 = -INFINITY, m2 = -INFINITY;
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        if (grp[i] == g) {
+          float v = sp[i];
+          if (v > m1) { m2 = m1; m1 = v; }
+          else if (v > m2) m2 = v;
+        }
+      }
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        const float o1 = __shfl_xor_sync(0xffffffffu, m1, o), o2 = __shfl_xor_sync(0xffffffffu, m2, o);
+        CAEE_TOP2_MERGE(m1, m2, o1, o2);
+      }
+      const float sc = gs >= 2 ? __fadd_rn(m1, m2) : m1;
+      if (lane == g) my_gscore = sc;
+    }
   }
-  uint32_t gsel = 0;
-  for (int j = 0; j < topk_group; ++j) {
-    float v = (lane < n_group && !((gsel >> lane) & 1u)) ? my_gscore : -INFINITY;
-    int id = (lane < n_group && !((gsel >> lane) & 1u)) ? lane : CAEE_NONE_ID;
-    caee_warp_argmax(v, id);
-    if (id != CAEE_NONE_ID) gsel |= 1u << id;
+#undef CAEE_TOP2_MERGE
+  // the topk_group best groups by (score desc, id asc): lane g counts the groups before it
+  int before = 0;
+  for (int g = 0; g < n_group; ++g) {
+    const float og = __shfl_sync(0xffffffffu, my_gscore, g);
+    before += caee_before(og, g, my_gscore, lane) ? 1 : 0;
   }
+  const uint32_t gsel = __ballot_sync(0xffffffffu, lane < n_group && before < topk_group);
   uint32_t m = 0;
 #pragma unroll
   for (int i = 0; i < NV; ++i)
@@ -110,10 +160,22 @@ __device__ __forceinline__ void caee_warp_select(const float (&s)[NV], const flo
 
 // One token's post-activation scores s (S0 tail): either loaded (scores_row) or computed from
 // the token's logits row + b_logit: sigmoid, or softmax over the E experts (R1).
+// Per-expert vector (b_logit, corr_bias) into the warp's register layout; zeros without one.
+// Kernels load these first so that their (cold) latency overlaps the first score loads.
+template <int NV>
+__device__ __forceinline__ void caee_load_vec(const float* __restrict__ p, int E, int lane, float (&v)[NV]) {
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int e = lane + 32 * i;
+    v[i] = (p && e < E) ? p[e] : 0.f;
+  }
+}
+
 template <int NV>
 __device__ __forceinline__ void caee_token_scores(const float* __restrict__ scores_row, const float* __restrict__ logits_row,
-                                                  const float* __restrict__ b_logit, int E, int score_fn, int lane,
+                                                  bool has_bl, const float (&bl)[NV], int E, int score_fn, int lane,
                                                   float (&s)[NV]) {
+  RSTAMP(0);
   if (scores_row) {
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
@@ -133,7 +195,7 @@ __device__ __forceinline__ void caee_token_scores(const float* __restrict__ scor
   for (int i = 0; i < NV; ++i) {
     int e = lane + 32 * i;
     if (e < E) {
-      if (b_logit) l[i] += b_logit[e];
+      if (has_bl) l[i] += bl[i];
       mx = fmaxf(mx, l[i]);
     }
   }
@@ -159,7 +221,7 @@ __device__ __forceinline__ void caee_token_scores(const float* __restrict__ scor
 
 // S1 for one token: selection score s' = s + corr_bias, group limit, top-k, gates.
 template <int NV>
-__device__ __forceinline__ void caee_route_token(const float (&s)[NV], const float* __restrict__ corr_bias, int E, int k,
+__device__ __forceinline__ void caee_route_token(const float (&s)[NV], bool has_cb, const float (&cb)[NV], int E, int k,
                                                  int n_group, int topk_group, int norm_topk, int lane, int32_t* idx_out,
                                                  float* gate_out) {
   float sp[NV];
@@ -167,16 +229,19 @@ __device__ __forceinline__ void caee_route_token(const float (&s)[NV], const flo
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     int e = lane + 32 * i;
-    sp[i] = (corr_bias && e < E) ? __fadd_rn(s[i], corr_bias[e]) : s[i];
+    sp[i] = (has_cb && e < E) ? __fadd_rn(s[i], cb[i]) : s[i];
     if (e < E) ok |= 1u << i;
   }
+  RSTAMP(1);
   if (n_group > 1 && topk_group < n_group) ok &= caee_group_mask<NV>(sp, ok, E, n_group, topk_group, lane);
+  RSTAMP(2);
   caee_warp_select<NV>(s, sp, ok, k, norm_topk, lane, idx_out, gate_out);
+  RSTAMP(3);
 }
 
 // S5 for one token: top-k of s' over the experts of A_trans only, no group limit (R13).
 template <int NV>
-__device__ __forceinline__ void caee_compensate_token(const float* __restrict__ scores_row, const float* __restrict__ corr_bias,
+__device__ __forceinline__ void caee_compensate_token(const float* __restrict__ scores_row, bool has_cb, const float (&cb)[NV],
                                                       const uint8_t* keep, int E, int k, int norm_topk, int lane,
                                                       int32_t* idx_out, float* gate_out) {
   float s[NV], sp[NV];
@@ -185,7 +250,7 @@ __device__ __forceinline__ void caee_compensate_token(const float* __restrict__ 
   for (int i = 0; i < NV; ++i) {
     int e = lane + 32 * i;
     s[i] = e < E ? scores_row[e] : 0.f;
-    sp[i] = (corr_bias && e < E) ? __fadd_rn(s[i], corr_bias[e]) : s[i];
+    sp[i] = (has_cb && e < E) ? __fadd_rn(s[i], cb[i]) : s[i];
     if (e < E && keep[e]) ok |= 1u << i;
   }
   __syncwarp();

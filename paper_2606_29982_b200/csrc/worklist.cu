@@ -16,8 +16,10 @@ __global__ void k_wl_count(const int32_t* __restrict__ idx, int n, int32_t* __re
   }
 }
 
-__global__ void k_wl_scan(caee_worklist wl, const uint8_t* __restrict__ resident, int T, int E, int S, int k) {
-  caee_wl_scan_warp(wl, wl.counts, wl.estart, resident, T, E, S, k, threadIdx.x);
+__global__ void __launch_bounds__(CAEE_MAX_E) k_wl_scan(caee_worklist wl, const uint8_t* __restrict__ resident, int T, int E,
+                                                        int S, int k) {
+  __shared__ int scratch[33 * 6];
+  caee_wl_scan_block(wl, threadIdx.x < E ? wl.counts[threadIdx.x] : 0, wl.estart, resident, T, E, S, k, true, scratch);
 }
 
 __global__ void k_wl_fill(caee_worklist wl, const int32_t* __restrict__ idx, const float* __restrict__ gate, int T, int E,
@@ -51,7 +53,7 @@ void caee_launch_worklist(caee_ctx* c, int T, const int32_t* idx, const float* g
   cudaMemsetAsync(c->wl.sched, 0, sizeof(int32_t) * (c->wl.n_tickets + c->wl.max_runs), st);
   int n = T * d.k;
   if (n > 0) k_wl_count<<<caee_ceil_div(n, 256), 256, 0, st>>>(idx, n, c->wl.counts);
-  k_wl_scan<<<1, 32, 0, st>>>(c->wl, c->resident, T, d.E, d.S, d.k);
+  k_wl_scan<<<1, CAEE_MAX_E, 0, st>>>(c->wl, c->resident, T, d.E, d.S, d.k);
   k_wl_fill<<<d.E + d.S, 32, 0, st>>>(c->wl, idx, gate, T, d.E, d.S, d.k);
 }
 

@@ -12,78 +12,6 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   return v;
 }
 
-// One warp (all 32 lanes call it): scans over experts -> compact ids/offsets, per-expert entry starts, runs.
-// Run order: resident routed experts (ascending id), then the shared experts, then the
-// non-resident routed experts (ascending id) — so that an offloading step can launch the
-// resident part while the misses are still being fetched (meta[4] = runs in the first two groups).
-__device__ __forceinline__ void caee_wl_scan_warp(const caee_worklist& wl, const int32_t* counts, int32_t* estart,
-                                                  const uint8_t* __restrict__ resident, int T, int E, int S, int k, int lane) {
-  int n_nz = 0, n_ent = 0;
-  for (int e0 = 0; e0 < E; e0 += 32) {
-    int e = e0 + lane;
-    int c = e < E ? counts[e] : 0;
-    int nz = c > 0;
-    int s_nz = warp_incl_scan(nz, lane), s_c = warp_incl_scan(c, lane);
-    if (e < E) {
-      int start = n_ent + s_c - c;
-      estart[e] = start;
-      if (nz) {
-        int pos = n_nz + s_nz - 1;
-        wl.expert_ids[pos] = e;
-        wl.offs[pos] = start;
-      }
-    }
-    n_nz += __shfl_sync(0xffffffffu, s_nz, 31);
-    n_ent += __shfl_sync(0xffffffffu, s_c, 31);
-  }
-  int n_runs = 0, n_rows = 0;
-  for (int pass = 0; pass < 2; ++pass) {
-    for (int e0 = 0; e0 < E; e0 += 32) {
-      int e = e0 + lane;
-      int c = (e < E && (resident[e] != 0) == (pass == 0)) ? counts[e] : 0;
-      int nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
-      int s_ch = warp_incl_scan(nch, lane), s_rows = warp_incl_scan(rows, lane);
-      if (c > 0) {
-        int start = estart[e];
-        int r0 = n_runs + s_ch - nch, h0 = n_rows + s_rows - rows;
-        for (int j = 0; j < nch; ++j) {
-          wl.run_expert[r0 + j] = e;
-          wl.run_start[r0 + j] = start + j * CAEE_RUN_TOKENS;
-          wl.run_n[r0 + j] = min(CAEE_RUN_TOKENS, c - j * CAEE_RUN_TOKENS);
-          wl.run_hrow[r0 + j] = h0 + j * CAEE_RUN_TOKENS;
-        }
-      }
-      n_runs += __shfl_sync(0xffffffffu, s_ch, 31);
-      n_rows += __shfl_sync(0xffffffffu, s_rows, 31);
-    }
-    if (pass == 0) {
-      if (lane == 0 && T > 0) {
-        const int TK = T * k;
-        for (int s = 0; s < S; ++s)
-          for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) {
-            int n = min(CAEE_RUN_TOKENS, T - t0);
-            wl.run_expert[n_runs] = E + s;
-            wl.run_start[n_runs] = TK + s * T + t0;
-            wl.run_n[n_runs] = n;
-            wl.run_hrow[n_runs] = n_rows;
-            n_rows += (n + 15) & ~15;
-            ++n_runs;
-          }
-      }
-      n_runs = __shfl_sync(0xffffffffu, n_runs, 0);
-      n_rows = __shfl_sync(0xffffffffu, n_rows, 0);
-      if (lane == 0) wl.meta[4] = n_runs;
-    }
-  }
-  if (lane == 0) {
-    wl.offs[n_nz] = n_ent;
-    wl.meta[0] = n_nz;
-    wl.meta[2] = n_ent;
-    wl.meta[1] = n_runs;
-    wl.meta[3] = n_rows;
-  }
-}
-
 // One warp lists expert e's (token, slot) pairs in ascending entry order (e < E), or the
 // entries of shared expert e - E (every token).
 __device__ __forceinline__ void caee_wl_fill_expert(const caee_worklist& wl, const int32_t* counts, const int32_t* estart,
@@ -116,6 +44,114 @@ __device__ __forceinline__ void caee_wl_fill_expert(const caee_worklist& wl, con
   }
 }
 
+
+// Block-wide exclusive scan of N ints per thread (blockDim.x <= 1024, a multiple of 32).
+// scratch: 33 * N ints of shared memory.  ex = sum over lower threads, tot = sum over the block.
+template <int N>
+__device__ __forceinline__ void caee_block_excl_scan(const int (&v)[N], int (&ex)[N], int (&tot)[N], int* scratch) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  int inc[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) inc[i] = warp_incl_scan(v[i], lane);
+  if (lane == 31) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) scratch[warp * N + i] = inc[i];
+  }
+  __syncthreads();
+  if (warp == 0) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+      const int w = lane < nwarps ? scratch[lane * N + i] : 0;
+      const int s = warp_incl_scan(w, lane);
+      if (lane < nwarps) scratch[lane * N + i] = s - w;
+      if (lane == 31) scratch[32 * N + i] = s;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    ex[i] = scratch[warp * N + i] + inc[i] - v[i];
+    tot[i] = scratch[32 * N + i];
+  }
+  __syncthreads();
+}
+
+// S6 scans for a whole CTA (blockDim.x >= E): thread e owns expert e.  Fills estart[e] (shared
+// or global) and, with `write`, the compact ids/offsets, the runs and meta of wl.
+// Run order: resident routed experts (ascending id), then the shared experts, then the
+// non-resident routed experts (ascending id) — so that an offloading step can launch the
+// resident part while the misses are still being fetched (meta[4] = runs in the first two groups).
+__device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int count_e, int32_t* estart,
+                                                   const uint8_t* __restrict__ resident, int T, int E, int S, int k, bool write,
+                                                   int* scratch /* 33 * 6 ints */) {
+  const int e = threadIdx.x;
+  const int c = e < E ? count_e : 0;
+  const bool res = e < E && resident[e] != 0;
+  const int nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
+  const int v[6] = {c > 0, c, res ? nch : 0, res ? rows : 0, res ? 0 : nch, res ? 0 : rows};
+  int ex[6], tot[6];
+  caee_block_excl_scan<6>(v, ex, tot, scratch);
+  if (e < E) estart[e] = ex[1];
+  if (!write) return;
+  const int sh_chunks = T > 0 ? (T + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS : 0;
+  const int sh_runs = S * sh_chunks;
+  int sh_rows_each = 0;   // h rows of one shared expert: every chunk padded to 16
+  for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) sh_rows_each += (min(CAEE_RUN_TOKENS, T - t0) + 15) & ~15;
+  if (c > 0) {
+    wl.expert_ids[ex[0]] = e;
+    wl.offs[ex[0]] = ex[1];
+    const int r0 = res ? ex[2] : tot[2] + sh_runs + ex[4];
+    const int h0 = res ? ex[3] : tot[3] + S * sh_rows_each + ex[5];
+    for (int j = 0; j < nch; ++j) {
+      wl.run_expert[r0 + j] = e;
+      wl.run_start[r0 + j] = ex[1] + j * CAEE_RUN_TOKENS;
+      wl.run_n[r0 + j] = min(CAEE_RUN_TOKENS, c - j * CAEE_RUN_TOKENS);
+      wl.run_hrow[r0 + j] = h0 + j * CAEE_RUN_TOKENS;
+    }
+  }
+  for (int i = e; i < sh_runs; i += blockDim.x) {   // shared-expert runs over all tokens
+    const int s = i / sh_chunks, j = i - s * sh_chunks, t0 = j * CAEE_RUN_TOKENS;
+    const int r = tot[2] + i;
+    wl.run_expert[r] = E + s;
+    wl.run_start[r] = T * k + s * T + t0;
+    wl.run_n[r] = min(CAEE_RUN_TOKENS, T - t0);
+    wl.run_hrow[r] = tot[3] + s * sh_rows_each + j * CAEE_RUN_TOKENS;
+  }
+  if (e == 0) {
+    wl.offs[tot[0]] = tot[1];
+    wl.meta[0] = tot[0];
+    wl.meta[1] = tot[2] + sh_runs + tot[4];
+    wl.meta[2] = tot[1];
+    wl.meta[3] = tot[3] + S * sh_rows_each + tot[5];
+    wl.meta[4] = tot[2] + sh_runs;
+  }
+}
+
+// Decode-size fill (T <= 256): M is the E x W bit matrix "expert e is in K_final of token t"
+// (W = 8 words per expert), so an entry's place in its expert's list is a popcount.
+// One warp, one token: lanes j < k place the token's routed entries, lanes s < S the shared ones.
+__device__ __forceinline__ void caee_wl_fill_token(const caee_worklist& wl, const uint32_t* M, int W, const int32_t* estart,
+                                                   const int32_t* ir, const float* gr, int t, int T, int E, int S, int k,
+                                                   int lane) {
+  const int KS = k + S, TK = T * k;
+  if (lane < k) {
+    const int e = ir[lane];
+    if (e >= 0) {
+      const uint32_t* row = M + (size_t)e * W;
+      int pos = estart[e];
+      for (int w = 0; w < (t >> 5); ++w) pos += __popc(__ldcg(row + w));
+      pos += __popc(__ldcg(row + (t >> 5)) & ((1u << (t & 31)) - 1u));
+      wl.ent_tok[pos] = t;
+      wl.ent_slot[pos] = lane;
+      wl.ent_wt[pos] = gr[lane];
+      wl.ent_dst[pos] = t * KS + lane;
+    }
+  }
+  if (lane < S) {
+    wl.ent_tok[TK + lane * T + t] = t;
+    wl.ent_dst[TK + lane * T + t] = t * KS + k + lane;
+  }
+}
 
 // caee_fwd_stats of one step (all threads of the calling group take part; nth >= 1).
 __device__ __forceinline__ void caee_stats_fill(caee_fwd_stats* st, const int64_t* scalars, const int64_t* load,
