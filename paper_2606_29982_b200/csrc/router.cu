@@ -10,94 +10,115 @@
 
 namespace {
 
-constexpr int TE = 64, KC = 32, WS = TE + 4;   // expert tile, k chunk, padded smem row (keeps 16 B alignment)
+constexpr int TE = 64, KC = 32;          // expert tile, k elements per pipeline stage
+constexpr int WROW = KC * 4 + 16;        // bytes of one W row in shared memory (16 B pad: conflict-free LDS.128)
 
-template <typename XT>
-__device__ __forceinline__ float4 ld_act4(const XT* p);
-template <>
-__device__ __forceinline__ float4 ld_act4<float>(const float* p) { return *reinterpret_cast<const float4*>(p); }
-template <>
-__device__ __forceinline__ float4 ld_act4<__nv_bfloat16>(const __nv_bfloat16* p) {
-  const uint2 u = *reinterpret_cast<const uint2*>(p);
-  return make_float4(__uint_as_float(u.x << 16), __uint_as_float(u.x & 0xffff0000u), __uint_as_float(u.y << 16),
-                     __uint_as_float(u.y & 0xffff0000u));
+template <typename XT> struct XTraits;
+template <> struct XTraits<float> {
+  static constexpr int kRow = KC * 4 + 16, kChunks = KC / 4, kStages = 3;
+  static __device__ __forceinline__ void ld4(const uint8_t* p, float (&v)[4]) {
+    const float4 f = *reinterpret_cast<const float4*>(p);
+    v[0] = f.x; v[1] = f.y; v[2] = f.z; v[3] = f.w;
+  }
+};
+template <> struct XTraits<__nv_bfloat16> {
+  static constexpr int kRow = KC * 2 + 16, kChunks = KC / 8, kStages = 4;
+  static __device__ __forceinline__ void ld4(const uint8_t* p, float (&v)[4]) {
+    const uint2 u = *reinterpret_cast<const uint2*>(p);
+    v[0] = __uint_as_float(u.x << 16); v[1] = __uint_as_float(u.x & 0xffff0000u);
+    v[2] = __uint_as_float(u.y << 16); v[3] = __uint_as_float(u.y & 0xffff0000u);
+  }
+};
+
+__device__ __forceinline__ void cp_async16(void* dst, const void* src, bool valid) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
+  const uint32_t n = valid ? 16u : 0u;   // src-size 0: zero fill
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
 }
 
 // Split-K router GEMM  logit[t,e] = sum_h x[t,h] W_r[e,h]  (S0).
 // Grid (E/64, T/TT, ksplit); CTA tile 64 experts x TT tokens, thread tile 4 x TT/16, fp32 FMAs in
-// ascending h.  Each CTA writes its partial tile; the LAST CTA of a tile to finish (ticket
-// counter) adds the ksplit partials in ascending ks and writes the logits, so the result
-// does not depend on which CTA came last: scores are deterministic.
+// ascending h.  W_r and x tiles stream through a cp.async ring (3-4 stages in flight: the
+// weights are cold in L2 every step, the expert stream has flushed them).  Each CTA writes its
+// partial tile; the LAST CTA of a tile to finish (ticket counter) adds the ksplit partials in
+// ascending ks and writes the logits, so the result does not depend on which CTA came last:
+// scores are deterministic.
 template <typename XT, int TT>
 __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x, const float* __restrict__ Wr,
                                                        float* __restrict__ partial, float* __restrict__ logits,
                                                        int* __restrict__ tile_ctr, int T, int H, int E, int Hs) {
-  constexpr int TPT = TT / 16, XS = TT + 4;
-  __shared__ __align__(16) float ws[KC][WS];
-  __shared__ __align__(16) float xs[KC][XS];
+  using XR = XTraits<XT>;
+  constexpr int TPT = TT / 16, NS = TT >= 64 ? (sizeof(XT) == 4 ? 2 : 3) : XR::kStages;   // static shared memory stays below 48 KB
+  constexpr int kStageBytes = TE * WROW + TT * XR::kRow;
+  __shared__ __align__(16) uint8_t ring[NS * kStageBytes];
   __shared__ int last_s;
   const int e0 = blockIdx.x * TE, t0 = blockIdx.y * TT, ks = blockIdx.z, ksplit = gridDim.z;
   const int h_lo = ks * Hs, h_hi = min(H, h_lo + Hs);
+  const int n_it = h_hi > h_lo ? (h_hi - h_lo + KC - 1) / KC : 0;
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   float acc[TPT][4];
 #pragma unroll
   for (int i = 0; i < TPT; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
-  // loaders: W tile = 64 rows x 32 k = 512 float4 (2 per thread); x tile = TT rows x 32 k = TT*8 float4
-  float4 wreg[2], xreg;
-  auto load_tiles = [&](int h0) {
+
+  auto issue = [&](int it) {
+    if (it < n_it) {
+      uint8_t* st = ring + (it % NS) * kStageBytes;
+      const int h0 = h_lo + it * KC;
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      const int i = tid + 256 * q, r = i >> 3, kq = (i & 7) * 4;
-      const int e = e0 + r, h = h0 + kq;
-      wreg[q] = (e < E && h < h_hi) ? *reinterpret_cast<const float4*>(Wr + (size_t)e * H + h) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    if (tid < TT * 8) {
-      const int r = tid >> 3, kq = (tid & 7) * 4;
-      const int t = t0 + r, h = h0 + kq;
-      xreg = (t < T && h < h_hi) ? ld_act4<XT>(x + (size_t)t * H + h) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-  };
-  auto store_tiles = [&]() {
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      const int i = tid + 256 * q, r = i >> 3, kq = (i & 7) * 4;
-      ws[kq][r] = wreg[q].x; ws[kq + 1][r] = wreg[q].y; ws[kq + 2][r] = wreg[q].z; ws[kq + 3][r] = wreg[q].w;
-    }
-    if (tid < TT * 8) {
-      const int r = tid >> 3, kq = (tid & 7) * 4;
-      xs[kq][r] = xreg.x; xs[kq + 1][r] = xreg.y; xs[kq + 2][r] = xreg.z; xs[kq + 3][r] = xreg.w;
-    }
-  };
-  load_tiles(h_lo);
-  for (int h0 = h_lo; h0 < h_hi; h0 += KC) {
-    store_tiles();
-    __syncthreads();
-    if (h0 + KC < h_hi) load_tiles(h0 + KC);   // next chunk's global loads overlap this chunk's FMAs
-#pragma unroll
-    for (int kk = 0; kk < KC; ++kk) {
-      const float4 w = *reinterpret_cast<const float4*>(&ws[kk][tx * 4]);
-      float xv[TPT];
-#pragma unroll
-      for (int i = 0; i < TPT; ++i) xv[i] = xs[kk][ty * TPT + i];
-#pragma unroll
-      for (int i = 0; i < TPT; ++i) {
-        acc[i][0] = fmaf(xv[i], w.x, acc[i][0]);
-        acc[i][1] = fmaf(xv[i], w.y, acc[i][1]);
-        acc[i][2] = fmaf(xv[i], w.z, acc[i][2]);
-        acc[i][3] = fmaf(xv[i], w.w, acc[i][3]);
+      for (int q = 0; q < 2; ++q) {   // W tile: 64 rows x 8 chunks of 4 floats
+        const int i = tid + 256 * q, r = i >> 3, c = i & 7;
+        const int e = e0 + r, h = h0 + c * 4;
+        const bool ok = e < E && h < h_hi;
+        cp_async16(st + r * WROW + c * 16, ok ? Wr + (size_t)e * H + h : Wr, ok);
+      }
+      if (tid < TT * XR::kChunks) {   // x tile: TT rows x kChunks chunks of 16 bytes
+        const int r = tid / XR::kChunks, c = tid % XR::kChunks;
+        const int t = t0 + r, h = h0 + c * (16 / (int)sizeof(XT));
+        const bool ok = t < T && h < h_hi;
+        cp_async16(st + TE * WROW + r * XR::kRow + c * 16, ok ? x + (size_t)t * H + h : x, ok);
       }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+#pragma unroll
+  for (int s = 0; s < NS - 1; ++s) issue(s);
+  for (int it = 0; it < n_it; ++it) {
+    asm volatile("cp.async.wait_group %0;" ::"n"(NS - 2) : "memory");
     __syncthreads();
+    issue(it + NS - 1);   // refills the slot consumed in iteration it - 1
+    const uint8_t* st = ring + (it % NS) * kStageBytes;
+    const uint8_t* wrow = st + tx * WROW;
+    const uint8_t* xrow = st + TE * WROW + (ty * TPT) * XR::kRow;
+#pragma unroll
+    for (int k4 = 0; k4 < KC / 4; ++k4) {
+      float4 w[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) w[j] = *reinterpret_cast<const float4*>(wrow + j * 16 * WROW + k4 * 16);
+#pragma unroll
+      for (int i = 0; i < TPT; ++i) {
+        float xv[4];
+        XR::ld4(xrow + i * XR::kRow + k4 * 4 * (int)sizeof(XT), xv);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          acc[i][j] = fmaf(xv[0], w[j].x, acc[i][j]);
+          acc[i][j] = fmaf(xv[1], w[j].y, acc[i][j]);
+          acc[i][j] = fmaf(xv[2], w[j].z, acc[i][j]);
+          acc[i][j] = fmaf(xv[3], w[j].w, acc[i][j]);
+        }
+      }
+    }
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  // thread (tx, ty) holds experts e0 + tx + 16 j, tokens t0 + ty*TPT + i
   float* out = ksplit == 1 ? logits : partial + (size_t)ks * T * E;
 #pragma unroll
   for (int i = 0; i < TPT; ++i) {
     const int t = t0 + ty * TPT + i;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      const int e = e0 + tx * 4 + j;
+      const int e = e0 + tx + 16 * j;
       if (t < T && e < E) out[(size_t)t * E + e] = acc[i][j];
     }
   }
@@ -114,22 +135,60 @@ __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x,
   __syncthreads();
   if (!last_s) return;
   __threadfence();
-  const int nt = min(TT, T - t0);
-  for (int i = tid; i < nt * (TE / 4); i += 256) {
-    const int t = t0 + i / (TE / 4), e = e0 + (i % (TE / 4)) * 4;
-    if ((E & 3) == 0 && e + 3 < E) {
+  // fixed summation tree: R threads per output quad each add a contiguous range of ks in
+  // ascending order, then the R range sums are added in ascending order
+  const int nt = min(TT, T - t0), items = nt * (TE / 4);
+  int R = 1;
+  while (R * 2 * items <= 256 && R * 2 <= ksplit) R *= 2;
+  const int L = (ksplit + R - 1) / R;
+  float4* part_s = reinterpret_cast<float4*>(ring);
+  if ((E & 3) == 0) {
+    for (int u = tid; u < items * R; u += 256) {
+      const int i = u / R, r = u - i * R;
+      const int t = t0 + i / (TE / 4), e = e0 + (i % (TE / 4)) * 4;
       float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-      for (int s = 0; s < ksplit; ++s) {
-        const float4 v = __ldcg(reinterpret_cast<const float4*>(partial + ((size_t)s * T + t) * E + e));
-        a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+      if (e + 3 < E) {
+        const int s_lo = r * L, s_hi = min(ksplit, s_lo + L);
+        const float* src = partial + (size_t)t * E + e;
+        const size_t stride = (size_t)T * E;
+        int sk = s_lo;
+        for (; sk + 4 <= s_hi; sk += 4) {
+          const float4 v0 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 0) * stride));
+          const float4 v1 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 1) * stride));
+          const float4 v2 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 2) * stride));
+          const float4 v3 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 3) * stride));
+          a.x += v0.x; a.y += v0.y; a.z += v0.z; a.w += v0.w;
+          a.x += v1.x; a.y += v1.y; a.z += v1.z; a.w += v1.w;
+          a.x += v2.x; a.y += v2.y; a.z += v2.z; a.w += v2.w;
+          a.x += v3.x; a.y += v3.y; a.z += v3.z; a.w += v3.w;
+        }
+        for (; sk < s_hi; ++sk) {
+          const float4 v = __ldcg(reinterpret_cast<const float4*>(src + sk * stride));
+          a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+        }
       }
-      *reinterpret_cast<float4*>(logits + (size_t)t * E + e) = a;
-    } else {
-      for (int j = 0; j < 4 && e + j < E; ++j) {
-        float a = 0.f;
-        for (int s = 0; s < ksplit; ++s) a += __ldcg(partial + ((size_t)s * T + t) * E + e + j);
-        logits[(size_t)t * E + e + j] = a;
+      if (R == 1) { if (e + 3 < E) *reinterpret_cast<float4*>(logits + (size_t)t * E + e) = a; }
+      else part_s[u] = a;
+    }
+    if (R > 1) {
+      __syncthreads();
+      for (int i = tid; i < items; i += 256) {
+        const int t = t0 + i / (TE / 4), e = e0 + (i % (TE / 4)) * 4;
+        float4 a = part_s[i * R];
+        for (int r = 1; r < R; ++r) {
+          const float4 v = part_s[i * R + r];
+          a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+        }
+        if (e + 3 < E) *reinterpret_cast<float4*>(logits + (size_t)t * E + e) = a;
       }
+    }
+  } else {
+    for (int i = tid; i < nt * TE; i += 256) {
+      const int t = t0 + i / TE, e = e0 + i % TE;
+      if (e >= E) continue;
+      float a = 0.f;
+      for (int sk = 0; sk < ksplit; ++sk) a += __ldcg(partial + ((size_t)sk * T + t) * E + e);
+      logits[(size_t)t * E + e] = a;
     }
   }
 }
@@ -173,6 +232,7 @@ void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
   const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), KC) * KC;
   dim3 grid(caee_ceil_div(d.E, TE), caee_ceil_div(T, tt), ks);
   if (tt == 16) k_router_logits<XT, 16><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
+  else if (tt == 64) k_router_logits<XT, 64><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
   else k_router_logits<XT, 32><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
 }
 
