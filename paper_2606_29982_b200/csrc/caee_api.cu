@@ -119,7 +119,7 @@ void free_all(caee_ctx* c) {
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
-                  c->packed.dev_ptrs, c->x16};
+                  c->packed.dev_ptrs, c->xq, c->xs, c->hq, c->hs};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (size_t e = 0; e < c->packed.base.size(); ++e) {
@@ -164,7 +164,10 @@ caee_status create_impl(caee_ctx* c) {
   c->h_rows_cap = Tm * k + 15 * std::min(E, Tm * k) + S * (Tm + 15) + 16;
   if (c->kernel == CAEE_KERNEL_SIMT) { A(c->hbuf_f32, c->h_rows_cap * d.I); }
   else { A(c->hbuf_b16, c->h_rows_cap * d.I); }
-  if (c->kernel == CAEE_KERNEL_UMMA && d.w_dtype == CAEE_E4M3) { A(c->x16, Tm * d.H); }
+  if (c->kernel == CAEE_KERNEL_UMMA && d.w_dtype == CAEE_E4M3) {
+    A(c->xq, 2 * Tm * d.H); A(c->xs, Tm * (d.H / 128));
+    A(c->hq, 2 * c->h_rows_cap * d.I); A(c->hs, c->h_rows_cap * (d.I / 128));
+  }
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));

@@ -99,7 +99,11 @@ struct caee_ctx {
   caee_worklist wl;
   float* hbuf_f32 = nullptr;         // SIMT: h rows [rows, I] fp32
   __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16 (bf16 weights) / fp16 (e4m3 weights)
-  __half* x16 = nullptr;             // UMMA e4m3: fp16 copy of x [Tmax, H]
+  __half* x16 = nullptr;             // (unused)
+  uint8_t* xq = nullptr;             // UMMA e4m3: hi | lo e4m3 terms of x, [Tmax, H] each
+  float* xs = nullptr;               //   and its (token, 128-block) scales [Tmax, H/128]
+  uint8_t* hq = nullptr;             // UMMA e4m3: hi | lo terms of h, [rows, I] each
+  float* hs = nullptr;               //   and its scales [rows, I/128]
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
@@ -156,6 +160,13 @@ void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst_dev, const void* g
                              const float* sg, const float* su, const float* sd, cudaStream_t s);
 void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
+// expert_fp8.cu
+caee_status caee_fp8_supported(const caee_ctx* c, std::string* why);
+size_t caee_fp8_packed_bytes(const caee_ctx* c);
+void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst_dev, const void* g, const void* u, const void* d, const float* sg,
+                                 const float* su, const float* sd, cudaStream_t s);
+void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
+void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);

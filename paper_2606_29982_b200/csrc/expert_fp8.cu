@@ -1,0 +1,527 @@
+// expert_fp8.cu — S7 grouped SwiGLU expert FFN for FP8-E4M3 weights with 128x128 block scales
+// (BASELINE.json config 4) on sm_100a: the weight bytes go from HBM to the tensor cores
+// untouched.
+//
+// Design.  At decode the bound is HBM bandwidth (Fig. 1), so the e4m3 codes are
+// streamed exactly once by the bulk async-copy engine into a shared-memory ring and fed to
+// tcgen05.mma kind::f8f6f4 as they are — no widening pass through shared memory (a converter
+// design spends 5x the HBM byte rate in shared-memory traffic and cannot keep up).  The tensor
+// cores need both operands in a narrow format, and rounding the bf16 activations to e4m3
+// would miss the 5e-2 x RMS tolerance, so each activation is split into TWO e4m3 terms,
+//     a / s = hi + lo,   hi = e4m3(a / s),   lo = e4m3(a / s - hi),
+// with one fp32 scale s = amax/448 per (token, 128-wide k block): 2^-8 relative error per
+// element, about bf16's own rounding.  Both terms accumulate into the same TMEM accumulator
+// (two MMAs per weight tile and k-step; the tensor pipe is far from busy at decode).
+// Block scales: a stage is one 128-k block of a 128-row tile pair, i.e. ONE weight scale per
+// accumulator, so the MMA warp gives every k block a fresh TMEM accumulator (double buffered)
+// and the epilogue warps promote it into fp32 registers:
+//     acc[row, tok] += D_kb[row, tok] * w_scale[tile half, kb] * a_scale[tok, kb].
+// x is split once per step (k_act_split); h is split by the phase-1 epilogue that produces it.
+//
+// Layout.  caee_set_weights(pack=1) rewrites every expert into 32 KB stage images: two 128-row x
+// 128-k e4m3 tiles in the UMMA canonical K-major no-swizzle order (8 rows x 16 B core matrices;
+// LBO 128 B, SBO 1024 B), phase 1 = [gate tile | up tile] of the same 128 features, phase 2 =
+// down rows [+0..127 | +128..255]; then the fp32 block-scale table, [tile][kb][half].
+//
+// Roles (384 threads, 1 CTA per SM): warp 0 = weight producer (bulk copies), warp 1 = MMA
+// issuer, warps 2-3 = token-operand loaders (cp.async gathers of the hi/lo rows), warps 4-11 =
+// epilogue (two warps per TMEM lane quadrant, each half of the token columns).  Tiles are
+// claimed by atomic ticket, phase-1 tickets first (see umma_common.cuh).
+#include "umma_common.cuh"
+
+namespace {
+
+using namespace caee_umma;
+
+constexpr int kThreads = 384;
+constexpr int kKBlock = 128;      // k elements per stage = one block-scale block
+constexpr int kEpiWarps = 8;
+
+struct Fp8Params {
+  caee_worklist wl;
+  uint8_t* const* packed;   // [E+S] stage images + scale table
+  const uint8_t* xq_hi;     // [T,H] e4m3
+  const uint8_t* xq_lo;     // [T,H]
+  const float* xs;          // [T,H/128]
+  uint8_t* hq_hi;           // [rows,I]
+  uint8_t* hq_lo;
+  float* hs;                // [rows,I/128]
+  float* obuf;              // [T*(k+S),H]
+  int H, I;
+  int P1, P2, KB1, KB2;     // tiles per run and 128-k stages per tile, per phase
+  int n_stages, stage_bytes, b_term_bytes;
+  int run_begin, run_count, ticket;
+  int sc_off;               // byte offset of the scale table in a packed image
+  int t2_off;               // float offset of its phase-2 part
+};
+
+// two floats -> two e4m3 codes (low byte = a), round to nearest even, saturating
+__device__ __forceinline__ uint16_t cvt_e4m3x2(float a, float b) {
+  uint16_t r;
+  asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(b), "f"(a));
+  return r;
+}
+// two e4m3 codes -> two floats (exact)
+__device__ __forceinline__ float2 e4m3x2_to_float2(uint16_t v) {
+  uint32_t h2;
+  asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(v));
+  return __half22float2(*reinterpret_cast<__half2*>(&h2));
+}
+// a/s as hi + lo (both e4m3), for a pair of values
+__device__ __forceinline__ void split_pair(float a, float b, float inv_s, uint16_t& hi, uint16_t& lo) {
+  const float va = a * inv_s, vb = b * inv_s;
+  hi = cvt_e4m3x2(va, vb);
+  const float2 h = e4m3x2_to_float2(hi);
+  lo = cvt_e4m3x2(va - h.x, vb - h.y);
+}
+
+// Once per step: x[T,H] bf16 -> hi/lo e4m3 terms and the (token, 128-block) scales.
+// One warp per block of 128 elements, 4 per lane.
+__global__ void __launch_bounds__(256) k_act_split(const __nv_bfloat16* __restrict__ x, uint8_t* __restrict__ hi,
+                                                   uint8_t* __restrict__ lo, float* __restrict__ scale, size_t n_blocks) {
+  const size_t b = (size_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (b >= n_blocks) return;
+  const uint2 u = *reinterpret_cast<const uint2*>(x + b * 128 + lane * 4);
+  const float v0 = __uint_as_float(u.x << 16), v1 = __uint_as_float(u.x & 0xffff0000u);
+  const float v2 = __uint_as_float(u.y << 16), v3 = __uint_as_float(u.y & 0xffff0000u);
+  float m = fmaxf(fmaxf(fabsf(v0), fabsf(v1)), fmaxf(fabsf(v2), fabsf(v3)));
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  const float s = m > 0.f ? m * (1.0f / 448.0f) : 1.0f;
+  const float inv = 1.0f / s;
+  uint16_t h01, l01, h23, l23;
+  split_pair(v0, v1, inv, h01, l01);
+  split_pair(v2, v3, inv, h23, l23);
+  *reinterpret_cast<uint32_t*>(hi + b * 128 + lane * 4) = (uint32_t)h01 | ((uint32_t)h23 << 16);
+  *reinterpret_cast<uint32_t*>(lo + b * 128 + lane * 4) = (uint32_t)l01 | ((uint32_t)l23 << 16);
+  if (lane == 0) scale[b] = s;
+}
+
+// One thread per 16 codes: raw row-major [rows, cols] e4m3 -> stage images.
+// which: 0 gate, 1 up (phase-1 region), 2 down (phase-2 region).
+__global__ void __launch_bounds__(256) k_pack_e4m3(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst, int rows,
+                                                   int cols, int which, size_t region_off) {
+  const size_t chunk = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int cpr = cols / 16;
+  if (chunk >= (size_t)rows * cpr) return;
+  const int r = (int)(chunk / cpr), k0 = (int)(chunk % cpr) * 16;
+  const int kb = k0 / kKBlock, kk = k0 % kKBlock, nkb = cols / kKBlock;
+  int tile, half;
+  const int rr = r % kTileRows;
+  if (which < 2) { tile = r / kTileRows; half = which; }
+  else { tile = r / (2 * kTileRows); half = (r / kTileRows) & 1; }
+  const size_t stage = (size_t)tile * nkb + kb;
+  const size_t in_stage = (size_t)half * kATileBytes + (rr / 8) * 1024 + (kk / 16) * 128 + (rr % 8) * 16;
+  const uint4 v = *reinterpret_cast<const uint4*>(src + (size_t)r * cols + k0);
+  *reinterpret_cast<uint4*>(dst + region_off + stage * kAStageBytes + in_stage) = v;
+}
+
+// Block-scale table of one expert: tab[(tile * KS + kb) * 2 + half], phase-1 tiles first.
+//   phase 1, tile ft:  halves = gate rows / up rows of feature block ft   (scale row ft of each)
+//   phase 2, tile op:  halves = down rows 256 op + [0,128) / + [128,256)  (scale rows 2 op, 2 op + 1)
+__global__ void k_scale_table(const float* __restrict__ sg, const float* __restrict__ su, const float* __restrict__ sd,
+                              float* __restrict__ tab, int P1, int P2, int KS1, int KS2) {
+  const int n1 = P1 * KS1 * 2, n2 = P2 * KS2 * 2;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n1 + n2; i += gridDim.x * blockDim.x) {
+    if (i < n1) {
+      const int half = i & 1, kb = (i >> 1) % KS1, ft = (i >> 1) / KS1;
+      tab[i] = (half ? su : sg)[(size_t)ft * KS1 + kb];
+    } else {
+      const int j = i - n1, half = j & 1, kb = (j >> 1) % KS2, op = (j >> 1) / KS2;
+      tab[i] = sd[(size_t)(2 * op + half) * KS2 + kb];
+    }
+  }
+}
+
+// ------------------------------------------------------------------ the kernel, part 1: roles 0-3
+__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p);
+
+// Per-tile epilogue body for CT token columns per warp (defined below).
+template <int CT>
+__device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile& t, uint32_t tmem_base, uint32_t tfull0,
+                                                  uint32_t tempty0, int& acc_it, int& p1_it, float (*amax_s)[kTileRows], int q,
+                                                  int hf, int lane);
+
+__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 4 + 2 * kQueue];
+  __shared__ uint32_t tmem_base_s;
+  __shared__ int tq_slots[kQueue];
+  __shared__ float amax_s[3][kTileRows];   // per-token |h| maxima of a phase-1 tile (3 buffers in rotation)
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kMaxStages]);
+  const uint32_t tfull0 = smem_u32(&bars[2 * kMaxStages]), tempty0 = smem_u32(&bars[2 * kMaxStages + 2]);
+  const uint32_t qfull0 = smem_u32(&bars[2 * kMaxStages + 4]), qempty0 = smem_u32(&bars[2 * kMaxStages + 4 + kQueue]);
+  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < p.n_stages; ++s) {
+      mbar_init(full0 + 8 * s, 3);   // producer's expect_tx arrive + 2 loader warps
+      mbar_init(empty0 + 8 * s, 1);  // tcgen05.commit
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(tfull0 + 8 * a, 1);           // tcgen05.commit
+      mbar_init(tempty0 + 8 * a, kEpiWarps);  // one lane of each epilogue warp
+    }
+    for (int q = 0; q < kQueue; ++q) {
+      mbar_init(qfull0 + 8 * q, 1);               // producer
+      mbar_init(qempty0 + 8 * q, 3 + kEpiWarps);  // MMA warp + 2 loader warps + epilogue warps
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  for (int i = threadIdx.x; i < 3 * kTileRows; i += kThreads) (&amax_s[0][0])[i] = 0.f;
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
+                 "n"(kTmemCols));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+  TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
+  Tile t;
+
+  if (warp == 0) {
+    // ===== weight producer: claims tiles; one 32 KB bulk copy per 128-k stage from the packed image
+    if (lane == 0) {
+      int stage = 0, ph = 0, q = 0, qph = 0;
+      for (;;) {
+        mbar_wait(qempty0 + 8 * q, qph ^ 1);
+        const int i = atomicAdd(p.wl.sched + p.ticket, 1);
+        tq_slots[q] = i;
+        mbar_arrive(qfull0 + 8 * q);
+        if (++q == kQueue) { q = 0; qph ^= 1; }
+        if (!tm.at(i, t)) break;
+        const int e = p.wl.run_expert[t.run];
+        const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+        const uint8_t* src = p.packed[e] + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(empty0 + 8 * stage, ph ^ 1);
+          mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
+          bulk_g2s(smem_base + stage * p.stage_bytes, src + (size_t)kb * kAStageBytes, kAStageBytes, full0 + 8 * stage);
+          if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: every 128-k stage gets a fresh TMEM accumulator pair (block-scale promotion)
+    int stage = 0, ph = 0, acc_it = 0;
+    while (tm.at(tq.pop(), t)) {
+      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      if (lane == 0) {
+        const int npad = (p.wl.run_n[t.run] + 15) & ~15;
+        const uint32_t idesc = make_idesc(npad, false);   // e4m3 x e4m3 (format 0), fp32 accumulate
+        for (int kb = 0; kb < nkb; ++kb, ++acc_it) {
+          const int as = acc_it & 1;
+          mbar_wait(tempty0 + 8 * as, ((acc_it >> 1) & 1) ^ 1);
+          mbar_wait(full0 + 8 * stage, ph);
+          tc_fence_after();
+          const uint32_t d0 = tmem_base + as * 256, d1 = d0 + 128;
+          const uint32_t a_addr = smem_base + stage * p.stage_bytes;
+          const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes);
+          const uint64_t bh = make_desc(a_addr + kAStageBytes), bl = make_desc(a_addr + kAStageBytes + p.b_term_bytes);
+#pragma unroll
+          for (int ks = 0; ks < kKBlock / 32; ++ks) {     // +256 B per 32-element k-step (>> 4)
+            const uint64_t o = (uint64_t)(ks * 16);
+            umma_f8(d0, a0 + o, bh + o, idesc, ks ? 1u : 0u);
+            umma_f8(d0, a0 + o, bl + o, idesc, 1u);
+            umma_f8(d1, a1 + o, bh + o, idesc, ks ? 1u : 0u);
+            umma_f8(d1, a1 + o, bl + o, idesc, 1u);
+          }
+          tc_commit(empty0 + 8 * stage);
+          tc_commit(tfull0 + 8 * as);
+          if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+        }
+      } else {
+        stage = (stage + nkb) % p.n_stages;   // keep the ring position in step with lane 0
+        acc_it += nkb;
+      }
+      __syncwarp();
+    }
+  } else if (warp == 2 || warp == 3) {
+    // ===== token-operand loaders: gather the hi and lo e4m3 rows (x or h) into the canonical
+    // K-major layout with cp.async, a few stages in flight per warp
+    const int wq = warp - 2;
+    const int r8 = lane & 7, c4 = lane >> 3;  // row in 8-row group, 16-byte chunks c4 and c4 + 4
+    int stage = 0, ph = 0, pend_stage = 0, pending = 0;
+    const int lag = min(kLag, p.n_stages - 1);
+    auto publish = [&](int count) {
+      fence_proxy_async_smem();
+      __syncwarp();
+      for (int j = 0; j < count; ++j) {
+        if (lane == 0) mbar_arrive(full0 + 8 * pend_stage);
+        if (++pend_stage == p.n_stages) pend_stage = 0;
+      }
+      pending -= count;
+    };
+    while (tm.at(tq.pop(), t)) {
+      const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
+      const int ngroups = (n + 15) / 16 * 2;
+      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const uint8_t* rowh[8];   // this lane's hi source row in each of its groups (nullptr: zero fill)
+      size_t lo_off;            // lo row = hi row + lo_off
+      if (t.phase == 1) lo_off = (size_t)(p.xq_lo - p.xq_hi);
+      else lo_off = (size_t)(p.hq_lo - p.hq_hi);
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        const int row = (2 * g + wq) * 8 + r8;
+        rowh[g] = nullptr;
+        if (row < n) {
+          if (t.phase == 1) rowh[g] = p.xq_hi + (size_t)p.wl.ent_tok[start + row] * p.H;
+          else rowh[g] = p.hq_hi + (size_t)(p.wl.run_hrow[t.run] + row) * p.I;
+        }
+      }
+      if (t.phase == 2) {
+        if (lane == 0) {
+          const int* flag = p.wl.ready + t.run;
+          while (ld_acquire(flag) < p.P1) __nanosleep(64);
+        }
+        __syncwarp();
+      }
+      for (int kb = 0; kb < nkb; ++kb) {
+        mbar_wait(empty0 + 8 * stage, ph ^ 1);
+        const uint32_t b_addr = smem_base + stage * p.stage_bytes + kAStageBytes;
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          if (2 * g + wq < ngroups) {
+            const uint32_t a = b_addr + (2 * g + wq) * 1024 + r8 * 16;
+            const bool ok = rowh[g] != nullptr;
+            const uint8_t* src = ok ? rowh[g] + (size_t)kb * kKBlock + c4 * 16 : p.xq_hi;
+            const uint32_t sz = ok ? 16u : 0u;  // src-size 0: zero fill
+            const size_t lo = ok ? lo_off : 0, d64 = ok ? 64 : 0;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + c4 * 128), "l"(src), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + (c4 + 4) * 128), "l"(src + d64), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + p.b_term_bytes + c4 * 128), "l"(src + lo), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + p.b_term_bytes + (c4 + 4) * 128), "l"(src + lo + d64), "r"(sz) : "memory");
+          }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        ++pending;
+        if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+        if (pending > lag) {
+          if (lag >= 3) asm volatile("cp.async.wait_group 3;" ::: "memory");
+          else if (lag == 2) asm volatile("cp.async.wait_group 2;" ::: "memory");
+          else asm volatile("cp.async.wait_group 1;" ::: "memory");
+          publish(1);
+        }
+      }
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      publish(pending);
+    }
+  } else {
+    // ===== epilogue (warps 4-11): warp -> TMEM lane quadrant q = warp % 4, column half hf
+    const int q = warp & 3, hf = (warp - 4) >> 2;
+    int acc_it = 0, p1_it = 0;
+    while (tm.at(tq.pop(), t)) {
+      const int half_cols = ((p.wl.run_n[t.run] + 15) & ~15) >> 1;   // 8, 16, ..., 64
+      if (half_cols <= 8) fp8_epilogue_tile<8>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
+      else if (half_cols <= 16) fp8_epilogue_tile<16>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
+      else if (half_cols <= 32) fp8_epilogue_tile<32>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
+      else fp8_epilogue_tile<64>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
+  }
+}
+
+// ------------------------------------------------------------------ the kernel, part 2: epilogue of one tile
+// The warp owns TMEM lanes [32 q, 32 q + 32) (weight rows of the tile) and token columns
+// [hf CT, hf CT + CT).  Every 128-k block: wait for its accumulator pair, scale by
+// w_scale[half, kb] * a_scale[token, kb], add into fp32 registers, hand the buffer back.
+template <int CT>
+__device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile& t, uint32_t tmem_base, uint32_t tfull0,
+                                                  uint32_t tempty0, int& acc_it, int& p1_it, float (*amax_s)[kTileRows], int q,
+                                                  int hf, int lane) {
+  constexpr int NJ = CT > 32 ? 2 : 1;
+  const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run], hrow = p.wl.run_hrow[t.run];
+  const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+  const int col0 = hf * CT, row = q * 32 + lane;
+  const float* tab = reinterpret_cast<const float*>(p.packed[p.wl.run_expert[t.run]] + p.sc_off);
+  const float* wsc = t.phase == 1 ? tab + (size_t)t.sub * p.KB1 * 2 : tab + p.t2_off + (size_t)t.sub * p.KB2 * 2;
+  // activation scales: lane l fetches those of column col0 + l (+ 32), broadcast by shuffle below
+  const float* abase[NJ];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) {
+    const int cl = lane + 32 * j, col = col0 + cl;
+    abase[j] = nullptr;
+    if (cl < CT && col < n)
+      abase[j] = t.phase == 1 ? p.xs + (size_t)p.wl.ent_tok[start + col] * p.KB1 : p.hs + (size_t)(hrow + col) * p.KB2;
+  }
+  float acc0[CT], acc1[CT];
+#pragma unroll
+  for (int c = 0; c < CT; ++c) { acc0[c] = 0.f; acc1[c] = 0.f; }
+
+  // h and its scales come from other SMs (L2 loads) and exist only once the run's phase-1 tiles
+  // are done: the first completed accumulator proves it (the loaders waited for the run's
+  // counter), so the scales of block kb + 1 are fetched while block kb is being added.
+  float sv[NJ], sv_next[NJ];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) sv_next[j] = 0.f;
+  for (int kb = 0; kb < nkb; ++kb, ++acc_it) {
+    const int as = acc_it & 1;
+    const float w0 = __ldg(wsc + kb * 2), w1 = __ldg(wsc + kb * 2 + 1);
+    mbar_wait(tfull0 + 8 * as, (acc_it >> 1) & 1);
+    tc_fence_after();
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      sv[j] = kb == 0 ? (abase[j] ? __ldcg(abase[j]) : 0.f) : sv_next[j];
+      if (kb + 1 < nkb) sv_next[j] = abase[j] ? __ldcg(abase[j] + kb + 1) : 0.f;
+    }
+    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * 256 + col0;
+#pragma unroll
+    for (int c0 = 0; c0 < CT; c0 += 8) {
+      uint32_t d0[8], d1[8];
+      tmem_ld8(taddr + c0, d0);
+      tmem_ld8(taddr + 128 + c0, d1);
+      tmem_ld_wait();
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int c = c0 + j;
+        const float a = __shfl_sync(0xffffffffu, sv[c >> 5], c & 31);
+        acc0[c] = fmaf(__uint_as_float(d0[j]), w0 * a, acc0[c]);
+        acc1[c] = fmaf(__uint_as_float(d1[j]), w1 * a, acc1[c]);
+      }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+  }
+
+  if (t.phase == 1) {
+    // h = silu(gate) * up; per-token maximum over the tile's 128 features -> the (token, k block)
+    // scale of phase 2's activation operand; then the two e4m3 terms
+    const int buf = p1_it % 3;
+    unsigned* amax_u = reinterpret_cast<unsigned*>(amax_s[buf]);
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+      const float g = acc0[c], u = acc1[c];
+      const float hv = col0 + c < n ? g / (1.0f + __expf(-g)) * u : 0.f;
+      acc0[c] = hv;
+      float m = fabsf(hv);
+#pragma unroll
+      for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+      if (lane == 0 && col0 + c < n) atomicMax(amax_u + col0 + c, __float_as_uint(m));
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (lane < 16) amax_s[(p1_it + 2) % 3][(q + 4 * hf) * 16 + lane] = 0.f;   // the buffer of the tile after next
+    uint8_t* hi_base = p.hq_hi + (size_t)hrow * p.I + t.sub * kTileRows + row;
+    uint8_t* lo_base = p.hq_lo + (size_t)hrow * p.I + t.sub * kTileRows + row;
+#pragma unroll
+    for (int c = 0; c < CT; c += 2) {
+      const int col = col0 + c;
+      if (col < n) {
+        const float m0 = amax_s[buf][col], m1 = col + 1 < n ? amax_s[buf][col + 1] : 0.f;
+        const float s0 = m0 > 0.f ? m0 * (1.0f / 448.0f) : 1.0f, s1 = m1 > 0.f ? m1 * (1.0f / 448.0f) : 1.0f;
+        const float v0 = acc0[c] / s0, v1 = acc0[c + 1] / s1;
+        const uint16_t hi = cvt_e4m3x2(v0, v1);
+        const float2 hf2 = e4m3x2_to_float2(hi);
+        const uint16_t lo = cvt_e4m3x2(v0 - hf2.x, v1 - hf2.y);
+        hi_base[(size_t)col * p.I] = (uint8_t)(hi & 0xff);
+        lo_base[(size_t)col * p.I] = (uint8_t)(lo & 0xff);
+        if (row == 0) p.hs[(size_t)(hrow + col) * p.KB2 + t.sub] = s0;
+        if (col + 1 < n) {
+          hi_base[(size_t)(col + 1) * p.I] = (uint8_t)(hi >> 8);
+          lo_base[(size_t)(col + 1) * p.I] = (uint8_t)(lo >> 8);
+          if (row == 0) p.hs[(size_t)(hrow + col + 1) * p.KB2 + t.sub] = s1;
+        }
+      }
+    }
+    ++p1_it;
+    // publish this tile's slice of h: all 256 epilogue threads' stores, then one release add
+    __threadfence();
+    asm volatile("bar.sync 2, 256;" ::: "memory");
+    if (threadIdx.x == 128) atomicAdd(p.wl.ready + t.run, 1);
+  } else {
+    float* ocol = p.obuf + t.sub * 2 * kTileRows + row;
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+      const int col = col0 + c;
+      if (col < n) {
+        float* o = ocol + (size_t)p.wl.ent_dst[start + col] * p.H;
+        o[0] = acc0[c];
+        o[kTileRows] = acc1[c];
+      }
+    }
+  }
+}
+
+size_t table_floats(const caee_ctx* c) {
+  const int P1 = c->d.I / kTileRows, P2 = c->d.H / (2 * kTileRows), KS1 = c->d.H / kKBlock, KS2 = c->d.I / kKBlock;
+  return (size_t)P1 * KS1 * 2 + (size_t)P2 * KS2 * 2;
+}
+
+}  // namespace
+
+caee_status caee_fp8_supported(const caee_ctx* c, std::string* why) {
+  const caee_layer_desc& d = c->d;
+  if (d.H % 256 || d.I % 128) {
+    *why = "the e4m3 UMMA expert kernel needs H % 256 == 0 and I % 128 == 0";
+    return CAEE_ESHAPE;
+  }
+  return CAEE_OK;
+}
+
+size_t caee_fp8_packed_bytes(const caee_ctx* c) {
+  return (size_t)3 * c->d.H * c->d.I + ((table_floats(c) * 4 + 15) & ~(size_t)15);
+}
+
+void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst, const void* g, const void* u, const void* dn, const float* sg,
+                                 const float* su, const float* sd, cudaStream_t st) {
+  const int H = c->d.H, I = c->d.I;
+  const size_t n1 = (size_t)I * (H / 16), n2 = (size_t)H * (I / 16);
+  const size_t p2_off = (size_t)2 * I * H;
+  k_pack_e4m3<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>((const uint8_t*)g, dst, I, H, 0, 0);
+  k_pack_e4m3<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>((const uint8_t*)u, dst, I, H, 1, 0);
+  k_pack_e4m3<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>((const uint8_t*)dn, dst, H, I, 2, p2_off);
+  const int P1 = I / kTileRows, P2 = H / (2 * kTileRows);
+  k_scale_table<<<16, 256, 0, st>>>(sg, su, sd, reinterpret_cast<float*>(dst + (size_t)3 * H * I), P1, P2, H / kKBlock, I / kKBlock);
+}
+
+// Once per step, before the first expert launch: x -> its two e4m3 terms and block scales.
+void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
+  if (T <= 0) return;
+  const size_t n_blocks = (size_t)T * (c->d.H / kKBlock);
+  const size_t TH = (size_t)c->d.max_tokens * c->d.H;
+  k_act_split<<<(unsigned)((n_blocks + 7) / 8), 256, 0, st>>>((const __nv_bfloat16*)x, c->xq, c->xq + TH, c->xs, n_blocks);
+}
+
+// runs [run_begin, run_begin + run_count) (run_count < 0: every run of the work list), tile
+// tickets from wl.sched[ticket].
+void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
+  const caee_layer_desc& d = c->d;
+  Fp8Params p;
+  p.wl = c->wl;
+  p.packed = c->packed.dev_ptrs;
+  const size_t TH = (size_t)d.max_tokens * d.H, RI = c->h_rows_cap * (size_t)d.I;
+  p.xq_hi = c->xq; p.xq_lo = c->xq + TH; p.xs = c->xs;
+  p.hq_hi = c->hq; p.hq_lo = c->hq + RI; p.hs = c->hs;
+  p.obuf = c->obuf;
+  p.H = d.H; p.I = d.I;
+  p.P1 = d.I / kTileRows; p.P2 = d.H / (2 * kTileRows);
+  p.KB1 = d.H / kKBlock; p.KB2 = d.I / kKBlock;
+  p.run_begin = run_begin; p.run_count = run_count; p.ticket = ticket;
+  p.sc_off = (int)((size_t)3 * d.H * d.I);
+  p.t2_off = p.P1 * p.KB1 * 2;
+  const int ncap = std::min(CAEE_RUN_TOKENS, (T + 15) & ~15);
+  p.b_term_bytes = ncap * kKBlock;                  // one e4m3 term of the token operand
+  p.stage_bytes = kAStageBytes + 2 * p.b_term_bytes;
+  const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers / amax buffers
+  p.n_stages = std::min(kMaxStages, (max_dyn - 1024) / p.stage_bytes);
+  const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_expert_fp8, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
+    attr_set = true;
+  }
+  k_expert_fp8<<<c->num_sms, kThreads, dyn, st>>>(p);
+}

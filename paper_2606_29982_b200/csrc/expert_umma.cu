@@ -569,23 +569,24 @@ caee_status caee_umma_supported(const caee_ctx* c, std::string* why) {
     *why = "the UMMA expert kernel needs H % 256 == 0 and I % 128 == 0";
     return CAEE_ESHAPE;
   }
-  if (d.w_dtype == CAEE_E4M3 && (d.H / 128 * 2 > kMaxRatio || d.I / 128 * 2 > kMaxRatio)) {
-    *why = "the e4m3 UMMA expert kernel needs H, I <= 16384";
-    return CAEE_ESHAPE;
-  }
+  if (d.w_dtype == CAEE_E4M3) return caee_fp8_supported(c, why);
   return CAEE_OK;
 }
 
 size_t caee_umma_packed_bytes(const caee_ctx* c) {
   const size_t elems = (size_t)3 * c->d.H * c->d.I;
   if (c->d.w_dtype == CAEE_BF16) return elems * 2;
-  return elems + ((table_floats(c) * 4 + 15) & ~(size_t)15);
+  return caee_fp8_packed_bytes(c);
 }
 
 void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst, const void* g, const void* u, const void* dn, const float* sg,
                              const float* su, const float* sd, cudaStream_t st) {
   (void)e;
   const int H = c->d.H, I = c->d.I;
+  if (c->d.w_dtype == CAEE_E4M3) {
+    caee_launch_pack_expert_fp8(c, dst, g, u, dn, sg, su, sd, st);
+    return;
+  }
   if (c->d.w_dtype == CAEE_BF16) {
     const size_t n1 = (size_t)I * (H / 8), n2 = (size_t)H * (I / 8);
     const size_t p2_off = (size_t)2 * I * H * 2;
@@ -606,6 +607,8 @@ void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst, const void* g, co
 // Once per step, before the first expert launch: the fp16 copy of x the e4m3 path contracts with.
 void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (c->d.w_dtype != CAEE_E4M3 || T <= 0) return;
+  caee_launch_fp8_prepare(c, x, T, st);
+  return;
   const size_t n = (size_t)T * c->d.H;
   k_bf16_to_f16<<<(unsigned)((n / 2 + 256) / 256), 256, 0, st>>>((const __nv_bfloat16*)x, c->x16, n);
 }
@@ -615,6 +618,10 @@ void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st
 void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   const bool fp8 = d.w_dtype == CAEE_E4M3;
+  if (fp8) {
+    caee_launch_expert_fp8(c, T, run_begin, run_count, ticket, st);
+    return;
+  }
   UmmaParams p;
   p.wl = c->wl;
   p.packed = c->packed.dev_ptrs;

@@ -1,0 +1,133 @@
+// umma_common.cuh — PTX wrappers (mbarrier, bulk async copy, tcgen05 MMA / TMEM load,
+// shared-memory operand and instruction descriptors) and the dynamic tile schedule shared by
+// the bf16 and e4m3 expert kernels (expert_umma.cu, expert_fp8.cu).  sm_100a only.
+#pragma once
+#include "caee_internal.cuh"
+
+namespace caee_umma {
+
+constexpr int kTileRows = 128;          // UMMA M
+constexpr int kATileBytes = 16 * 1024;  // one 128-row weight tile of a stage (64 k bf16 or 128 k e4m3)
+constexpr int kAStageBytes = 2 * kATileBytes;  // two tiles per stage: ONE contiguous 32 KB bulk copy
+constexpr int kTmemCols = 512;
+constexpr int kMaxStages = 8;
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, kind::f16 (bf16 inputs, fp32 accumulate), M=128, K=16
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, kind::f8f6f4 (e4m3 x e4m3, fp32 accumulate), M=128, K=32
+__device__ __forceinline__ void umma_f8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, no-swizzle shared-memory operand descriptor: start address, LBO (k-adjacent core
+// matrices) = 128 B, SBO (adjacent 8-row groups) = 1024 B, descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46);
+}
+// kind::f16 instruction descriptor: D fp32, A/B bf16 (format 1) or fp16 (format 0), both K-major,
+// M = 128, N = n.
+__device__ __forceinline__ uint32_t make_idesc(int n, bool bf16) {
+  return (1u << 4) | (bf16 ? ((1u << 7) | (1u << 10)) : 0u) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)(kTileRows >> 4) << 24);
+}
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+struct Tile {
+  int phase, run, sub;  // sub = ft (phase 1) or op (phase 2)
+};
+struct TileMap {
+  int n_runs, run_begin, P1, P2;
+  __device__ __forceinline__ bool at(int i, Tile& t) const {
+    const int t1 = n_runs * P1;
+    if (i < t1) { const int r = i / P1; t.phase = 1; t.sub = i - r * P1; t.run = run_begin + r; return true; }
+    i -= t1;
+    if (i < n_runs * P2) { const int r = i / P2; t.phase = 2; t.sub = i - r * P2; t.run = run_begin + r; return true; }
+    return false;
+  }
+};
+
+// ------------------------------------------------------------------ the kernel
+constexpr int kQueue = 4;      // tile-queue depth (producer runs at most this many tiles ahead)
+constexpr int kLag = 3;        // token-operand stages each loader warp keeps in flight (cp.async groups), < ring depth
+
+// Next tile index for a role.  The weight producer claims tiles with one atomic ticket per
+// tile and broadcasts them through a small shared-memory queue; every other role pops the
+// same sequence.  Tickets are claimed in increasing order, phase-1 tiles have the lower
+// tickets, and a phase-1 tile never waits on another tile: a phase-2 tile's wait for its
+// run's h therefore always ends (the CTAs holding those phase-1 tickets are running).
+struct TileQueue {
+  uint32_t full0, empty0;  // mbarrier addresses
+  int* slots;
+  int q, ph;
+  __device__ __forceinline__ int pop() {
+    mbar_wait(full0 + 8 * q, ph);
+    const int t = slots[q];
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(empty0 + 8 * q);
+    if (++q == kQueue) { q = 0; ph ^= 1; }
+    return t;
+  }
+};
+
+
+}  // namespace caee_umma
