@@ -154,7 +154,9 @@ caee_status create_impl(caee_ctx* c) {
   A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
   A(c->partial, prow * E); A(c->logits, Tm * E); A(c->tile_ctr, ntile); A(c->decide_scratch, caee_decide_scratch_bytes(c)); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
   A(c->act, E); A(c->must, E); A(c->keep, E); A(c->I_fix, E); A(c->load, CAEE_MAX_D); A(c->scalars, 8);
-  c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS + S * ((Tm + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS));
+  c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS_MIN - 1) / CAEE_RUN_TOKENS_MIN +
+                         S * ((Tm + CAEE_RUN_TOKENS_MIN - 1) / CAEE_RUN_TOKENS_MIN));
+  c->wl.run_cap = CAEE_RUN_TOKENS;
   A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
   A(c->wl.ent_tok, Tm * (k + S)); A(c->wl.ent_slot, Tm * k); A(c->wl.ent_wt, Tm * k); A(c->wl.ent_dst, Tm * (k + S));
   A(c->wl.run_expert, c->wl.max_runs); A(c->wl.run_start, c->wl.max_runs); A(c->wl.run_n, c->wl.max_runs);
@@ -457,6 +459,7 @@ caee_status caee_prune(caee_ctx* c, const caee_prune_params* p, const float* sco
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
   caee_prune_params none = {CAEE_PRUNE_NONE, 0, 0.0};
+  c->wl.run_cap = CAEE_RUN_TOKENS;
   rc = enqueue_decisions(c, nullptr, scores, T, p ? p : &none, idx, gate, nullptr, false, st);
   if (rc != CAEE_OK) return rc;
   caee_launch_export_worklist(c, T, out, st);
@@ -484,6 +487,9 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
+  // e4m3 decode steps use 64-token runs: the token operand (two e4m3 terms) then leaves room for
+  // a deeper weight ring, and hi/lo share one MMA (expert_fp8.cu); prefill keeps 128 for weight reuse
+  c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
   const bool fused = caee_decide_fits(c, T);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)

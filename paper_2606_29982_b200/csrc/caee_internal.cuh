@@ -15,7 +15,8 @@
 #define CAEE_FIX_ONE_F 1099511627776.0f /* 2^40: fixed-point unit of I(e) */
 #define CAEE_MAX_E 512
 #define CAEE_MAX_D 64
-#define CAEE_RUN_TOKENS 128 /* tokens per run: one UMMA N tile */
+#define CAEE_RUN_TOKENS 128 /* most tokens per run: one UMMA N tile */
+#define CAEE_RUN_TOKENS_MIN 64
 #define CAEE_DECIDE_MAX_TOKENS 256 /* largest step the one-kernel decision path takes (decide.cu) */
 
 // One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
@@ -39,6 +40,7 @@ struct caee_worklist {
   int32_t* sched;       // [n_tickets + max_runs]: tile-ticket counters (one per expert-kernel launch of a step),
   int32_t* ready;       //   then (= sched + n_tickets) per-run "h complete" counters; zeroed every step
   int32_t max_runs, n_tickets;
+  int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, or 64 (e4m3 decode steps)
 };
 
 struct caee_packed {

@@ -209,39 +209,55 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: every 128-k stage gets a fresh TMEM accumulator pair (block-scale promotion)
+    // ===== MMA issuer: every 128-k stage gets a fresh TMEM accumulator pair (block-scale promotion).
+    // The whole warp runs the loop (uniform control flow); one elected lane issues.
     int stage = 0, ph = 0, acc_it = 0;
     while (tm.at(tq.pop(), t)) {
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-      if (lane == 0) {
-        const int npad = (p.wl.run_n[t.run] + 15) & ~15;
-        const uint32_t idesc = make_idesc(npad, false);   // e4m3 x e4m3 (format 0), fp32 accumulate
-        for (int kb = 0; kb < nkb; ++kb, ++acc_it) {
-          const int as = acc_it & 1;
-          mbar_wait(tempty0 + 8 * as, ((acc_it >> 1) & 1) ^ 1);
-          mbar_wait(full0 + 8 * stage, ph);
-          tc_fence_after();
-          const uint32_t d0 = tmem_base + as * 256, d1 = d0 + 128;
-          const uint32_t a_addr = smem_base + stage * p.stage_bytes;
-          const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes);
-          const uint64_t bh = make_desc(a_addr + kAStageBytes), bl = make_desc(a_addr + kAStageBytes + p.b_term_bytes);
+      const int npad = (__shfl_sync(0xffffffffu, p.wl.run_n[t.run], 0) + 15) & ~15;
+      // up to 64 tokens the lo rows follow the hi rows and ONE MMA of N = 2 npad takes both terms
+      // (hi and lo partial sums in separate columns, added by the epilogue): the weight tile is
+      // read from shared memory once per k-step.  Wider runs add both terms into the same columns.
+      const bool cat = npad <= 64;
+      const uint32_t idesc = make_idesc(cat ? 2 * npad : npad, false);   // e4m3 x e4m3 (format 0), fp32 accumulate
+      for (int kb = 0; kb < nkb; ++kb, ++acc_it) {
+        const int as = acc_it & 1;
+        mbar_wait(tempty0 + 8 * as, ((acc_it >> 1) & 1) ^ 1);
+        mbar_wait(full0 + 8 * stage, ph);
+        tc_fence_after();
+        const uint32_t d0 = tmem_base + as * 256, d1 = d0 + 128;
+        const uint32_t a_addr = smem_base + stage * p.stage_bytes;
+        const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes);
+        const uint64_t bh = make_desc(a_addr + kAStageBytes), bl = make_desc(a_addr + kAStageBytes + p.b_term_bytes);
+        if (elect_one()) {
+          if (cat) {
+            umma_f8_imm<false>(d0, a0, bh, idesc);
+            umma_f8_imm<false>(d1, a1, bh, idesc);
 #pragma unroll
-          for (int ks = 0; ks < kKBlock / 32; ++ks) {     // +256 B per 32-element k-step (>> 4)
-            const uint64_t o = (uint64_t)(ks * 16);
-            umma_f8(d0, a0 + o, bh + o, idesc, ks ? 1u : 0u);
-            umma_f8(d0, a0 + o, bl + o, idesc, 1u);
-            umma_f8(d1, a1 + o, bh + o, idesc, ks ? 1u : 0u);
-            umma_f8(d1, a1 + o, bl + o, idesc, 1u);
+            for (int ks = 1; ks < kKBlock / 32; ++ks) {     // +256 B per 32-element k-step (>> 4)
+              umma_f8_imm<true>(d0, a0 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 16), idesc);
+              umma_f8_imm<true>(d1, a1 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 16), idesc);
+            }
+          } else {
+            umma_f8_imm<false>(d0, a0, bh, idesc);
+            umma_f8_imm<true>(d0, a0, bl, idesc);
+            umma_f8_imm<false>(d1, a1, bh, idesc);
+            umma_f8_imm<true>(d1, a1, bl, idesc);
+#pragma unroll
+            for (int ks = 1; ks < kKBlock / 32; ++ks) {
+              const uint64_t o = (uint64_t)(ks * 16);
+              umma_f8_imm<true>(d0, a0 + o, bh + o, idesc);
+              umma_f8_imm<true>(d0, a0 + o, bl + o, idesc);
+              umma_f8_imm<true>(d1, a1 + o, bh + o, idesc);
+              umma_f8_imm<true>(d1, a1 + o, bl + o, idesc);
+            }
           }
           tc_commit(empty0 + 8 * stage);
           tc_commit(tfull0 + 8 * as);
-          if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
         }
-      } else {
-        stage = (stage + nkb) % p.n_stages;   // keep the ring position in step with lane 0
-        acc_it += nkb;
+        __syncwarp();
+        if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
       }
-      __syncwarp();
     }
   } else if (warp == 2 || warp == 3) {
     // ===== token-operand loaders: gather the hi and lo e4m3 rows (x or h) into the canonical
@@ -263,6 +279,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       const int ngroups = (n + 15) / 16 * 2;
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const uint32_t lo_smem = ngroups <= 8 ? (uint32_t)ngroups * 1024u : (uint32_t)p.b_term_bytes;   // see the MMA warp
       const uint8_t* rowh[8];   // this lane's hi source row in each of its groups (nullptr: zero fill)
       size_t lo_off;            // lo row = hi row + lo_off
       if (t.phase == 1) lo_off = (size_t)(p.xq_lo - p.xq_hi);
@@ -296,8 +313,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
             const size_t lo = ok ? lo_off : 0, d64 = ok ? 64 : 0;
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + c4 * 128), "l"(src), "r"(sz) : "memory");
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + (c4 + 4) * 128), "l"(src + d64), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + p.b_term_bytes + c4 * 128), "l"(src + lo), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + p.b_term_bytes + (c4 + 4) * 128), "l"(src + lo + d64), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + lo_smem + c4 * 128), "l"(src + lo), "r"(sz) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + lo_smem + (c4 + 4) * 128), "l"(src + lo + d64), "r"(sz) : "memory");
           }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
@@ -345,6 +362,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
   constexpr int NJ = CT > 32 ? 2 : 1;
   const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run], hrow = p.wl.run_hrow[t.run];
   const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+  const int npad = (n + 15) & ~15;
   const int col0 = hf * CT, row = q * 32 + lane;
   const float* tab = reinterpret_cast<const float*>(p.packed[p.wl.run_expert[t.run]] + p.sc_off);
   const float* wsc = t.phase == 1 ? tab + (size_t)t.sub * p.KB1 * 2 : tab + p.t2_off + (size_t)t.sub * p.KB2 * 2;
@@ -383,7 +401,19 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
       uint32_t d0[8], d1[8];
       tmem_ld8(taddr + c0, d0);
       tmem_ld8(taddr + 128 + c0, d1);
-      tmem_ld_wait();
+      if (CT <= 32) {   // hi and lo partial sums sit npad columns apart
+        uint32_t e0[8], e1[8];
+        tmem_ld8(taddr + npad + c0, e0);
+        tmem_ld8(taddr + 128 + npad + c0, e1);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          d0[j] = __float_as_uint(__uint_as_float(d0[j]) + __uint_as_float(e0[j]));
+          d1[j] = __float_as_uint(__uint_as_float(d1[j]) + __uint_as_float(e1[j]));
+        }
+      } else {
+        tmem_ld_wait();
+      }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int c = c0 + j;
@@ -512,7 +542,7 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
   p.run_begin = run_begin; p.run_count = run_count; p.ticket = ticket;
   p.sc_off = (int)((size_t)3 * d.H * d.I);
   p.t2_off = p.P1 * p.KB1 * 2;
-  const int ncap = std::min(CAEE_RUN_TOKENS, (T + 15) & ~15);
+  const int ncap = std::min((int)c->wl.run_cap, (T + 15) & ~15);
   p.b_term_bytes = ncap * kKBlock;                  // one e4m3 term of the token operand
   p.stage_bytes = kAStageBytes + 2 * p.b_term_bytes;
   const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers / amax buffers

@@ -84,19 +84,19 @@ __device__ __forceinline__ void caee_block_excl_scan(const int (&v)[N], int (&ex
 __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int count_e, int32_t* estart,
                                                    const uint8_t* __restrict__ resident, int T, int E, int S, int k, bool write,
                                                    int* scratch /* 33 * 6 ints */) {
-  const int e = threadIdx.x;
+  const int e = threadIdx.x, cap = wl.run_cap;   // tokens per run (a multiple of 16)
   const int c = e < E ? count_e : 0;
   const bool res = e < E && resident[e] != 0;
-  const int nch = (c + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS, rows = (c + 15) & ~15;
+  const int nch = (c + cap - 1) / cap, rows = (c + 15) & ~15;
   const int v[6] = {c > 0, c, res ? nch : 0, res ? rows : 0, res ? 0 : nch, res ? 0 : rows};
   int ex[6], tot[6];
   caee_block_excl_scan<6>(v, ex, tot, scratch);
   if (e < E) estart[e] = ex[1];
   if (!write) return;
-  const int sh_chunks = T > 0 ? (T + CAEE_RUN_TOKENS - 1) / CAEE_RUN_TOKENS : 0;
+  const int sh_chunks = T > 0 ? (T + cap - 1) / cap : 0;
   const int sh_runs = S * sh_chunks;
   int sh_rows_each = 0;   // h rows of one shared expert: every chunk padded to 16
-  for (int t0 = 0; t0 < T; t0 += CAEE_RUN_TOKENS) sh_rows_each += (min(CAEE_RUN_TOKENS, T - t0) + 15) & ~15;
+  for (int t0 = 0; t0 < T; t0 += cap) sh_rows_each += (min(cap, T - t0) + 15) & ~15;
   if (c > 0) {
     wl.expert_ids[ex[0]] = e;
     wl.offs[ex[0]] = ex[1];
@@ -104,18 +104,18 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
     const int h0 = res ? ex[3] : tot[3] + S * sh_rows_each + ex[5];
     for (int j = 0; j < nch; ++j) {
       wl.run_expert[r0 + j] = e;
-      wl.run_start[r0 + j] = ex[1] + j * CAEE_RUN_TOKENS;
-      wl.run_n[r0 + j] = min(CAEE_RUN_TOKENS, c - j * CAEE_RUN_TOKENS);
-      wl.run_hrow[r0 + j] = h0 + j * CAEE_RUN_TOKENS;
+      wl.run_start[r0 + j] = ex[1] + j * cap;
+      wl.run_n[r0 + j] = min(cap, c - j * cap);
+      wl.run_hrow[r0 + j] = h0 + j * cap;
     }
   }
   for (int i = e; i < sh_runs; i += blockDim.x) {   // shared-expert runs over all tokens
-    const int s = i / sh_chunks, j = i - s * sh_chunks, t0 = j * CAEE_RUN_TOKENS;
+    const int s = i / sh_chunks, j = i - s * sh_chunks, t0 = j * cap;
     const int r = tot[2] + i;
     wl.run_expert[r] = E + s;
     wl.run_start[r] = T * k + s * T + t0;
-    wl.run_n[r] = min(CAEE_RUN_TOKENS, T - t0);
-    wl.run_hrow[r] = tot[3] + s * sh_rows_each + j * CAEE_RUN_TOKENS;
+    wl.run_n[r] = min(cap, T - t0);
+    wl.run_hrow[r] = tot[3] + s * sh_rows_each + j * cap;
   }
   if (e == 0) {
     wl.offs[tot[0]] = tot[1];
