@@ -167,6 +167,20 @@ def run_reference(args, cfg, prune):
         "gpu_launches": 0}))
 
 
+def job_throughput(ms_local, tokens_local, world, device):
+    """Whole-job tokens/s of N independent replicas: every rank's tokens over the
+    slowest rank's time.  The only collective of the whole program is this timing reduction."""
+    if world == 1:
+        return tokens_local / (ms_local * 1e-3), ms_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    n = torch.tensor([float(tokens_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(n.item()) / (float(t.item()) * 1e-3), float(t.item())
+
+
 # --------------------------------------------------------------------------- the CUDA arm
 def run_caee(args, cfg, prune):
     import torch
@@ -204,11 +218,7 @@ def run_caee(args, cfg, prune):
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return job_throughput(ms, T * steps, world, dev)[1]      # max over ranks
 
     step = lambda i: L.forward(xs[i % len(xs)], params, y=y, stats=stats)
     for i in range(W):
