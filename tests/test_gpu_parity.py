@@ -367,3 +367,37 @@ def test_forward_c4_full_size_sampled(H, T, mode):
         print(f"C4 T={T} {mode}: max|err|/RMS = {r:.3e}")
     finally:
         L.close()
+
+
+def test_forward_is_cuda_graph_capturable(H):
+    """The per-step calls only enqueue (include/caee.h): a decode step — router GEMM, the cooperative
+    decision kernel, the expert kernel, the combine — can be captured once and replayed; the replay
+    on new inputs matches a direct call bit for bit."""
+    from paper_2606_29982_b200 import binding as B
+    from paper_2606_29982_b200.layer import Layer
+    L = Layer(R1S, seed=0, max_tokens=64)
+    try:
+        T = 48
+        params = B.prune_params(B.CAEE_PRUNE_CIR, 0.8)
+        x = wl.hidden(R1S, T, 31, L.device)
+        y = torch.empty_like(x)
+        stats = B.stats_buffer(L.device)
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            L.forward(x, params, y=y, stats=stats, stream=side)      # warm-up outside capture
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            L.forward(x, params, y=y, stats=stats, stream=torch.cuda.current_stream())
+        for seed in (32, 33):
+            x.copy_(wl.hidden(R1S, T, seed, L.device))
+            g.replay()
+            torch.cuda.synchronize()
+            y_graph, n_run_graph = y.clone(), B.read_stats(stats).n_run
+            y_direct = L.forward(x, params, stats=stats)
+            torch.cuda.synchronize()
+            assert torch.isfinite(y_graph.float()).all() and y_graph.float().abs().max() > 0
+            assert torch.equal(y_graph, y_direct)
+            assert n_run_graph == B.read_stats(stats).n_run
+    finally:
+        L.close()
