@@ -296,7 +296,7 @@ def test_forward_small_fp8(H, kernel):
     from paper_2606_29982_b200 import binding as B
     L = _layer(H, C4S, max_tokens=300, kernel=B.CAEE_KERNEL_SIMT if kernel == "simt" else B.CAEE_KERNEL_UMMA)
     try:
-        for T, mode in ((1, "dense"), (8, "frac"), (32, "cir"), (128, "frac"), (300, "dense"), (19, "rank")):
+        for T, mode in ((1, "dense"), (8, "frac"), (32, "cir"), (128, "frac"), (200, "thresh"), (300, "dense"), (19, "rank")):
             r = _forward_case(H, L, T, mode)
             print(f"fp8 {kernel} T={T} {mode}: max|err|/RMS = {r:.3e}")
     finally:
@@ -365,6 +365,18 @@ def test_forward_c4_full_size_sampled(H, T, mode):
         toks = sorted(set([0, T // 3, T - 1]))
         r = _forward_case(H, L, T, mode, tokens=toks, seed=100)
         print(f"C4 T={T} {mode}: max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
+
+
+def test_forward_c4_prefill_4096_sampled(H):
+    """Config 4's 4096-token prefill batch (stand-alone decision kernels, 128-token runs, the wide
+    epilogue of the e4m3 kernel): K_final and F_* for all 4096 tokens bit-exact, y on sampled tokens."""
+    L = H.GpuLayer(wl.C4, seed=0, max_tokens=4096, keep_raw=False)
+    try:
+        T = 4096
+        r = _forward_case(H, L, T, "frac", tokens=[0, 1365, T - 1], seed=100)
+        print(f"C4 T={T} frac: max|err|/RMS = {r:.3e}")
     finally:
         L.close()
 
