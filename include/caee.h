@@ -174,8 +174,10 @@ caee_status caee_set_router(caee_ctx* ctx, const float* W_r, const float* b_logi
  * the same size for non-resident ones) and no longer refers to the caller's buffers
  * afterwards.  The UMMA kernel (bf16 or e4m3 weights with bf16 activations) requires
  * pack != 0; the SIMT kernel reads the caller's buffers in place and needs every expert in
- * device memory.  The e4m3 UMMA kernel contracts in fp16 (fp32 accumulate): |x| and the
- * SwiGLU intermediate must stay below 65504.
+ * device memory.  The e4m3 UMMA kernel feeds the e4m3 codes to the tensor cores as they are and
+ * carries each activation (x and the SwiGLU intermediate) as two e4m3 terms with one fp32 scale per
+ * (token, 128-wide block): about 2^-8 relative error per activation, fp32 accumulation, the
+ * 128x128 weight block scales applied in fp32.
  * Call caee_set_residency first when some experts live in host memory (changing the
  * residency afterwards invalidates the weights: set them again). */
 caee_status caee_set_weights(caee_ctx* ctx, const caee_expert_weights* w, int32_t pack);

@@ -101,7 +101,6 @@ struct caee_ctx {
   caee_worklist wl;
   float* hbuf_f32 = nullptr;         // SIMT: h rows [rows, I] fp32
   __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16 (bf16 weights) / fp16 (e4m3 weights)
-  __half* x16 = nullptr;             // (unused)
   uint8_t* xq = nullptr;             // UMMA e4m3: hi | lo e4m3 terms of x, [Tmax, H] each
   float* xs = nullptr;               //   and its (token, 128-block) scales [Tmax, H/128]
   uint8_t* hq = nullptr;             // UMMA e4m3: hi | lo terms of h, [rows, I] each
