@@ -169,6 +169,7 @@ caee_status create_impl(caee_ctx* c) {
   if (c->kernel == CAEE_KERNEL_UMMA && d.w_dtype == CAEE_E4M3) {
     A(c->xq, 2 * Tm * d.H); A(c->xs, Tm * (d.H / 128));
     A(c->hq, 2 * c->h_rows_cap * d.I); A(c->hs, c->h_rows_cap * (d.I / 128));
+    if ((rc = caee_fp8_make_tensor_maps(c)) != CAEE_OK) return rc;
   }
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A

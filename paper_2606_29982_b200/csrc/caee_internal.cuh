@@ -105,6 +105,8 @@ struct caee_ctx {
   float* xs = nullptr;               //   and its (token, 128-block) scales [Tmax, H/128]
   uint8_t* hq = nullptr;             // UMMA e4m3: hi | lo terms of h, [rows, I] each
   float* hs = nullptr;               //   and its scales [rows, I/128]
+  alignas(64) unsigned char tm_x[128] = {0}, tm_h[128] = {0};  // CUtensorMap of xq / hq (row gathers), see expert_fp8.cu
+  bool tm_ready = false;
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
@@ -167,6 +169,7 @@ size_t caee_fp8_packed_bytes(const caee_ctx* c);
 void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst_dev, const void* g, const void* u, const void* d, const float* sg,
                                  const float* su, const float* sd, cudaStream_t s);
 void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
+caee_status caee_fp8_make_tensor_maps(caee_ctx* c);
 void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);

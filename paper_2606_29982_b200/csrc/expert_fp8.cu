@@ -24,9 +24,13 @@
 // down rows [+0..127 | +128..255]; then the fp32 block-scale table, [tile][kb][half].
 //
 // Roles (384 threads, 1 CTA per SM): warp 0 = weight producer (bulk copies), warp 1 = MMA
-// issuer, warps 2-3 = token-operand loaders (cp.async gathers of the hi/lo rows), warps 4-11 =
+// issuer, warp 2 = token-operand loader (TMA row gathers of the hi/lo rows), warps 4-11 =
 // epilogue (two warps per TMEM lane quadrant, each half of the token columns).  Tiles are
 // claimed by atomic ticket, phase-1 tickets first (see umma_common.cuh).
+#include <cuda.h>
+
+#include <cstring>
+
 #include "umma_common.cuh"
 
 namespace {
@@ -53,7 +57,27 @@ struct Fp8Params {
   int run_begin, run_count, ticket;
   int sc_off;               // byte offset of the scale table in a packed image
   int t2_off;               // float offset of its phase-2 part
+  // token operand by TMA row gather (tile::gather4, 128 B rows, 128 B swizzle): 2D maps over the
+  // [hi rows | lo rows] x k byte arrays of x and of h; lo row = hi row + lo_row_*
+  CUtensorMap tm_x, tm_h;
+  int lo_row_x, lo_row_h;
 };
+
+constexpr int kOobRow = 0x40000000;   // beyond any tensor: the TMA unit writes zeros (padding rows)
+
+// Four rows of 128 bytes (k bytes [col, col + 128) of rows r0..r3) -> 512 bytes at dst, swizzled
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int col, int r0, int r1, int r2,
+                                            int r3) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(dst), "l"(tm), "r"(bar), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
+}
+// K-major operand descriptor for the 128-byte-swizzled token operand: 8-row atoms of 1024 B (SBO),
+// layout type 2 (SWIZZLE_128B), descriptor version 1; a 32-byte k-step advances the start address.
+__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
 
 // two floats -> two e4m3 codes (low byte = a), round to nearest even, saturating
 __device__ __forceinline__ uint16_t cvt_e4m3x2(float a, float b) {
@@ -135,7 +159,7 @@ __global__ void k_scale_table(const float* __restrict__ sg, const float* __restr
 }
 
 // ------------------------------------------------------------------ the kernel, part 1: roles 0-3
-__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p);
+__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constant__ Fp8Params p);
 
 // Per-tile epilogue body for CT token columns per warp (defined below).
 template <int CT>
@@ -143,7 +167,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
                                                   uint32_t tempty0, int& acc_it, int& p1_it, float (*amax_s)[kTileRows], int q,
                                                   int hf, int lane);
 
-__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
+__global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constant__ Fp8Params p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 4 + 2 * kQueue];
@@ -160,7 +184,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < p.n_stages; ++s) {
-      mbar_init(full0 + 8 * s, 3);   // producer's expect_tx arrive + 2 loader warps
+      mbar_init(full0 + 8 * s, 2);   // expect_tx arrives of the weight producer and of the token-operand loader
       mbar_init(empty0 + 8 * s, 1);  // tcgen05.commit
     }
     for (int a = 0; a < 2; ++a) {
@@ -169,7 +193,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
     }
     for (int q = 0; q < kQueue; ++q) {
       mbar_init(qfull0 + 8 * q, 1);               // producer
-      mbar_init(qempty0 + 8 * q, 3 + kEpiWarps);  // MMA warp + 2 loader warps + epilogue warps
+      mbar_init(qempty0 + 8 * q, 2 + kEpiWarps);  // MMA warp + loader warp + epilogue warps
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -228,15 +252,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
         const uint32_t d0 = tmem_base + as * 256, d1 = d0 + 128;
         const uint32_t a_addr = smem_base + stage * p.stage_bytes;
         const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes);
-        const uint64_t bh = make_desc(a_addr + kAStageBytes), bl = make_desc(a_addr + kAStageBytes + p.b_term_bytes);
+        const uint64_t bh = make_desc_sw128(a_addr + kAStageBytes), bl = make_desc_sw128(a_addr + kAStageBytes + p.b_term_bytes);
         if (elect_one()) {
           if (cat) {
             umma_f8_imm<false>(d0, a0, bh, idesc);
             umma_f8_imm<false>(d1, a1, bh, idesc);
 #pragma unroll
-            for (int ks = 1; ks < kKBlock / 32; ++ks) {     // +256 B per 32-element k-step (>> 4)
-              umma_f8_imm<true>(d0, a0 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 16), idesc);
-              umma_f8_imm<true>(d1, a1 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 16), idesc);
+            for (int ks = 1; ks < kKBlock / 32; ++ks) {     // per 32-element k-step: weights +256 B, tokens +32 B (>> 4)
+              umma_f8_imm<true>(d0, a0 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 2), idesc);
+              umma_f8_imm<true>(d1, a1 + (uint64_t)(ks * 16), bh + (uint64_t)(ks * 2), idesc);
             }
           } else {
             umma_f8_imm<false>(d0, a0, bh, idesc);
@@ -245,11 +269,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
             umma_f8_imm<true>(d1, a1, bl, idesc);
 #pragma unroll
             for (int ks = 1; ks < kKBlock / 32; ++ks) {
-              const uint64_t o = (uint64_t)(ks * 16);
-              umma_f8_imm<true>(d0, a0 + o, bh + o, idesc);
-              umma_f8_imm<true>(d0, a0 + o, bl + o, idesc);
-              umma_f8_imm<true>(d1, a1 + o, bh + o, idesc);
-              umma_f8_imm<true>(d1, a1 + o, bl + o, idesc);
+              const uint64_t o = (uint64_t)(ks * 16), ob = (uint64_t)(ks * 2);
+              umma_f8_imm<true>(d0, a0 + o, bh + ob, idesc);
+              umma_f8_imm<true>(d0, a0 + o, bl + ob, idesc);
+              umma_f8_imm<true>(d1, a1 + o, bh + ob, idesc);
+              umma_f8_imm<true>(d1, a1 + o, bl + ob, idesc);
             }
           }
           tc_commit(empty0 + 8 * stage);
@@ -259,77 +283,53 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const Fp8Params p) {
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
       }
     }
-  } else if (warp == 2 || warp == 3) {
-    // ===== token-operand loaders: gather the hi and lo e4m3 rows (x or h) into the canonical
-    // K-major layout with cp.async, a few stages in flight per warp
-    const int wq = warp - 2;
-    const int r8 = lane & 7, c4 = lane >> 3;  // row in 8-row group, 16-byte chunks c4 and c4 + 4
-    int stage = 0, ph = 0, pend_stage = 0, pending = 0;
-    const int lag = min(kLag, p.n_stages - 1);
-    auto publish = [&](int count) {
-      fence_proxy_async_smem();
-      __syncwarp();
-      for (int j = 0; j < count; ++j) {
-        if (lane == 0) mbar_arrive(full0 + 8 * pend_stage);
-        if (++pend_stage == p.n_stages) pend_stage = 0;
-      }
-      pending -= count;
-    };
+  } else if (warp == 2) {
+    // ===== token-operand loader: TMA row gathers (4 rows x 128 B per instruction) of the hi and lo
+    // e4m3 rows of x (phase 1) or h (phase 2) into 128-byte-swizzled 8-row atoms; lane l owns rows
+    // 4l..4l+3 of the run, padding rows come back as zeros
+    int stage = 0, ph = 0;
     while (tm.at(tq.pop(), t)) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
-      const int ngroups = (n + 15) / 16 * 2;
+      const int npad = (n + 15) & ~15;
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-      const uint32_t lo_smem = ngroups <= 8 ? (uint32_t)ngroups * 1024u : (uint32_t)p.b_term_bytes;   // see the MMA warp
-      const uint8_t* rowh[8];   // this lane's hi source row in each of its groups (nullptr: zero fill)
-      size_t lo_off;            // lo row = hi row + lo_off
-      if (t.phase == 1) lo_off = (size_t)(p.xq_lo - p.xq_hi);
-      else lo_off = (size_t)(p.hq_lo - p.hq_hi);
+      const uint32_t lo_smem = npad <= 64 ? (uint32_t)npad * kKBlock : (uint32_t)p.b_term_bytes;   // see the MMA warp
+      const CUtensorMap* tmap = t.phase == 1 ? &p.tm_x : &p.tm_h;
+      const int lo_row = t.phase == 1 ? p.lo_row_x : p.lo_row_h;
+      int rh[4], rl[4];
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
-        const int row = (2 * g + wq) * 8 + r8;
-        rowh[g] = nullptr;
+      for (int i = 0; i < 4; ++i) {
+        const int row = lane * 4 + i;
+        rh[i] = kOobRow; rl[i] = kOobRow;
         if (row < n) {
-          if (t.phase == 1) rowh[g] = p.xq_hi + (size_t)p.wl.ent_tok[start + row] * p.H;
-          else rowh[g] = p.hq_hi + (size_t)(p.wl.run_hrow[t.run] + row) * p.I;
+          rh[i] = t.phase == 1 ? p.wl.ent_tok[start + row] : p.wl.run_hrow[t.run] + row;
+          rl[i] = rh[i] + lo_row;
         }
       }
       if (t.phase == 2) {
+        // h of this run is complete once all P1 gate/up tiles have published it (generic-proxy
+        // stores of other SMs, read here through the async proxy)
         if (lane == 0) {
           const int* flag = p.wl.ready + t.run;
           while (ld_acquire(flag) < p.P1) __nanosleep(64);
         }
         __syncwarp();
+        asm volatile("fence.proxy.async;" ::: "memory");
       }
+      const bool mine = lane * 4 < npad;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty0 + 8 * stage, ph ^ 1);
         const uint32_t b_addr = smem_base + stage * p.stage_bytes + kAStageBytes;
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          if (2 * g + wq < ngroups) {
-            const uint32_t a = b_addr + (2 * g + wq) * 1024 + r8 * 16;
-            const bool ok = rowh[g] != nullptr;
-            const uint8_t* src = ok ? rowh[g] + (size_t)kb * kKBlock + c4 * 16 : p.xq_hi;
-            const uint32_t sz = ok ? 16u : 0u;  // src-size 0: zero fill
-            const size_t lo = ok ? lo_off : 0, d64 = ok ? 64 : 0;
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + c4 * 128), "l"(src), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + (c4 + 4) * 128), "l"(src + d64), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + lo_smem + c4 * 128), "l"(src + lo), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + lo_smem + (c4 + 4) * 128), "l"(src + lo + d64), "r"(sz) : "memory");
-          }
+        if (lane == 0) mbar_arrive_expect_tx(full0 + 8 * stage, 2u * npad * kKBlock);
+        __syncwarp();
+        if (mine) {
+          tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, kb * kKBlock, rh[0], rh[1], rh[2], rh[3]);
+          tma_gather4(b_addr + lo_smem + lane * 512, tmap, full0 + 8 * stage, kb * kKBlock, rl[0], rl[1], rl[2], rl[3]);
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        ++pending;
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
-        if (pending > lag) {
-          if (lag >= 3) asm volatile("cp.async.wait_group 3;" ::: "memory");
-          else if (lag == 2) asm volatile("cp.async.wait_group 2;" ::: "memory");
-          else asm volatile("cp.async.wait_group 1;" ::: "memory");
-          publish(1);
-        }
       }
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-      publish(pending);
     }
+  } else if (warp == 3) {
+    // spare warp
   } else {
     // ===== epilogue (warps 4-11): warp -> TMEM lane quadrant q = warp % 4, column half hf
     const int q = warp & 3, hf = (warp - 4) >> 2;
@@ -467,7 +467,9 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
       }
     }
     ++p1_it;
-    // publish this tile's slice of h: all 256 epilogue threads' stores, then one release add
+    // publish this tile's slice of h: all 256 epilogue threads' stores (read later through the
+    // async proxy by other SMs' TMA gathers), then one release add
+    asm volatile("fence.proxy.async;" ::: "memory");
     __threadfence();
     asm volatile("bar.sync 2, 256;" ::: "memory");
     if (threadIdx.x == 128) atomicAdd(p.wl.ready + t.run, 1);
@@ -517,6 +519,31 @@ void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst, const void* g, const
   k_scale_table<<<16, 256, 0, st>>>(sg, su, sd, reinterpret_cast<float*>(dst + (size_t)3 * H * I), P1, P2, H / kKBlock, I / kKBlock);
 }
 
+// 2D byte tensor maps over the [hi rows | lo rows] x k arrays of x and h for tile::gather4 row
+// gathers: box = one row of 128 bytes, 128-byte swizzle (the layout the MMA descriptor names).
+caee_status caee_fp8_make_tensor_maps(caee_ctx* c) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  EncodeFn enc = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &q) != cudaSuccess || !enc)
+    return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  const cuuint32_t box[2] = {kKBlock, 1}, es[2] = {1, 1};
+  struct { unsigned char* tm; void* base; cuuint64_t cols, rows; } maps[2] = {
+      {c->tm_x, c->xq, (cuuint64_t)c->d.H, (cuuint64_t)2 * c->d.max_tokens},
+      {c->tm_h, c->hq, (cuuint64_t)c->d.I, (cuuint64_t)2 * c->h_rows_cap}};
+  for (auto& m : maps) {
+    const cuuint64_t gd[2] = {m.cols, m.rows}, gs[1] = {m.cols};
+    const CUresult rc = enc(reinterpret_cast<CUtensorMap*>(m.tm), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, m.base, gd, gs, box, es,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)rc);
+  }
+  c->tm_ready = true;
+  return CAEE_OK;
+}
+
 // Once per step, before the first expert launch: x -> its two e4m3 terms and block scales.
 void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (T <= 0) return;
@@ -542,6 +569,10 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
   p.run_begin = run_begin; p.run_count = run_count; p.ticket = ticket;
   p.sc_off = (int)((size_t)3 * d.H * d.I);
   p.t2_off = p.P1 * p.KB1 * 2;
+  memcpy(&p.tm_x, c->tm_x, sizeof(CUtensorMap));
+  memcpy(&p.tm_h, c->tm_h, sizeof(CUtensorMap));
+  p.lo_row_x = d.max_tokens;
+  p.lo_row_h = (int)c->h_rows_cap;
   const int ncap = std::min((int)c->wl.run_cap, (T + 15) & ~15);
   p.b_term_bytes = ncap * kKBlock;                  // one e4m3 term of the token operand
   p.stage_bytes = kAStageBytes + 2 * p.b_term_bytes;
