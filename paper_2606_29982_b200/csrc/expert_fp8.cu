@@ -27,8 +27,6 @@
 // issuer, warp 2 = token-operand loader (TMA row gathers of the hi/lo rows), warps 4-11 =
 // epilogue (two warps per TMEM lane quadrant, each half of the token columns).  Tiles are
 // claimed by atomic ticket, phase-1 tickets first (see umma_common.cuh).
-#include <cuda.h>
-
 #include <cstring>
 
 #include "umma_common.cuh"
@@ -62,22 +60,6 @@ struct Fp8Params {
   CUtensorMap tm_x, tm_h;
   int lo_row_x, lo_row_h;
 };
-
-constexpr int kOobRow = 0x40000000;   // beyond any tensor: the TMA unit writes zeros (padding rows)
-
-// Four rows of 128 bytes (k bytes [col, col + 128) of rows r0..r3) -> 512 bytes at dst, swizzled
-__device__ __forceinline__ void tma_gather4(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int col, int r0, int r1, int r2,
-                                            int r3) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
-      ::"r"(dst), "l"(tm), "r"(bar), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
-      : "memory");
-}
-// K-major operand descriptor for the 128-byte-swizzled token operand: 8-row atoms of 1024 B (SBO),
-// layout type 2 (SWIZZLE_128B), descriptor version 1; a 32-byte k-step advances the start address.
-__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr) {
-  return (uint64_t)((saddr >> 4) & 0x3FFF) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
-}
 
 // two floats -> two e4m3 codes (low byte = a), round to nearest even, saturating
 __device__ __forceinline__ uint16_t cvt_e4m3x2(float a, float b) {
@@ -522,24 +504,9 @@ void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst, const void* g, const
 // 2D byte tensor maps over the [hi rows | lo rows] x k arrays of x and h for tile::gather4 row
 // gathers: box = one row of 128 bytes, 128-byte swizzle (the layout the MMA descriptor names).
 caee_status caee_fp8_make_tensor_maps(caee_ctx* c) {
-  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  EncodeFn enc = nullptr;
-  cudaDriverEntryPointQueryResult q;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &q) != cudaSuccess || !enc)
-    return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
-  const cuuint32_t box[2] = {kKBlock, 1}, es[2] = {1, 1};
-  struct { unsigned char* tm; void* base; cuuint64_t cols, rows; } maps[2] = {
-      {c->tm_x, c->xq, (cuuint64_t)c->d.H, (cuuint64_t)2 * c->d.max_tokens},
-      {c->tm_h, c->hq, (cuuint64_t)c->d.I, (cuuint64_t)2 * c->h_rows_cap}};
-  for (auto& m : maps) {
-    const cuuint64_t gd[2] = {m.cols, m.rows}, gs[1] = {m.cols};
-    const CUresult rc = enc(reinterpret_cast<CUtensorMap*>(m.tm), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, m.base, gd, gs, box, es,
-                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (rc != CUDA_SUCCESS) return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)rc);
-  }
+  if (!encode_row_gather_map(c->tm_x, c->xq, (size_t)c->d.H, (size_t)2 * c->d.max_tokens) ||
+      !encode_row_gather_map(c->tm_h, c->hq, (size_t)c->d.I, (size_t)2 * c->h_rows_cap))
+    return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled failed for the e4m3 token-operand maps");
   c->tm_ready = true;
   return CAEE_OK;
 }

@@ -19,17 +19,21 @@
 //                       [gate tile][up tile]      -> D0 = gate rows, D1 = up rows (TMEM)
 //   phase 2 (down):     tile op = out rows [256 op, +256), stage kb over I:
 //                       [rows +0..127][rows +128..255] -> D0, D1
-// B operand (tokens): x rows (phase 1) or h rows (phase 2), gathered by two loader warps with
-// ordinary loads (they are L2-resident and 0.1% of the bytes) into the same canonical layout.
+// B operand (tokens): x rows (phase 1) or h rows (phase 2), 128 bytes (64 k) per row and stage,
+// gathered by the TMA unit (cp.async.bulk.tensor tile::gather4: four rows per instruction, rows
+// named by the work list, padding rows zero-filled) into 128-byte-swizzled 8-row atoms — the
+// SWIZZLE_128B K-major layout the token-operand descriptor names.
 //
 // e4m3 weights have their own kernel (expert_fp8.cu).
 //
 // Roles (256 threads; 1 CTA per SM):  warp 0 = weight producer (one lane issues bulk copies),
-// warp 1 = MMA issuer (one lane), warps 2-3 = token-operand loaders (warp 2 also owns TMEM
+// warp 1 = MMA issuer (one lane), warp 2 = token-operand loader (one TMA gather per lane and stage; also owns TMEM
 // alloc/free), warps 4-7 = epilogue (TMEM -> registers -> SwiGLU -> h, or -> o rows).
 // Tiles are claimed dynamically (one atomic ticket per tile, phase-1 tickets first); a
 // phase-2 tile only waits (per-run counter) for phase-1 tiles, which never wait, so the
 // schedule cannot deadlock and CTAs that finish early simply claim more tiles.
+#include <cstring>
+
 #include "umma_common.cuh"
 
 namespace {
@@ -50,10 +54,11 @@ struct UmmaParams {
   int n_stages, b_stage_bytes, stage_bytes;
   int run_begin, run_count;   // runs [run_begin, run_begin + run_count) of the work list; run_count < 0: all
   int ticket;                 // which tile-ticket counter of wl.sched this launch uses
+  CUtensorMap tm_x, tm_h;     // byte maps over x [T, 2H] and hbuf [rows, 2I] for the TMA row gathers
 };
 
 // ------------------------------------------------------------------ the kernel
-__global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p) {
+__global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_constant__ UmmaParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   __shared__ __align__(8) uint64_t bars[2 * kMaxStages + 4 + 2 * kQueue];
@@ -69,7 +74,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < p.n_stages; ++s) {
-      mbar_init(full0 + 8 * s, 3);   // producer's expect_tx arrive + 2 loader warps
+      mbar_init(full0 + 8 * s, 2);   // expect_tx arrives of the weight producer and of the token-operand loader
       mbar_init(empty0 + 8 * s, 1);  // tcgen05.commit
     }
     for (int a = 0; a < 2; ++a) {
@@ -78,7 +83,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
     }
     for (int q = 0; q < kQueue; ++q) {
       mbar_init(qfull0 + 8 * q, 1);                // producer
-      mbar_init(qempty0 + 8 * q, 7);               // MMA warp + 2 loader warps + 4 epilogue warps
+      mbar_init(qempty0 + 8 * q, 6);               // MMA warp + loader warp + 4 epilogue warps
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -131,7 +136,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
         mbar_wait(full0 + 8 * stage, ph);
         tc_fence_after();
         const uint32_t a_addr = smem_base + stage * p.stage_bytes;
-        const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes), b = make_desc(a_addr + kAStageBytes);
+        const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes), b = make_desc_sw128(a_addr + kAStageBytes);
         if (elect_one()) {
           if (kb == 0) {
             umma_bf16_imm<false>(d0, a0, b, idesc);
@@ -141,9 +146,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
             umma_bf16_imm<true>(d1, a1, b, idesc);
           }
 #pragma unroll
-          for (int ks = 1; ks < kKBlock / 16; ++ks) {   // +256 B per k-step (>> 4)
-            umma_bf16_imm<true>(d0, a0 + (uint64_t)(ks * 16), b + (uint64_t)(ks * 16), idesc);
-            umma_bf16_imm<true>(d1, a1 + (uint64_t)(ks * 16), b + (uint64_t)(ks * 16), idesc);
+          for (int ks = 1; ks < kKBlock / 16; ++ks) {   // per 16-element k-step: weights +256 B, tokens +32 B (>> 4)
+            umma_bf16_imm<true>(d0, a0 + (uint64_t)(ks * 16), b + (uint64_t)(ks * 2), idesc);
+            umma_bf16_imm<true>(d1, a1 + (uint64_t)(ks * 16), b + (uint64_t)(ks * 2), idesc);
           }
           tc_commit(empty0 + 8 * stage);
           if (kb == nkb - 1) tc_commit(tfull0 + 8 * as);
@@ -152,71 +157,45 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
       }
     }
-  } else if (warp == 2 || warp == 3) {
-    // ===== token-operand loaders: gather B rows (x or h) into the canonical K-major layout with
-    // cp.async, kLag stages in flight per warp so that L2 latency is off the critical path
-    const int wq = warp - 2;
-    const int r8 = lane & 7, c4 = lane >> 3;  // row in 8-row group, 16-byte chunk (c4 and c4+4)
-    int stage = 0, ph = 0, pend_stage = 0, pending = 0;
-    const int lag = min(kLag, p.n_stages - 1);  // a stage is published `lag` stages late: must stay inside the ring
-    auto publish = [&](int count) {  // the oldest `count` in-flight stages have landed
-      fence_proxy_async_smem();
-      __syncwarp();
-      for (int j = 0; j < count; ++j) {
-        if (lane == 0) mbar_arrive(full0 + 8 * pend_stage);
-        if (++pend_stage == p.n_stages) pend_stage = 0;
-      }
-      pending -= count;
-    };
+  } else if (warp == 2) {
+    // ===== token-operand loader: TMA row gathers (tile::gather4: 4 rows x 128 B per instruction)
+    // of the x rows (phase 1) or h rows (phase 2) of the run into 128-byte-swizzled 8-row atoms;
+    // lane l owns rows 4l..4l+3, padding rows come back as zeros
+    int stage = 0, ph = 0;
     while (tm.at(tq.pop(), t)) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
-      const int ngroups = (n + 15) / 16 * 2;  // 8-row groups in the padded tile
+      const int npad = (n + 15) & ~15;
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-      const uint8_t* rowp[8];  // this lane's source row in each of its groups (nullptr: zero fill)
+      const CUtensorMap* tmap = t.phase == 1 ? &p.tm_x : &p.tm_h;
+      int r[4];
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
-        const int row = (2 * g + wq) * 8 + r8;
-        rowp[g] = nullptr;
-        if (row < n) {
-          if (t.phase == 1) rowp[g] = reinterpret_cast<const uint8_t*>(p.x + (size_t)p.wl.ent_tok[start + row] * p.H);
-          else rowp[g] = reinterpret_cast<const uint8_t*>(p.hbuf + (size_t)(p.wl.run_hrow[t.run] + row) * p.I);
-        }
+      for (int i = 0; i < 4; ++i) {
+        const int row = lane * 4 + i;
+        r[i] = kOobRow;
+        if (row < n) r[i] = t.phase == 1 ? p.wl.ent_tok[start + row] : p.wl.run_hrow[t.run] + row;
       }
       if (t.phase == 2) {
-        // h of this run is complete once all P1 gate/up tiles have published it
+        // h of this run is complete once all P1 gate/up tiles have published it (generic-proxy
+        // stores of other SMs, read here through the async proxy)
         if (lane == 0) {
           const int* flag = p.wl.ready + t.run;
           while (ld_acquire(flag) < p.P1) __nanosleep(64);
         }
         __syncwarp();
+        asm volatile("fence.proxy.async;" ::: "memory");
       }
+      const bool mine = lane * 4 < npad;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty0 + 8 * stage, ph ^ 1);
         const uint32_t b_addr = smem_base + stage * p.stage_bytes + kAStageBytes;
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          if (2 * g + wq < ngroups) {
-            const uint32_t a = b_addr + (2 * g + wq) * 1024 + r8 * 16;
-            const uint8_t* src = rowp[g] ? rowp[g] + (size_t)kb * 128 + c4 * 16 : reinterpret_cast<const uint8_t*>(p.x);
-            const uint32_t sz = rowp[g] ? 16u : 0u;  // src-size 0: zero fill
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + c4 * 128), "l"(src), "r"(sz) : "memory");
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a + (c4 + 4) * 128), "l"(src + (rowp[g] ? 64 : 0)), "r"(sz) : "memory");
-          }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        ++pending;
+        if (lane == 0) mbar_arrive_expect_tx(full0 + 8 * stage, (uint32_t)npad * 128u);
+        __syncwarp();
+        if (mine) tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, kb * 128, r[0], r[1], r[2], r[3]);
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
-        if (pending > lag) {
-          if (lag >= 3) asm volatile("cp.async.wait_group 3;" ::: "memory");
-          else if (lag == 2) asm volatile("cp.async.wait_group 2;" ::: "memory");
-          else asm volatile("cp.async.wait_group 1;" ::: "memory");
-          publish(1);
-        }
       }
-      // flush at the tile boundary: nothing of this tile may wait behind a later tile's dependency
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-      publish(pending);
     }
+  } else if (warp == 3) {
+    // spare warp
   } else if (warp < 8) {
     // ===== epilogue: TMEM -> registers -> SwiGLU -> h (phase 1) or -> o rows (phase 2)
     const int q = warp - 4;  // TMEM lane quadrant of this warp (warp % 4)
@@ -264,7 +243,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const UmmaParams p)
       __syncwarp();
       if (lane == 0) mbar_arrive(tempty0 + 8 * as);
       if (t.phase == 1) {
-        // publish this tile's slice of h: all 128 epilogue threads' stores, then one release add
+        // publish this tile's slice of h: all 128 epilogue threads' stores (read later through the
+        // async proxy by other SMs' TMA gathers), then one release add
+        asm volatile("fence.proxy.async;" ::: "memory");
         __threadfence();
         asm volatile("bar.sync 1, 128;" ::: "memory");
         if (threadIdx.x == 128) atomicAdd(p.wl.ready + t.run, 1);
@@ -362,6 +343,12 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
   p.P1 = d.I / kTileRows; p.P2 = d.H / (2 * kTileRows);
   p.KB1 = d.H / kKBlock; p.KB2 = d.I / kKBlock;
   p.run_begin = run_begin; p.run_count = run_count; p.ticket = ticket;
+  // x is the caller's buffer: its map is encoded per call (host-side, ~1 us); h is ours
+  if (!c->tm_ready) {
+    if (encode_row_gather_map(c->tm_h, c->hbuf_b16, (size_t)d.I * 2, c->h_rows_cap)) c->tm_ready = true;
+  }
+  encode_row_gather_map(&p.tm_x, x, (size_t)d.H * 2, (size_t)T);
+  memcpy(&p.tm_h, c->tm_h, sizeof(CUtensorMap));
   const int ncap = std::min((int)c->wl.run_cap, (T + 15) & ~15);
   p.b_stage_bytes = ncap * kKBlock * 2;
   p.stage_bytes = kAStageBytes + p.b_stage_bytes;

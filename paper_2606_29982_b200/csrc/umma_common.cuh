@@ -2,6 +2,8 @@
 // shared-memory operand and instruction descriptors) and the dynamic tile schedule shared by
 // the bf16 and e4m3 expert kernels (expert_umma.cu, expert_fp8.cu).  sm_100a only.
 #pragma once
+#include <cuda.h>
+
 #include "caee_internal.cuh"
 
 namespace caee_umma {
@@ -117,6 +119,22 @@ __device__ __forceinline__ uint32_t make_idesc(int n, bool bf16) {
   return (1u << 4) | (bf16 ? ((1u << 7) | (1u << 10)) : 0u) | ((uint32_t)(n >> 3) << 17) |
          ((uint32_t)(kTileRows >> 4) << 24);
 }
+constexpr int kOobRow = 0x40000000;   // beyond any tensor: the TMA unit writes zeros (padding rows)
+
+// Four rows of 128 bytes (k bytes [col, col + 128) of rows r0..r3) -> 512 bytes at dst, swizzled
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int col, int r0, int r1, int r2,
+                                            int r3) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(dst), "l"(tm), "r"(bar), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
+}
+// K-major operand descriptor for the 128-byte-swizzled token operand: 8-row atoms of 1024 B (SBO),
+// layout type 2 (SWIZZLE_128B), descriptor version 1; a 32-byte k-step advances the start address.
+__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+
 __device__ __forceinline__ int ld_acquire(const int* p) {
   int v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -159,5 +177,24 @@ struct TileQueue {
   }
 };
 
+
+// Host: 2D byte tensor map over a [rows, row_bytes] array for tile::gather4 row gathers of 128-byte
+// pieces with the 128-byte swizzle (box = {128 bytes, 1 row}).  Returns false if the driver refuses.
+inline bool encode_row_gather_map(void* tm_out, const void* base, size_t row_bytes, size_t rows) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn enc = nullptr;
+  if (!enc) {
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &q) != cudaSuccess) enc = nullptr;
+    if (!enc) return false;
+  }
+  const cuuint64_t gd[2] = {(cuuint64_t)row_bytes, (cuuint64_t)rows}, gs[1] = {(cuuint64_t)row_bytes};
+  const cuuint32_t box[2] = {128, 1}, es[2] = {1, 1};
+  return enc(reinterpret_cast<CUtensorMap*>(tm_out), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), gd, gs, box, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 }  // namespace caee_umma
