@@ -488,9 +488,10 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  // e4m3 decode steps use 64-token runs: the token operand (two e4m3 terms) then leaves room for
-  // a deeper weight ring, and hi/lo share one MMA (expert_fp8.cu); prefill keeps 128 for weight reuse
-  c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
+  // decode steps (T <= 128) use 64-token runs: the smaller token operand leaves room for a deeper
+  // weight ring (only the shared experts and the few hottest experts are split and streamed twice),
+  // and the e4m3 kernel's hi/lo terms share one MMA (expert_fp8.cu); larger steps keep 128 for weight reuse
+  c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
   const bool fused = caee_decide_fits(c, T);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)

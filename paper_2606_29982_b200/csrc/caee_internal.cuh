@@ -40,7 +40,7 @@ struct caee_worklist {
   int32_t* sched;       // [n_tickets + max_runs]: tile-ticket counters (one per expert-kernel launch of a step),
   int32_t* ready;       //   then (= sched + n_tickets) per-run "h complete" counters; zeroed every step
   int32_t max_runs, n_tickets;
-  int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, or 64 (e4m3 decode steps)
+  int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, or 64 (UMMA decode steps, T <= 128)
 };
 
 struct caee_packed {
