@@ -2,6 +2,7 @@
 // sequences of the per-layer hot path.  No torch types, no exceptions across the boundary.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -119,7 +120,7 @@ void free_all(caee_ctx* c) {
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
-                  c->packed.dev_ptrs, c->xq, c->xs, c->hq, c->hs};
+                  c->packed.dev_ptrs, c->xq, c->xs, c->hq, c->hs, c->xg, c->wl_hist};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (size_t e = 0; e < c->packed.base.size(); ++e) {
@@ -163,6 +164,7 @@ caee_status create_impl(caee_ctx* c) {
   c->wl.n_tickets = (int)E + 2;
   A(c->wl.run_hrow, c->wl.max_runs); A(c->wl.meta, 16); A(c->wl.sched, c->wl.n_tickets + c->wl.max_runs);
   c->wl.ready = c->wl.sched + c->wl.n_tickets;
+  if (caee_wl_hist_ints(c)) { A(c->wl_hist, caee_wl_hist_ints(c)); }
   c->h_rows_cap = Tm * k + 15 * std::min(E, Tm * k) + S * (Tm + 15) + 16;
   if (c->kernel == CAEE_KERNEL_SIMT) { A(c->hbuf_f32, c->h_rows_cap * d.I); }
   else { A(c->hbuf_b16, c->h_rows_cap * d.I); }
@@ -170,6 +172,8 @@ caee_status create_impl(caee_ctx* c) {
     A(c->xq, 2 * Tm * d.H); A(c->xs, Tm * (d.H / 128));
     A(c->hq, 2 * c->h_rows_cap * d.I); A(c->hs, c->h_rows_cap * (d.I / 128));
     if ((rc = caee_fp8_make_tensor_maps(c)) != CAEE_OK) return rc;
+    if (const char* v = getenv("CAEE_FP8_WIDE_MIN_TOKENS")) c->fp8_wide_min_tokens = std::max(1, atoi(v));   // tuning aid
+    if (d.max_tokens >= c->fp8_wide_min_tokens) { A(c->xg, caee_fp8_wide_xg_bytes(c)); }
   }
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A
@@ -491,7 +495,9 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   // decode steps (T <= 128) use 64-token runs: the smaller token operand leaves room for a deeper
   // weight ring (only the shared experts and the few hottest experts are split and streamed twice),
   // and the e4m3 kernel's hi/lo terms share one MMA (expert_fp8.cu); larger steps keep 128 for weight reuse
+  // e4m3 prefill-size steps: 256-token runs for the converter kernel (expert_fp8_wide.cu)
   c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
+  if (c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && T >= c->fp8_wide_min_tokens) c->wl.run_cap = CAEE_RUN_TOKENS_WIDE;
   const bool fused = caee_decide_fits(c, T);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)

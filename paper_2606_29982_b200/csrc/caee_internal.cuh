@@ -17,6 +17,8 @@
 #define CAEE_MAX_D 64
 #define CAEE_RUN_TOKENS 128 /* most tokens per run: one UMMA N tile */
 #define CAEE_RUN_TOKENS_MIN 64
+#define CAEE_RUN_TOKENS_WIDE 256 /* e4m3 prefill kernel (expert_fp8_wide.cu): one N = 256 UMMA tile */
+#define CAEE_FP8_WIDE_MIN_TOKENS 257 /* steps of at least this many tokens take the e4m3 prefill kernel */
 #define CAEE_DECIDE_MAX_TOKENS 256 /* largest step the one-kernel decision path takes (decide.cu) */
 
 // One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
@@ -40,7 +42,8 @@ struct caee_worklist {
   int32_t* sched;       // [n_tickets + max_runs]: tile-ticket counters (one per expert-kernel launch of a step),
   int32_t* ready;       //   then (= sched + n_tickets) per-run "h complete" counters; zeroed every step
   int32_t max_runs, n_tickets;
-  int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, or 64 (UMMA decode steps, T <= 128)
+  int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, 64 (UMMA decode steps, T <= 128) or
+                        // CAEE_RUN_TOKENS_WIDE (e4m3 prefill steps)
 };
 
 struct caee_packed {
@@ -99,6 +102,7 @@ struct caee_ctx {
   int64_t* load = nullptr;   // [D]
   int64_t* scalars = nullptr;  // [8]
   caee_worklist wl;
+  int32_t* wl_hist = nullptr;        // [ceil(Tmax k / 256), E] per-block entry counts of the large-step fill (worklist.cu)
   float* hbuf_f32 = nullptr;         // SIMT: h rows [rows, I] fp32
   __nv_bfloat16* hbuf_b16 = nullptr; // UMMA: h rows [rows, I] bf16 (bf16 weights) / fp16 (e4m3 weights)
   uint8_t* xq = nullptr;             // UMMA e4m3: hi | lo e4m3 terms of x, [Tmax, H] each
@@ -106,7 +110,9 @@ struct caee_ctx {
   uint8_t* hq = nullptr;             // UMMA e4m3: hi | lo terms of h, [rows, I] each
   float* hs = nullptr;               //   and its scales [rows, I/128]
   alignas(64) unsigned char tm_x[128] = {0}, tm_h[128] = {0};  // CUtensorMap of xq / hq (row gathers), see expert_fp8.cu
+  uint8_t* xg = nullptr;             // e4m3 prefill kernel (expert_fp8_wide.cu): per-run stage images of the gathered x rows
   bool tm_ready = false;
+  int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
@@ -153,6 +159,7 @@ void caee_launch_compensate(caee_ctx* c, int flags, const float* scores, int T, 
                             cudaStream_t s);
 // worklist.cu
 void caee_launch_worklist(caee_ctx* c, int T, const int32_t* idx, const float* gate, cudaStream_t s);
+size_t caee_wl_hist_ints(const caee_ctx* c);
 void caee_launch_export_worklist(caee_ctx* c, int T, const caee_prune_out* out, cudaStream_t s);
 // expert_simt.cu
 void caee_launch_expert_simt(caee_ctx* c, const void* x, int T, cudaStream_t s);
@@ -166,11 +173,16 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
 // expert_fp8.cu
 caee_status caee_fp8_supported(const caee_ctx* c, std::string* why);
 size_t caee_fp8_packed_bytes(const caee_ctx* c);
+size_t caee_fp8_norm_offset(const caee_ctx* c);
 void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst_dev, const void* g, const void* u, const void* d, const float* sg,
                                  const float* su, const float* sd, cudaStream_t s);
 void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 caee_status caee_fp8_make_tensor_maps(caee_ctx* c);
 void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
+// expert_fp8_wide.cu
+size_t caee_fp8_wide_xg_bytes(const caee_ctx* c);
+void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
+void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);

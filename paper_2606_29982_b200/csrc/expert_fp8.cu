@@ -140,6 +140,31 @@ __global__ void k_scale_table(const float* __restrict__ sg, const float* __restr
   }
 }
 
+// Per-expert power of two 2^J with max |scale| 2^J in [64, 128): the prefill kernel
+// (expert_fp8_wide.cu) folds scale 2^J into fp16 weights (|code| <= 448, so products stay below
+// 65504) and multiplies its accumulators by 2^-J.  norm[0] = 2^J, norm[1] = 2^-J.
+__global__ void __launch_bounds__(256) k_scale_norm(const float* __restrict__ tab, int n, float* __restrict__ norm) {
+  __shared__ float red[8];
+  float m = 0.f;
+  for (int i = threadIdx.x; i < n; i += 256) {
+    const float v = fabsf(tab[i]);
+    if (v <= 3.0e38f) m = fmaxf(m, v);   // skips inf / nan
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int i = 1; i < 8; ++i) m = fmaxf(m, red[i]);
+    int ex = 7;
+    if (m > 0.f) frexpf(m, &ex);          // m = f 2^ex, f in [0.5, 1)
+    int J = 7 - ex;
+    J = max(-100, min(100, J));
+    norm[0] = ldexpf(1.0f, J);
+    norm[1] = ldexpf(1.0f, -J);
+  }
+}
+
 // ------------------------------------------------------------------ the kernel, part 1: roles 0-3
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constant__ Fp8Params p);
 
@@ -486,6 +511,10 @@ caee_status caee_fp8_supported(const caee_ctx* c, std::string* why) {
 }
 
 size_t caee_fp8_packed_bytes(const caee_ctx* c) {
+  return (size_t)3 * c->d.H * c->d.I + ((table_floats(c) * 4 + 15) & ~(size_t)15) + 16;   // + the 2^J pair
+}
+
+size_t caee_fp8_norm_offset(const caee_ctx* c) {
   return (size_t)3 * c->d.H * c->d.I + ((table_floats(c) * 4 + 15) & ~(size_t)15);
 }
 
@@ -498,7 +527,9 @@ void caee_launch_pack_expert_fp8(caee_ctx* c, uint8_t* dst, const void* g, const
   k_pack_e4m3<<<(unsigned)((n1 + 255) / 256), 256, 0, st>>>((const uint8_t*)u, dst, I, H, 1, 0);
   k_pack_e4m3<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>((const uint8_t*)dn, dst, H, I, 2, p2_off);
   const int P1 = I / kTileRows, P2 = H / (2 * kTileRows);
-  k_scale_table<<<16, 256, 0, st>>>(sg, su, sd, reinterpret_cast<float*>(dst + (size_t)3 * H * I), P1, P2, H / kKBlock, I / kKBlock);
+  float* tab = reinterpret_cast<float*>(dst + (size_t)3 * H * I);
+  k_scale_table<<<16, 256, 0, st>>>(sg, su, sd, tab, P1, P2, H / kKBlock, I / kKBlock);
+  k_scale_norm<<<1, 256, 0, st>>>(tab, (int)table_floats(c), reinterpret_cast<float*>(dst + caee_fp8_norm_offset(c)));
 }
 
 // 2D byte tensor maps over the [hi rows | lo rows] x k arrays of x and h for tile::gather4 row

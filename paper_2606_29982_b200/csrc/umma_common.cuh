@@ -175,6 +175,14 @@ struct TileQueue {
     if (++q == kQueue) { q = 0; ph ^= 1; }
     return t;
   }
+  // the same for a role that runs on a single lane
+  __device__ __forceinline__ int pop1() {
+    mbar_wait(full0 + 8 * q, ph);
+    const int t = slots[q];
+    mbar_arrive(empty0 + 8 * q);
+    if (++q == kQueue) { q = 0; ph ^= 1; }
+    return t;
+  }
 };
 
 

@@ -101,6 +101,38 @@ def test_prune_compensate_compact_bit_exact(H, cfg, mode):
         L.close()
 
 
+@pytest.mark.parametrize("mode", ["none", "frac", "thresh"])
+def test_compact_large_step_segmented_fill(H, mode):
+    """Steps of more than 4096 (token, slot) entries take the segmented fill of worklist.cu
+    (per-block histograms + in-block ranks): lists must still be the oracle's, entry for entry.
+    T = 1500 x k = 4 gives 6000 entries, the last block ragged."""
+    from paper_2606_29982_b200 import binding as B
+    cfg, T = R1S, 1500
+    L = _layer(H, cfg, max_tokens=T)
+    try:
+        m, theta = MODES[mode]
+        th = _thresh_theta(cfg, T) if theta is None else theta
+        x = wl.hidden(cfg, T, 21, L.device)
+        s = L.oracle_scores(x)
+        d = L.oracle_decisions(s, m, th)
+        idx = torch.from_numpy(d["idx0"]).to(L.device)
+        gate = torch.from_numpy(d["gate0"]).to(L.device)
+        out = B.PruneOut(cfg.E, cfg.D, T, cfg.k, L.device)
+        B.caee_prune(L.ctx, B.prune_params(m, th), torch.from_numpy(s).to(L.device), T, idx, gate, out.struct)
+        torch.cuda.synchronize()
+        g = {k: v.cpu().numpy() for k, v in out.t.items()}
+        cp = d["compact"]
+        assert np.array_equal(idx.cpu().numpy(), d["idx"])
+        nr = int(g["n_run"][0])
+        assert nr == cp["n_run"]
+        assert np.array_equal(g["expert_ids"][:nr], cp["expert_ids"]) and np.array_equal(g["offs"][:nr + 1], cp["offs"])
+        ne = int(cp["offs"][-1])
+        assert np.array_equal(g["tok"][:ne], cp["tok"]) and np.array_equal(g["slot"][:ne], cp["slot"])
+        assert np.array_equal(g["wt"][:ne].view(np.uint32), cp["wt"].view(np.uint32))
+    finally:
+        L.close()
+
+
 @pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, wl.scaled(wl.C3, name="R1-router", H=256, I=128)], ids=lambda c: c.name)
 @pytest.mark.parametrize("mode", ["dense"] + list(MODES))
 def test_forward_decisions_bit_exact_fused_and_standalone(H, cfg, mode):
