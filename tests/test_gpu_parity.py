@@ -402,8 +402,9 @@ def test_forward_c4_full_size_sampled(H, T, mode):
 
 
 def test_forward_c4_prefill_4096_sampled(H):
-    """Config 4's 4096-token prefill batch (stand-alone decision kernels, 128-token runs, the wide
-    epilogue of the e4m3 kernel): K_final and F_* for all 4096 tokens bit-exact, y on sampled tokens."""
+    """Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill,
+    256-token runs, the e4m3 prefill kernel expert_fp8_wide.cu): K_final and F_* for all 4096 tokens
+    bit-exact, y on sampled tokens."""
     L = H.GpuLayer(wl.C4, seed=0, max_tokens=4096, keep_raw=False)
     try:
         T = 4096
