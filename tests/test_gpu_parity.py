@@ -335,12 +335,14 @@ def test_forward_small_fp8(H, kernel):
         L.close()
 
 
-def test_forward_fp8_uneven_block_scales(H):
-    """Block scales spread over three decades inside one tile row: the ratio/ref folding of the
-    UMMA path must still match the oracle's exact dequantisation."""
+@pytest.mark.parametrize("T", [24, 300])
+def test_forward_fp8_uneven_block_scales(H, T):
+    """Block scales spread over three decades inside one tile row: the per-block promotion of the
+    decode kernel (T = 24) and the scale x 2^J folding into fp16 weights of the prefill kernel
+    (T = 300) must still match the oracle's exact dequantisation."""
     from paper_2606_29982_b200 import binding as B
     cfg = C4S
-    L = _layer(H, cfg, max_tokens=32, kernel=B.CAEE_KERNEL_UMMA)
+    L = _layer(H, cfg, max_tokens=max(32, T), kernel=B.CAEE_KERNEL_UMMA)
     try:
         g = torch.Generator(device=L.device)
         g.manual_seed(5)
@@ -352,8 +354,8 @@ def test_forward_fp8_uneven_block_scales(H):
                            [r["gate_scale"] for r in L.raw], [r["up_scale"] for r in L.raw],
                            [r["down_scale"] for r in L.raw], pack=1)
         L._host.clear()
-        r = _forward_case(H, L, 24, "dense")
-        print(f"fp8 uneven scales: max|err|/RMS = {r:.3e}")
+        r = _forward_case(H, L, T, "dense")
+        print(f"fp8 uneven scales T={T}: max|err|/RMS = {r:.3e}")
     finally:
         L.close()
 
