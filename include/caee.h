@@ -238,6 +238,38 @@ caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gat
 caee_status caee_profile(caee_ctx* ctx, int32_t n_slots);
 caee_status caee_profile_read(caee_ctx* ctx, float* expert_ms, int32_t* n_out);
 
+/* ---- LFU expert cache (Fig. 8: "each HBM caches only a subset of 1024 experts,
+ * managed by a Least Frequently Used (LFU) eviction policy").  Turns the
+ * static residency mask R(e,d) of caee_set_residency into state that evolves over the steps of a
+ * multi-layer decode loop.  Rules (R30-R34): keys are (layer, routed expert); a
+ * key's frequency is the number of steps that executed it (after pruning), kept across
+ * evictions; a step first counts its executed experts, then inserts its misses in ascending
+ * expert order into the lowest free slot, else over the least frequently used key that the
+ * step does not execute (ties: smaller (layer, expert)); the cache starts empty; the cost
+ * model of a step sees the cache as it is when the step starts.
+ *
+ * n_slots device slots of one packed expert each are allocated when the first attached layer's
+ * weights are set.  caee_cache_attach must precede caee_set_weights(pack != 0) on that context
+ * (UMMA kernels only); from then on every routed expert of the layer lives in pinned host
+ * memory, caee_set_residency is refused, and caee_moe_forward* fetches the step's misses with
+ * one cudaMemcpyAsync each on a side stream while the hits compute (one host synchronisation per
+ * step, as in the static offload path).  All layers of one cache must have the same packed
+ * expert size and be driven from ONE stream.  A step whose executed experts outnumber the slots
+ * fails with CAEE_ESTATE.  The cache must outlive its attached contexts' calls; destroy the
+ * contexts first. */
+typedef struct caee_cache caee_cache;
+typedef struct caee_cache_stats {
+  int64_t hits, misses, evictions; /* per executed (layer, expert, step), since creation */
+  int64_t h2d_bytes;               /* misses x packed expert bytes                        */
+} caee_cache_stats;
+caee_status caee_cache_create(int32_t n_slots, caee_cache** out);
+void caee_cache_destroy(caee_cache* cache);
+caee_status caee_cache_attach(caee_cache* cache, caee_ctx* ctx, int32_t layer_id);
+caee_status caee_cache_read_stats(const caee_cache* cache, caee_cache_stats* out);
+/* Contents per slot (host arrays of n_slots): layer and expert (-1: free slot) and the key's
+ * frequency. */
+caee_status caee_cache_snapshot(const caee_cache* cache, int32_t* layer, int32_t* expert, int64_t* freq);
+
 /* Library / build identification, e.g. "caee-b200 0.1 sm_100a". */
 const char* caee_version(void);
 

@@ -27,7 +27,8 @@ CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",
            "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_route",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
-           "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version"]
+           "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version",
+           "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot"]
 
 
 class caee_layer_desc(C.Structure):
@@ -66,7 +67,17 @@ class caee_cost_fit(C.Structure):
                 ("gbytes_per_s", C.c_double), ("n_points", C.c_int32), ("valid", C.c_int32)]
 
 
+class caee_cache_stats(C.Structure):
+    _fields_ = [("hits", C.c_int64), ("misses", C.c_int64), ("evictions", C.c_int64), ("h2d_bytes", C.c_int64)]
+
+
 _ctx_p = C.c_void_p
+_lib.caee_cache_create.argtypes = [C.c_int32, C.POINTER(C.c_void_p)]
+_lib.caee_cache_destroy.argtypes = [C.c_void_p]
+_lib.caee_cache_destroy.restype = None
+_lib.caee_cache_attach.argtypes = [C.c_void_p, _ctx_p, C.c_int32]
+_lib.caee_cache_read_stats.argtypes = [C.c_void_p, C.POINTER(caee_cache_stats)]
+_lib.caee_cache_snapshot.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_create.argtypes = [C.POINTER(caee_layer_desc), C.POINTER(_ctx_p)]
 _lib.caee_destroy.argtypes = [_ctx_p]
 _lib.caee_last_error.argtypes = [_ctx_p]
@@ -90,7 +101,7 @@ _lib.caee_last_routing.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p, C.
 _lib.caee_profile.argtypes = [_ctx_p, C.c_int32]
 _lib.caee_profile_read.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
 for _n in EXPORTS:
-    if _n not in ("caee_last_error", "caee_version"):
+    if _n not in ("caee_last_error", "caee_version", "caee_cache_destroy"):
         getattr(_lib, _n).restype = C.c_int32
 
 
@@ -219,6 +230,34 @@ def caee_profile_read(ctx, n_slots):
     n = C.c_int32(0)
     _check(_lib.caee_profile_read(ctx, _ptr(ms), C.addressof(n)), ctx)
     return ms[:n.value].copy()
+
+
+def caee_cache_create(n_slots):
+    cache = C.c_void_p()
+    _check(_lib.caee_cache_create(int(n_slots), C.byref(cache)))
+    return cache
+
+
+def caee_cache_destroy(cache):
+    _lib.caee_cache_destroy(cache)
+
+
+def caee_cache_attach(cache, ctx, layer_id):
+    _check(_lib.caee_cache_attach(cache, ctx, int(layer_id)), ctx)
+
+
+def caee_cache_read_stats(cache):
+    st = caee_cache_stats()
+    _check(_lib.caee_cache_read_stats(cache, C.byref(st)))
+    return st
+
+
+def caee_cache_snapshot(cache, n_slots):
+    """[(layer, expert, freq) or None] per slot."""
+    layer, expert = np.zeros(n_slots, np.int32), np.zeros(n_slots, np.int32)
+    freq = np.zeros(n_slots, np.int64)
+    _check(_lib.caee_cache_snapshot(cache, _ptr(layer), _ptr(expert), _ptr(freq)))
+    return [None if layer[s] < 0 else (int(layer[s]), int(expert[s]), int(freq[s])) for s in range(n_slots)]
 
 
 # ---- small conveniences for tests / bench (marshalling only) -----------------------------

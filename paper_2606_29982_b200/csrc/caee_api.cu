@@ -1,5 +1,6 @@
 // caee_api.cu — the C ABI of include/caee.h: context, validation, tables, and the enqueue
 // sequences of the per-layer hot path.  No torch types, no exceptions across the boundary.
+#include <algorithm>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -132,6 +133,7 @@ void free_all(caee_ctx* c) {
     if (p) cudaFree(p);
   for (cudaEvent_t e : c->fetch_ev) cudaEventDestroy(e);
   if (c->host_meta) cudaFreeHost(c->host_meta);
+  if (c->cache_up) cudaFreeHost(c->cache_up);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   c->prof_ev.clear();
   if (c->side_stream) cudaStreamDestroy(c->side_stream);
@@ -278,6 +280,7 @@ caee_status caee_destroy(caee_ctx* c) {
   if (!c) return CAEE_EINVAL;
   DeviceGuard g(c->device);
   cudaDeviceSynchronize();
+  caee_cache_detach(c);
   free_all(c);
   delete c;
   return CAEE_OK;
@@ -308,6 +311,7 @@ caee_status caee_set_partitions(caee_ctx* c, const int32_t* part, int32_t D) {
 caee_status caee_set_residency(caee_ctx* c, const uint8_t* resident) {
   if (!c) return CAEE_EINVAL;
   if (!resident) return caee_fail(c, CAEE_EINVAL, "resident is NULL");
+  if (c->cache) return caee_fail(c, CAEE_ESTATE, "the context is attached to an expert cache: its residency is the cache's state");
   DeviceGuard g(c->device);
   CAEE_CUDA(c, cudaDeviceSynchronize());
   bool changed = false;
@@ -372,10 +376,15 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     c->stage_slot.assign(n, nullptr);
     c->fetch_ev.clear();
     c->any_offload = false;
+    if (c->cache) {
+      caee_status crc = caee_cache_prepare_layer(c, P.bytes_per_expert);
+      if (crc != CAEE_OK) return crc;
+      if (!c->cache_up) CAEE_CUDA(c, cudaMallocHost((void**)&c->cache_up, (size_t)c->d.E * 9 + sizeof(void*) * n));
+    }
     std::vector<uint8_t*> dptr(n, nullptr);
     uint8_t* tmp = nullptr;  // device scratch for packing a host-resident expert
     for (int e = 0; e < n; ++e) {
-      const bool res = e >= c->d.E || c->resident_h[e];
+      const bool res = e >= c->d.E || (!c->cache && c->resident_h[e]);
       if (res) {
         CAEE_CUDA(c, cudaMalloc((void**)&P.base[e], P.bytes_per_expert));
         caee_launch_pack_expert(c, e, P.base[e], c->wg_h[e], c->wu_h[e], c->wd_h[e], c->sg_h[e], c->su_h[e], c->sd_h[e], 0);
@@ -388,8 +397,10 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
         CAEE_CUDA(c, cudaMallocHost((void**)&P.base[e], P.bytes_per_expert));
         P.on_host[e] = 1;
         CAEE_CUDA(c, cudaMemcpy(P.base[e], tmp, P.bytes_per_expert, cudaMemcpyDeviceToHost));
-        CAEE_CUDA(c, cudaMalloc((void**)&c->stage_slot[e], P.bytes_per_expert));
-        dptr[e] = c->stage_slot[e];
+        if (!c->cache) {   // static offload: a staging slot per expert; cache mode: the cache's slots
+          CAEE_CUDA(c, cudaMalloc((void**)&c->stage_slot[e], P.bytes_per_expert));
+          dptr[e] = c->stage_slot[e];
+        }
         cudaEvent_t ev;
         CAEE_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         c->fetch_ev.push_back(ev);
@@ -400,6 +411,8 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     if (tmp) cudaFree(tmp);
     CAEE_CUDA(c, cudaMemcpy(P.dev_ptrs, dptr.data(), pb, cudaMemcpyHostToDevice));
     CAEE_CUDA(c, cudaDeviceSynchronize());
+    c->dptr_h = dptr;
+    if (c->cache) { caee_status urc = upload_costs(c); if (urc != CAEE_OK) return urc; }
   } else {
     for (int e = 0; e < c->d.E; ++e)
       if (!c->resident_h[e]) return caee_fail(c, CAEE_EUNSUPPORTED, "the SIMT expert kernel needs every expert in device memory");
@@ -498,6 +511,20 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   // e4m3 prefill-size steps: 256-token runs for the converter kernel (expert_fp8_wide.cu)
   c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
   if (c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && T >= c->fp8_wide_min_tokens) c->wl.run_cap = CAEE_RUN_TOKENS_WIDE;
+  if (c->cache) {
+    // R33: the step's cost model and run order see the cache as it is now (other layers' misses
+    // may have evicted this layer's experts since its last step).  The pinned staging buffer is
+    // free to rewrite: every cached step ends its decision part with a stream synchronisation.
+    const int E = c->d.E, n = E + c->d.S;
+    int64_t* w = reinterpret_cast<int64_t*>(c->cache_up);
+    uint8_t** dp = reinterpret_cast<uint8_t**>(c->cache_up + (size_t)E * 8);
+    uint8_t* rs = c->cache_up + (size_t)E * 8 + sizeof(void*) * n;
+    for (int e = 0; e < E; ++e) { w[e] = c->resident_h[e] ? c->ticks_res_h[e] : c->ticks_miss_h[e]; rs[e] = c->resident_h[e]; }
+    for (int e = 0; e < n; ++e) dp[e] = c->dptr_h[e];
+    CAEE_CUDA(c, cudaMemcpyAsync(c->w_eff, w, sizeof(int64_t) * E, cudaMemcpyHostToDevice, st));
+    CAEE_CUDA(c, cudaMemcpyAsync(c->resident, rs, E, cudaMemcpyHostToDevice, st));
+    CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs, dp, sizeof(void*) * n, cudaMemcpyHostToDevice, st));
+  }
   const bool fused = caee_decide_fits(c, T);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
@@ -536,9 +563,25 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
       if (!segs.empty() && segs.back().e == run_expert[r]) ++segs.back().count;
       else segs.push_back({run_expert[r], r, 1});
     }
+    std::vector<uint8_t*> miss_slots;
+    if (c->cache) {
+      // LFU cache (cache.cu, R30-R32): count the step's routed experts, give every miss a slot
+      std::vector<int32_t> executed;
+      for (int r = 0; r < n_runs; ++r)
+        if (run_expert[r] < c->d.E && (executed.empty() || executed.back() != run_expert[r])) executed.push_back(run_expert[r]);
+      std::sort(executed.begin(), executed.end());
+      executed.erase(std::unique(executed.begin(), executed.end()), executed.end());
+      if ((rc = caee_cache_step(c, executed.data(), (int)executed.size(), &miss_slots)) != CAEE_OK) return rc;
+      if (miss_slots.size() != segs.size()) return caee_fail(c, CAEE_ESTATE, "expert cache out of step with the run list (%zu misses, %zu non-resident experts)", miss_slots.size(), segs.size());
+      // the misses' image pointers, before any expert kernel of this step (second half of the staging buffer is not
+      // needed: write the few changed entries straight from dptr_h, pageable -> staged at call time)
+      for (size_t i = 0; i < segs.size(); ++i)
+        CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs + segs[i].e, &c->dptr_h[segs[i].e], sizeof(void*), cudaMemcpyHostToDevice, st));
+    }
     for (size_t i = 0; i < segs.size(); ++i) {
       const int e = segs[i].e;
-      CAEE_CUDA(c, cudaMemcpyAsync(c->stage_slot[e], c->packed.base[e], c->packed.bytes_per_expert, cudaMemcpyHostToDevice, c->side_stream));
+      uint8_t* dst = c->cache ? miss_slots[i] : c->stage_slot[e];
+      CAEE_CUDA(c, cudaMemcpyAsync(dst, c->packed.base[e], c->packed.bytes_per_expert, cudaMemcpyHostToDevice, c->side_stream));
       CAEE_CUDA(c, cudaEventRecord(c->fetch_ev[i], c->side_stream));
     }
     n_fetch = (int)segs.size();

@@ -55,6 +55,20 @@ struct caee_packed {
   size_t p1_tile_bytes = 0, p2_tile_bytes = 0;  // bytes of one phase-1 / phase-2 tile (all k-blocks)
 };
 
+struct caee_ctx;
+
+// LFU expert cache shared by the layers (contexts) attached to it (cache.cu; include/caee.h).
+struct caee_cache {
+  int n_slots = 0, device = 0;
+  size_t slot_bytes = 0;                       // packed expert bytes; 0 until the first layer's weights are set
+  std::vector<uint8_t*> slot_ptr;              // [n_slots] device slots
+  std::vector<int32_t> slot_layer, slot_expert;  // [n_slots] key of each slot, -1 = free
+  std::vector<caee_ctx*> layers;               // by layer id (NULL: not attached)
+  std::vector<std::vector<int64_t>> freq;      // [layer][E] executions so far (kept across evictions)
+  std::vector<std::vector<int32_t>> slot_of;   // [layer][E] slot of a cached key, else -1
+  caee_cache_stats st = {0, 0, 0, 0};
+};
+
 struct caee_ctx {
   caee_layer_desc d;
   int device = 0, num_sms = 0;
@@ -129,6 +143,12 @@ struct caee_ctx {
   std::vector<cudaEvent_t> fetch_ev;     // one per non-resident expert
   int32_t* host_meta = nullptr;          // pinned: meta[16] then run_expert[max_runs]
   bool any_offload = false;
+
+  // LFU cache mode (cache.cu): residency, effective costs and image pointers change every step
+  caee_cache* cache = nullptr;
+  int cache_layer = -1;
+  std::vector<uint8_t*> dptr_h;          // host copy of packed.dev_ptrs
+  uint8_t* cache_up = nullptr;           // pinned staging: w_eff [E] int64 | dev_ptrs [E+S] | resident [E]
 };
 
 caee_status caee_fail(caee_ctx* c, caee_status code, const char* fmt, ...);
@@ -183,6 +203,10 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
 size_t caee_fp8_wide_xg_bytes(const caee_ctx* c);
 void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
+// cache.cu
+caee_status caee_cache_prepare_layer(caee_ctx* c, size_t slot_bytes);
+void caee_cache_detach(caee_ctx* c);
+caee_status caee_cache_step(caee_ctx* c, const int32_t* executed, int n_executed, std::vector<uint8_t*>* miss_slots);
 // combine.cu
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);

@@ -9,20 +9,29 @@ from . import workloads as wl
 
 
 class Layer:
-    def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=False, device="cuda:0"):
+    def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=False, device="cuda:0",
+                 cache=None, layer_id=0, weight_seed=None):
+        """cache: a caee_cache handle — the layer's routed experts then live in pinned host memory and
+        are served through the LFU cache (layer_id = its key there).  weight_seed: seed of the expert
+        weights when it should differ from the router's seed (layers of a synthetic multi-layer model)."""
         self.cfg, self.seed, self.device, self.max_tokens = cfg, seed, device, max_tokens
+        self.weight_seed = seed if weight_seed is None else weight_seed
         torch.cuda.set_device(device)
         self.ctx = B.caee_create(B.layer_desc(cfg, max_tokens, kernel))
         self.Wr, self.b_logit, self.corr_bias = wl.router(cfg, seed, device)
         B.caee_set_router(self.ctx, self.Wr, self.b_logit, self.corr_bias)
         self.part = wl.partitions(cfg)
         B.caee_set_partitions(self.ctx, self.part, cfg.D)
-        self.resident = wl.residency(cfg, seed)
-        B.caee_set_residency(self.ctx, self.resident)          # before the weights: it decides where images live
+        if cache is not None:
+            B.caee_cache_attach(cache, self.ctx, layer_id)         # before the weights; the cache starts empty
+            self.resident = wl.residency(cfg, seed) * 0
+        else:
+            self.resident = wl.residency(cfg, seed)
+            B.caee_set_residency(self.ctx, self.resident)          # before the weights: it decides where images live
         self.ticks_res, self.ticks_miss = wl.cost_tables(cfg)
         B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
         n = cfg.E + cfg.S
-        raw = [wl.expert_weights(cfg, seed, e, device) for e in range(n)]
+        raw = [wl.expert_weights(cfg, self.weight_seed, e, device) for e in range(n)]
         fp8 = cfg.w_dtype == wl.DT_E4M3
         B.caee_set_weights(self.ctx, [r["gate"] for r in raw], [r["up"] for r in raw], [r["down"] for r in raw],
                            [r["gate_scale"] for r in raw] if fp8 else None, [r["up_scale"] for r in raw] if fp8 else None,

@@ -15,14 +15,14 @@ TOL = {wl.DT_F32: 1e-4, wl.DT_BF16: 2e-2, wl.DT_E4M3: 5e-2}   # x RMS(y), BASELI
 
 
 class GpuLayer(Layer):
-    def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=True, device="cuda:0"):
-        super().__init__(cfg, seed, max_tokens, kernel, keep_raw, device)
+    def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=True, device="cuda:0", **kw):
+        super().__init__(cfg, seed, max_tokens, kernel, keep_raw, device, **kw)
         self._host = {}
 
     # ---- host copies of exactly the bits the GPU holds
     def host_expert(self, e):
         if e not in self._host:
-            r = self.raw[e] if self.raw is not None else wl.expert_weights(self.cfg, self.seed, e, self.device)
+            r = self.raw[e] if self.raw is not None else wl.expert_weights(self.cfg, self.weight_seed, e, self.device)
             self._host[e] = {k: wl.bits(v) for k, v in r.items()}
         return self._host[e]
 

@@ -391,6 +391,68 @@ def test_forward_offload_small(H, mode):
         L.close()
 
 
+@pytest.mark.parametrize("mode", ["dense", "cir"])
+def test_lfu_cache_multi_layer_decode_loop(H, mode):
+    """a two-layer decode loop over an LFU expert cache smaller than the two
+    layers' working set (12 slots; the skewed router touches ~21 of the 2 x 64 keys).  Closed loop against the oracle: at every (step, layer)
+    the oracle's cache gives the residency its cost model sees, its decisions give the executed
+    experts, its LFU rules the fetches and evictions — the library must make the same decisions,
+    fetch exactly the oracle's misses, hold the same keys with the same frequencies in the same
+    slots, and produce the all-resident oracle's y."""
+    from oracle.lfu_cache import LFUCache
+    from paper_2606_29982_b200 import binding as B
+    n_slots, n_layers, n_steps, T = 12, 2, 6, 8
+    cache = B.caee_cache_create(n_slots)
+    layers = [_layer(H, C5S, seed=l, max_tokens=T, kernel=B.CAEE_KERNEL_UMMA, cache=cache, layer_id=l) for l in range(n_layers)]
+    ref = LFUCache(n_slots)
+    try:
+        m, theta = (None, 0.0) if mode == "dense" else MODES[mode]
+        params = None if mode == "dense" else B.prune_params(m, theta)
+        fetched_total = 0
+        for step in range(n_steps):
+            for l, L in enumerate(layers):
+                x = wl.hidden(L.cfg, T, 1000 + 10 * step + l, L.device)
+                s = L.oracle_scores(x)
+                L.resident = np.array(ref.resident_mask(l, L.cfg.E), np.uint8)      # R33
+                d = L.oracle_decisions(s, m, theta)
+                executed = [int(e) for e in d["compact"]["expert_ids"]]
+                fetched, _ = ref.step(l, executed)
+                y, st = L.forward(x, params, torch.from_numpy(s).to(L.device), want_stats=True)
+                idx_g, _ = L.last_routing(T)
+                assert np.array_equal(idx_g, d["idx"]), (step, l)
+                assert st.n_fetch == len(fetched) and st.h2d_bytes == len(fetched) * L.cfg.expert_bytes, (step, l)
+                if mode != "dense":
+                    assert st.F_cost == d["prune"]["F_cost"] and st.n_keep == d["prune"]["n_keep"], (step, l)
+                assert B.caee_cache_snapshot(cache, n_slots) == ref.snapshot(), (step, l)
+                H.check_y(y, L.oracle_y(x, d["idx"], d["gate"], range(T)), range(T), H.TOL[L.cfg.w_dtype])
+                fetched_total += len(fetched)
+        cs = B.caee_cache_read_stats(cache)
+        assert (cs.hits, cs.misses, cs.evictions) == (ref.hits, ref.misses, ref.evictions)
+        assert cs.misses == fetched_total and ref.evictions > 0 and ref.hits > 0
+        # the residency of an attached layer is the cache's state
+        with pytest.raises(B.CaeeError):
+            B.caee_set_residency(layers[0].ctx, np.ones(C5S.E, np.uint8))
+    finally:
+        for L in layers:
+            L.close()
+        B.caee_cache_destroy(cache)
+
+
+def test_lfu_cache_too_small_is_an_error(H):
+    """A step whose executed experts outnumber the slots fails with CAEE_ESTATE (R32)."""
+    from paper_2606_29982_b200 import binding as B
+    cache = B.caee_cache_create(3)
+    L = _layer(H, C5S, seed=0, max_tokens=8, kernel=B.CAEE_KERNEL_UMMA, cache=cache, layer_id=5)
+    try:
+        x = wl.hidden(L.cfg, 8, 1, L.device)
+        with pytest.raises(B.CaeeError) as ei:
+            L.forward(x)
+        assert ei.value.code == B.CAEE_ESTATE
+    finally:
+        L.close()
+        B.caee_cache_destroy(cache)
+
+
 @pytest.mark.parametrize("T,mode", [(128, "frac"), (8, "dense"), (1, "frac")])
 def test_forward_c4_full_size_sampled(H, T, mode):
     """Config 4 (DeepSeek-R1-shaped, FP8 E4M3 weights + 128x128 block scales, 11.3 GB)."""
