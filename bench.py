@@ -346,6 +346,75 @@ def run_caee(args, cfg, prune):
     print(json.dumps(out))
 
 
+# --------------------------------------------------------------------------- NEXT-1: LFU cache decode loop
+def run_cache_loop(args, cfg):
+    """SURVEY.md §8(f) NEXT-1 (Table II): a multi-layer decode loop over an LFU expert
+    cache.  Every routed expert of every layer lives in pinned host memory; `--cache-slots` device
+    slots are shared by the layers.  The settings (dense baseline, CIR theta_imp = 0.9 / 0.8 / 0.7) run
+    one after the other on the same cache; each is warmed for --warmup steps (which re-converges the
+    cache contents to that setting) and timed for --steps steps (one step = T tokens through all
+    layers, the same token batches for every setting); reported: ms per step (the TPOT proxy), misses and H2D bytes per step, the
+    achieved H2D rate.  Synthetic stand-in for the paper's 58-layer DeepSeek-R1 run: layers share the
+    layer shape and differ in router and weights (seeds), token batches change every step."""
+    import torch
+    from paper_2606_29982_b200 import binding as B
+    from paper_2606_29982_b200 import workloads as wl
+    from paper_2606_29982_b200.layer import Layer
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libcaee has no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = "cuda:0"
+    T, K, W, NL = args.tokens, args.steps, max(args.warmup, 3), args.layers
+    cache = B.caee_cache_create(args.cache_slots)
+    layers = [Layer(cfg, seed=l, max_tokens=max(T, 16), device=dev, cache=cache, layer_id=l) for l in range(NL)]
+    xs = [wl.hidden(cfg, T, 5000 + i, dev) for i in range(W + K)]
+    y = torch.empty_like(xs[0])
+    stats = B.stats_buffer(dev)
+    stream = torch.cuda.current_stream()
+    rows = []
+    try:
+        for name, params in (("dense", None), ("cir:0.9", B.prune_params(2, 0.9)), ("cir:0.8", B.prune_params(2, 0.8)),
+                             ("cir:0.7", B.prune_params(2, 0.7))):
+            def step(i):
+                h = xs[i]
+                for L in layers:
+                    L.forward(h, params, y=y, stats=stats)     # x -> every layer (layers are independent MoE blocks here)
+            for i in range(W):
+                step(i)
+            torch.cuda.synchronize()
+            c0 = B.caee_cache_read_stats(cache)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for i in range(W, W + K):
+                step(i)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / K
+            c1 = B.caee_cache_read_stats(cache)
+            miss, hit = (c1.misses - c0.misses) / K, (c1.hits - c0.hits) / K
+            h2d = (c1.h2d_bytes - c0.h2d_bytes) / K
+            rows.append({"setting": name, "ms_per_step": ms, "misses_per_step": miss, "hits_per_step": hit,
+                         "h2d_gb_per_step": h2d / 1e9, "h2d_gbs": h2d / (ms * 1e-3) / 1e9})
+    finally:
+        for L in layers:
+            L.close()
+        B.caee_cache_destroy(cache)
+    base = rows[0]["ms_per_step"]
+    for r in rows:
+        r["vs_dense"] = r["ms_per_step"] / base
+    print(json.dumps({
+        "metric": "cached_decode_step_ms", "value": rows[2]["ms_per_step"], "unit": "ms/step", "n_gpus": 1, "steps": K,
+        "warmup": W, "higher_is_better": False, "vs_baseline": None, "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.w_dtype],
+        "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: {NL} layers x (E={cfg.E}+{cfg.S}, H={cfg.H}, I={cfg.I}, top-{cfg.k}), LFU cache of "
+                               f"{args.cache_slots} slots x {cfg.expert_bytes / 1e6:.1f} MB, T={T} tokens per step; value = CIR 0.8"},
+        "roofline": {"bound": "pcie", "achieved": rows[0]["h2d_gbs"], "unit": "GB/s", "peak": 55.6,
+                     "peak_source": "caee_calibrate_cost H2D tier on this pool's B200 (DESIGN.md §4)",
+                     "frac": rows[0]["h2d_gbs"] / 55.6, "traffic": None},
+        "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -356,11 +425,16 @@ def main():
     ap.add_argument("--tokens", type=int, default=128)
     ap.add_argument("--prune", default="thresh:0.6", help="dense | none | thresh:θ | cir:θ_imp | rank:b | frac:p")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cache-loop", action="store_true", help="SURVEY §8(f) NEXT-1: multi-layer decode loop over an LFU expert cache")
+    ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--cache-slots", type=int, default=128)
     args = ap.parse_args()
     from paper_2606_29982_b200 import workloads as wl
     cfg = wl.CONFIGS[args.workload.upper()]
     prune = parse_prune(args.prune)
-    if args.impl == "reference":
+    if args.cache_loop:
+        run_cache_loop(args, cfg)
+    elif args.impl == "reference":
         run_reference(args, cfg, prune)
     else:
         run_caee(args, cfg, prune)
