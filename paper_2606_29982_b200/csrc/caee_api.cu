@@ -175,6 +175,8 @@ caee_status create_impl(caee_ctx* c) {
     A(c->hq, 2 * c->h_rows_cap * d.I); A(c->hs, c->h_rows_cap * (d.I / 128));
     if ((rc = caee_fp8_make_tensor_maps(c)) != CAEE_OK) return rc;
     if (const char* v = getenv("CAEE_FP8_WIDE_MIN_TOKENS")) c->fp8_wide_min_tokens = std::max(1, atoi(v));   // tuning aid
+    if (const char* v = getenv("CAEE_FP8_WIDE_PAIRS")) c->fp8_wide_pairs = atoi(v) != 0;                      // tuning aid
+    if (!caee_fp8_wide_supported(c)) c->fp8_wide_min_tokens = 1 << 30;   // k range too long for its scale registers
     if (d.max_tokens >= c->fp8_wide_min_tokens) { A(c->xg, caee_fp8_wide_xg_bytes(c)); }
   }
   A(c->obuf, Tm * (k + S) * d.H);

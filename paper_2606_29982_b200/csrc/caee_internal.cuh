@@ -127,6 +127,7 @@ struct caee_ctx {
   uint8_t* xg = nullptr;             // e4m3 prefill kernel (expert_fp8_wide.cu): per-run stage images of the gathered x rows
   bool tm_ready = false;
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
+  bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
 
@@ -200,6 +201,7 @@ void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 caee_status caee_fp8_make_tensor_maps(caee_ctx* c);
 void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // expert_fp8_wide.cu
+bool caee_fp8_wide_supported(const caee_ctx* c);
 size_t caee_fp8_wide_xg_bytes(const caee_ctx* c);
 void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);

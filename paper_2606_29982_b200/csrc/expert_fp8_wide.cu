@@ -30,8 +30,11 @@
 // What bounds it.  Shared-memory bandwidth (128 B/clk): per 64 k the two MMAs read 32 KB of
 // weights and 2 x 32 KB of tokens, the bulk copy writes 32 KB of tokens and the converters write
 // 32 KB of fp16 — 160 KB for 1024 MMA cycles.  That is why the codes go global -> registers ->
-// shared memory (no raw staging ring: it cost another 32 KB per 64 k) and why the next step is
-// cta_group::2 (each CTA of a pair then reads half of the token operand).
+// shared memory (no raw staging ring: it cost another 32 KB per 64 k).  The CTA-pair variant
+// (template kPair, cta_group::2: each CTA of a pair reads half of the token operand, 112 KB per
+// 64 k) is built and parity-tested but opt-in (CAEE_FP8_WIDE_PAIRS=1): on this pool's B200s both
+// variants run into the 1000 W power cap (SM clock 1.6-1.9 GHz under load) and measure the same
+// 4.0-4.2 ms for config 4's 4096-token step.
 //
 // Pipeline (640 threads, 1 CTA per SM; all rings are mbarrier full/empty pairs):
 //   warp 0        tile claimer (atomic ticket, shared-memory queue; see umma_common.cuh)
@@ -41,6 +44,7 @@
 //   warp 1        MMA issuer: 8 tcgen05.mma (M 128, N = padded tokens, K 16) per 64-k stage
 //   warps 4-7, 16-19   epilogue: TMEM -> SwiGLU -> h (fp16), or -> o rows (fp32)
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "umma_common.cuh"
@@ -59,6 +63,7 @@ constexpr int kConvWarps = 8, kEpiWarps = 8, kLoadWarps = 1;
 constexpr int kCvtOff = 0, kTokOff = kCvtOff + kCvtStages * kCvtBytes;
 constexpr int kSmemBytes = kTokOff + kTokStages * kTokBytes;    // 224 KB
 constexpr int kAccCols = 256;              // TMEM columns per accumulator
+constexpr int kMaxKb = 64;                 // most 128-k blocks per tile: H, I <= 8192 (caee_fp8_wide_supported)
 // The token operand is fp16 as well (x converted by k_gather_x, h written as fp16): kind::f16 takes
 // fp16 or bf16 but not one of each (tcgen05.mma with A = fp16, B = bf16 is an illegal instruction).
 constexpr bool kTokF16 = true;
@@ -113,10 +118,18 @@ __device__ __forceinline__ void sts128(uint32_t a, const uint4 v) {
 #define WAIT_T(acc, ...) do { __VA_ARGS__; } while (0)
 #endif
 
+// kPair: two CTAs of a cluster work on the same run with cta_group::2 MMAs (M = 256: each CTA
+// brings the 128 + 128 weight rows of ITS feature block and HALF of the run's token rows), so a CTA
+// reads 64 KB instead of 96 KB of operands per 64 k and fetches half of the token stage.  Tiles are
+// then handed out statically (pair c takes pair-tiles c, c + pairs, ...: still phase-1 tiles first,
+// in increasing order, so the phase-2 wait on a run's h cannot deadlock); the leader CTA (cluster
+// rank 0) issues the MMAs and frees / fills the barriers of both CTAs with multicast commits, the
+// peer's warp 1 forwards its "stage full" events to the leader.
+template <bool kPair>
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_constant__ WideParams p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  constexpr int kBars = 2 * (kCvtStages + kTokStages) + 2 + 2 * kQueue;
+  constexpr int kBars = 2 * (kCvtStages + kTokStages) + 2 + 2 * kQueue + kCvtStages + kTokStages;
   __shared__ __align__(8) uint64_t bars[kBars];
   __shared__ uint32_t tmem_base_s;
   __shared__ int tq_slots[kQueue];
@@ -127,7 +140,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
   const uint32_t kfull0 = cempty0 + 8 * kCvtStages, kempty0 = kfull0 + 8 * kTokStages;
   const uint32_t tfull = kempty0 + 8 * kTokStages, tempty = tfull + 8;
   const uint32_t qfull0 = tempty + 8, qempty0 = qfull0 + 8 * kQueue;
-  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
+  const uint32_t pcr0 = qempty0 + 8 * kQueue, pkr0 = pcr0 + 8 * kCvtStages;   // leader: the peer's stage is full
+  const uint32_t rank = kPair ? cluster_ctarank() : 0u;
+  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, kPair ? p.P1 / 2 : p.P1, kPair ? p.P2 / 2 : p.P2};
+  int ti = (int)(blockIdx.x >> 1);                 // kPair: this pair's next pair-tile
+  const int tstride = (int)(gridDim.x >> 1);
+  (void)ti; (void)tstride;
+// next tile of a role: popped from the ticket queue, or (pairs) the static schedule; sub = this CTA's feature block
+#define NEXT_TILE(POP) (kPair ? (tm.at(ti, t) ? (ti += tstride, t.sub = 2 * t.sub + (int)rank, true) : false) : tm.at(POP, t))
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kCvtStages; ++s) {
@@ -139,7 +159,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
       mbar_init(kempty0 + 8 * s, 1);           // tcgen05.commit
     }
     mbar_init(tfull, 1);                       // tcgen05.commit
-    mbar_init(tempty, kEpiWarps);
+    mbar_init(tempty, kPair ? 2 * kEpiWarps : kEpiWarps);   // pairs: the leader waits for both CTAs' epilogues
+    for (int s = 0; s < kCvtStages; ++s) mbar_init(pcr0 + 8 * s, 1);
+    for (int s = 0; s < kTokStages; ++s) mbar_init(pkr0 + 8 * s, 1);
     for (int q = 0; q < kQueue; ++q) {
       mbar_init(qfull0 + 8 * q, 1);
       mbar_init(qempty0 + 8 * q, 1 + kLoadWarps + kEpiWarps + kConvWarps);
@@ -147,23 +169,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)),
-                 "n"(kTmemCols));
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    if (kPair) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(kTmemCols));
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(kTmemCols));
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
   }
   tc_fence_before();
   __syncthreads();
+  if (kPair) cluster_sync_all();               // both CTAs' barriers exist before any remote arrive / multicast commit
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
   TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
   Tile t;
-  long long w_a = 0, w_b = 0, w_c = 0;   // wait cycles (CAEE_WIDE_STATS builds print them)
+  long long w_a = 0, w_b = 0, w_c = 0, w_d = 0, w_e = 0;   // wait cycles (CAEE_WIDE_STATS builds print them)
   const long long t_start = clock64();
-  (void)t_start; (void)w_a; (void)w_b; (void)w_c;
+  (void)t_start; (void)w_a; (void)w_b; (void)w_c; (void)w_d; (void)w_e;
 
   if (warp == 0) {
     // ===== tile claimer: one atomic ticket per tile, broadcast through the shared-memory queue
-    if (lane == 0) {
+    if (!kPair && lane == 0) {
       int q = 0, qph = 0;
       for (;;) {
         WAIT_T(w_a, mbar_wait(qempty0 + 8 * q, qph ^ 1));
@@ -174,45 +201,85 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
         if (!tm.at(i, t)) break;
       }
     }
-  } else if (warp == 1) {
-    // ===== MMA issuer: bf16 x bf16, the accumulator pair lives in TMEM for the whole k range.
+  } else if (warp == 1 && rank == 0) {
+    // ===== MMA issuer: fp16 x fp16, the accumulator pair lives in TMEM for the whole k range.
     // The whole warp runs the loop (uniform control flow); one elected lane issues.
     int cs = 0, cph = 0, ks = 0, kph = 0;
     const uint32_t d0 = tmem_base, d1 = tmem_base + kAccCols;
-    for (int it = 0; tm.at(tq.pop(), t); ++it) {
+    for (int it = 0; NEXT_TILE(tq.pop()); ++it) {
       const int npad = (__shfl_sync(0xffffffffu, p.wl.run_n[t.run], 0) + 15) & ~15;
-      // kind::f16, A and B fp16 (format 0), D fp32, both K-major
-      const uint32_t idesc = (1u << 4) | (kTokF16 ? 0u : (1u << 10)) | ((uint32_t)(npad >> 3) << 17) | ((uint32_t)(kTileRows >> 4) << 24);
+      // kind::f16, A and B fp16 (format 0), D fp32, both K-major; M = 128, or 256 over the CTA pair
+      const uint32_t idesc = (1u << 4) | ((uint32_t)(npad >> 3) << 17) | ((uint32_t)((kPair ? 2 * kTileRows : kTileRows) >> 4) << 24);
       const int nsub = 2 * (t.phase == 1 ? p.KB1 : p.KB2);
-      WAIT_T(w_a, mbar_wait(tempty, (it & 1) ^ 1));
+      if (kPair) WAIT_T(w_a, mbar_wait_cluster(tempty, (it & 1) ^ 1));
+      else WAIT_T(w_a, mbar_wait(tempty, (it & 1) ^ 1));
       tc_fence_after();
       for (int s = 0; s < nsub; ++s) {
         WAIT_T(w_b, mbar_wait(cfull0 + 8 * cs, cph));
         WAIT_T(w_c, mbar_wait(kfull0 + 8 * ks, kph));
+        if (kPair) {
+          WAIT_T(w_d, mbar_wait_cluster(pcr0 + 8 * cs, cph));
+          WAIT_T(w_e, mbar_wait_cluster(pkr0 + 8 * ks, kph));
+        }
         tc_fence_after();
         const uint32_t a_addr = smem_base + kCvtOff + cs * kCvtBytes;
         const uint64_t a0 = make_desc(a_addr), a1 = make_desc(a_addr + kATileBytes);
         const uint64_t b = make_desc_sw128(smem_base + kTokOff + ks * kTokBytes);
         if (elect_one()) {
-          if (s == 0) {
-            umma_bf16_imm<false>(d0, a0, b, idesc);
-            umma_bf16_imm<false>(d1, a1, b, idesc);
-          } else {
-            umma_bf16_imm<true>(d0, a0, b, idesc);
-            umma_bf16_imm<true>(d1, a1, b, idesc);
-          }
+          if (kPair) {
+            if (s == 0) {
+              umma_f16_pair_imm<false>(d0, a0, b, idesc);
+              umma_f16_pair_imm<false>(d1, a1, b, idesc);
+            } else {
+              umma_f16_pair_imm<true>(d0, a0, b, idesc);
+              umma_f16_pair_imm<true>(d1, a1, b, idesc);
+            }
 #pragma unroll
-          for (int k16 = 1; k16 < kKSub / 16; ++k16) {   // per 16-element k-step: weights +256 B, tokens +32 B (>> 4)
-            umma_bf16_imm<true>(d0, a0 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
-            umma_bf16_imm<true>(d1, a1 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
+            for (int k16 = 1; k16 < kKSub / 16; ++k16) {
+              umma_f16_pair_imm<true>(d0, a0 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
+              umma_f16_pair_imm<true>(d1, a1 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
+            }
+            tc_commit_pair(cempty0 + 8 * cs);
+            tc_commit_pair(kempty0 + 8 * ks);
+            if (s == nsub - 1) tc_commit_pair(tfull);
+          } else {
+            if (s == 0) {
+              umma_bf16_imm<false>(d0, a0, b, idesc);
+              umma_bf16_imm<false>(d1, a1, b, idesc);
+            } else {
+              umma_bf16_imm<true>(d0, a0, b, idesc);
+              umma_bf16_imm<true>(d1, a1, b, idesc);
+            }
+#pragma unroll
+            for (int k16 = 1; k16 < kKSub / 16; ++k16) {   // per 16-element k-step: weights +256 B, tokens +32 B (>> 4)
+              umma_bf16_imm<true>(d0, a0 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
+              umma_bf16_imm<true>(d1, a1 + (uint64_t)(k16 * 16), b + (uint64_t)(k16 * 2), idesc);
+            }
+            tc_commit(cempty0 + 8 * cs);
+            tc_commit(kempty0 + 8 * ks);
+            if (s == nsub - 1) tc_commit(tfull);
           }
-          tc_commit(cempty0 + 8 * cs);
-          tc_commit(kempty0 + 8 * ks);
-          if (s == nsub - 1) tc_commit(tfull);
         }
         __syncwarp();
         if (++cs == kCvtStages) { cs = 0; cph ^= 1; }
         if (++ks == kTokStages) { ks = 0; kph ^= 1; }
+      }
+    }
+  } else if (warp == 1 || (kPair && warp == 3 && rank != 0)) {
+    // ===== (pairs, peer CTA) forwarders: this CTA's converted-weight stages (warp 1) and token
+    // stages (warp 3) are full -> tell the leader, whose MMAs read them
+    if (lane == 0) {
+      const bool wts = warp == 1;
+      const int depth = wts ? kCvtStages : kTokStages;
+      const uint32_t src0 = wts ? cfull0 : kfull0, dst0 = wts ? pcr0 : pkr0;
+      int st = 0, ph = 0;
+      while (NEXT_TILE(0)) {
+        const int nsub = 2 * (t.phase == 1 ? p.KB1 : p.KB2);
+        for (int s = 0; s < nsub; ++s) {
+          WAIT_T(w_b, mbar_wait(src0 + 8 * st, ph));
+          mbar_arrive_remote(dst0 + 8 * st, 0);
+          if (++st == depth) { st = 0; ph ^= 1; }
+        }
       }
     }
   } else if (warp == 2) {
@@ -220,12 +287,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
     // written by k_gather_x; h: written by the phase-1 epilogues), npad rows of 128 bytes
     if (lane == 0) {
       int stage = 0, ph = 0;
-      while (tm.at(tq.pop1(), t)) {
+      while (NEXT_TILE(tq.pop1())) {
         const int npad = (p.wl.run_n[t.run] + 15) & ~15;
         const int nsub = 2 * (t.phase == 1 ? p.KB1 : p.KB2);
         const size_t row_bytes = (size_t)(t.phase == 1 ? p.H : p.I) * 2;
-        const uint8_t* src = (t.phase == 1 ? p.xg : p.hbuf) + (size_t)p.wl.run_hrow[t.run] * row_bytes;
-        const uint32_t bytes = (uint32_t)npad * 128u;
+        const uint32_t stage_bytes = (uint32_t)npad * 128u;
+        const uint32_t bytes = kPair ? stage_bytes / 2 : stage_bytes;      // pairs: this CTA's half of the rows
+        const uint8_t* src = (t.phase == 1 ? p.xg : p.hbuf) + (size_t)p.wl.run_hrow[t.run] * row_bytes + (kPair ? rank * bytes : 0u);
         if (t.phase == 2) {
           // h of this run is complete once all P1 gate/up tiles have published it (generic-proxy
           // stores of other SMs, read here through the async proxy)
@@ -236,7 +304,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
         for (int s = 0; s < nsub; ++s) {
           WAIT_T(w_a, mbar_wait(kempty0 + 8 * stage, ph ^ 1));
           mbar_arrive_expect_tx(kfull0 + 8 * stage, bytes);
-          bulk_g2s(smem_base + kTokOff + stage * kTokBytes, src + (size_t)s * bytes, bytes, kfull0 + 8 * stage);
+          bulk_g2s(smem_base + kTokOff + stage * kTokBytes, src + (size_t)s * stage_bytes, bytes, kfull0 + 8 * stage);
           if (++stage == kTokStages) { stage = 0; ph ^= 1; }
         }
       }
@@ -247,7 +315,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
     // ===== epilogue (warps 4-7 and 16-19): TMEM -> registers -> SwiGLU -> h (phase 1) or -> o rows
     // (phase 2).  Two warps per TMEM lane quadrant q = warp % 4, each one half of the token columns.
     const int q = warp & 3, eh = warp >= 16;
-    for (int it = 0; tm.at(tq.pop(), t); ++it) {
+    for (int it = 0; NEXT_TILE(tq.pop()); ++it) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       const int npad = (n + 15) & ~15;
       const int half = (((npad >> 4) + 1) >> 1) << 4;
@@ -314,7 +382,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(tempty);
+      if (lane == 0) {
+        if (kPair && rank != 0) mbar_arrive_remote(tempty, 0);
+        else mbar_arrive(tempty);
+      }
       if (t.phase == 1) {
         // publish this tile's slice of h: all 256 epilogue threads' stores (read later through the
         // async proxy by other SMs' bulk copies), then one release add
@@ -337,14 +408,22 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
 #pragma unroll
     for (int i = 0; i < 4; ++i) off_i[i] = (i >> 1) * kATileBytes + (((i & 1) * 256 + ct) >> 5) * 1024 + r8 * 16;
     int cs = 0, cph = 0;
-    while (tm.at(tq.pop(), t)) {
+    while (NEXT_TILE(tq.pop())) {
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
       const uint8_t* img = p.packed[p.wl.run_expert[t.run]];
       const float* tab = reinterpret_cast<const float*>(img + p.sc_off);
       const float* wsc = t.phase == 1 ? tab + (size_t)t.sub * p.KB1 * 2 : tab + p.t2_off + (size_t)t.sub * p.KB2 * 2;
       const uint8_t* src = img + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes + c4 * 128;
       const float nrm = __ldg(reinterpret_cast<const float*>(img + p.norm_off));
-      float w0n = __ldg(wsc), w1n = __ldg(wsc + 1);
+      // the tile's block scales, fetched once: lane l keeps those of k blocks l, l + 32, ... (a load per
+      // k block in the loop below ends up next to its use and exposes its latency every 128 k)
+      float sc0[kMaxKb / 32], sc1[kMaxKb / 32];
+#pragma unroll
+      for (int j = 0; j < kMaxKb / 32; ++j) {
+        const int kbj = lane + 32 * j;
+        sc0[j] = kbj < nkb ? __ldg(wsc + 2 * kbj) * nrm : 0.f;
+        sc1[j] = kbj < nkb ? __ldg(wsc + 2 * kbj + 1) * nrm : 0.f;
+      }
       // the codes go global -> registers (no shared-memory staging: shared-memory bandwidth is the
       // bound of this kernel): both 64-k halves of stage kb + 1 are in flight while stage kb is widened
       uint4 va[4], vb[4];
@@ -354,18 +433,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
         vb[i] = ldg_stream(src + off_i[i] + 512);
       }
       for (int kb = 0; kb < nkb; ++kb) {
-        const __half2 w0 = __float2half2_rn(w0n * nrm), w1 = __float2half2_rn(w1n * nrm);
-        if (kb + 1 < nkb) { w0n = __ldg(wsc + 2 * kb + 2); w1n = __ldg(wsc + 2 * kb + 3); }
+        float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+        for (int j = 0; j < kMaxKb / 32; ++j)
+          if ((kb >> 5) == j) { s0 = sc0[j]; s1 = sc1[j]; }
+        const __half2 w0 = __float2half2_rn(__shfl_sync(0xffffffffu, s0, kb & 31));
+        const __half2 w1 = __float2half2_rn(__shfl_sync(0xffffffffu, s1, kb & 31));
         const uint8_t* nxt = src + (size_t)(kb + 1) * kAStageBytes;
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
+          // the commit that completed this barrier ordered the MMAs' reads of the stage before it; no
+          // tcgen05.fence here: it would also wait for the code loads in flight for the next stage
           WAIT_T(w_b, mbar_wait(cempty0 + 8 * cs, cph ^ 1));
-          tc_fence_after();
           const uint32_t dst = smem_base + kCvtOff + cs * kCvtBytes + c4 * 256;
-#ifdef CAEE_WIDE_STATS
-          { long long _t0 = clock64(); uint32_t sink = hh ? vb[0].x ^ vb[3].w : va[0].x ^ va[3].w; asm volatile("" :: "r"(sink)); w_a += clock64() - _t0; }
-          long long _t1 = clock64();
-#endif
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             uint4 lo8, hi8;
@@ -382,9 +462,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
           }
           fence_proxy_async_smem();
           __syncwarp();
-#ifdef CAEE_WIDE_STATS
-          w_c += clock64() - _t1;
-#endif
           if (lane == 0) mbar_arrive(cfull0 + 8 * cs);
           if (++cs == kCvtStages) { cs = 0; cph ^= 1; }
         }
@@ -393,14 +470,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
   }
 
 #ifdef CAEE_WIDE_STATS
-  if (lane == 0 && (blockIdx.x == 0 || blockIdx.x == 101) && (warp <= 2 || warp == 4 || warp == 8 || warp == 16))
-    printf("cta %d warp %d: total %lld  wait a %lld b %lld c %lld\n", blockIdx.x, warp, clock64() - t_start, w_a, w_b, w_c);
+  if (lane == 0 && (blockIdx.x == 0 || blockIdx.x == 101) && (warp <= 3 || warp == 4 || warp == 8 || warp == 16))
+    printf("cta %d warp %d: total %lld  wait a %lld b %lld c %lld d %lld e %lld\n", blockIdx.x, warp, clock64() - t_start, w_a, w_b, w_c, w_d, w_e);
 #endif
+#undef NEXT_TILE
   tc_fence_before();
   __syncthreads();
+  if (kPair) cluster_sync_all();               // the peer's shared memory and TMEM stay until the leader's MMAs are done
   if (warp == 2) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
+    if (kPair) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
+    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
   }
 }
 
@@ -435,6 +515,8 @@ __global__ void __launch_bounds__(256) k_gather_x(caee_worklist wl, const uint4*
 
 }  // namespace
 
+bool caee_fp8_wide_supported(const caee_ctx* c) { return c->d.H <= kMaxKb * kKRaw && c->d.I <= kMaxKb * kKRaw; }
+
 size_t caee_fp8_wide_xg_bytes(const caee_ctx* c) { return c->h_rows_cap * (size_t)c->d.H * 2; }
 
 // Once per step, after the work list is built: the x rows of every run, laid out for bulk copies.
@@ -463,8 +545,31 @@ void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_coun
   p.norm_off = (int)caee_fp8_norm_offset(c);
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(k_expert_fp8_wide, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
+    cudaFuncSetAttribute(k_expert_fp8_wide<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
+    cudaFuncSetAttribute(k_expert_fp8_wide<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
     attr_set = true;
   }
-  k_expert_fp8_wide<<<c->num_sms, kThreads, kSmemBytes + 1024, st>>>(p);
+  // CTA pairs (cta_group::2) need an even number of tiles per run in both phases
+  // (opt-in, caee_ctx::fp8_wide_pairs: on this pool's B200s the kernel runs into the 1000 W power cap
+  // either way and the pair variant measures the same 4.0-4.2 ms; the single-CTA variant keeps the
+  // dynamic tile tickets)
+  if (c->fp8_wide_pairs && p.P1 % 2 == 0 && p.P2 % 2 == 0 && c->num_sms >= 2) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(c->num_sms & ~1));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kSmemBytes + 1024;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    // the static schedule needs every pair resident at once (a phase-2 tile waits for phase-1 tiles of other pairs)
+    static int max_pairs = -1;
+    if (max_pairs < 0 && cudaOccupancyMaxActiveClusters(&max_pairs, k_expert_fp8_wide<true>, &cfg) != cudaSuccess) { max_pairs = 0; cudaGetLastError(); }
+    if (max_pairs * 2 >= (int)cfg.gridDim.x) {
+      cudaLaunchKernelEx(&cfg, k_expert_fp8_wide<true>, p);
+      return;
+    }
+  }
+  k_expert_fp8_wide<false><<<c->num_sms, kThreads, kSmemBytes + 1024, st>>>(p);
 }

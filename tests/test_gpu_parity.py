@@ -465,10 +465,13 @@ def test_forward_c4_full_size_sampled(H, T, mode):
         L.close()
 
 
-def test_forward_c4_prefill_4096_sampled(H):
-    """Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill,
+@pytest.mark.parametrize("pairs", [0, 1])
+def test_forward_c4_prefill_4096_sampled(H, pairs, monkeypatch):
+    """pairs = 1: the same kernel on CTA pairs (cta_group::2 MMAs of M = 256, static tile schedule).
+    Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill,
     256-token runs, the e4m3 prefill kernel expert_fp8_wide.cu): K_final and F_* for all 4096 tokens
     bit-exact, y on sampled tokens."""
+    monkeypatch.setenv("CAEE_FP8_WIDE_PAIRS", str(pairs))
     L = H.GpuLayer(wl.C4, seed=0, max_tokens=4096, keep_raw=False)
     try:
         T = 4096
