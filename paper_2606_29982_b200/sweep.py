@@ -1,0 +1,82 @@
+"""Knob sweep of one CAEE layer: the paper's THRESH grid θ ∈ [0.3, 1.2]
+(on-device inference) and CIR grid θ_imp ∈ {0.9, 0.8, 0.7} (offloading)
+across decode batch sizes, with a Fig. 10-style per-partition load report (Fig. 10:
+expert cost per device before and after pruning).
+
+    python -m paper_2606_29982_b200.sweep --workload c3 --tokens 8,32,64,128 > sweep.md
+
+Everything is measured through the C ABI (caee_moe_forward + caee_fwd_stats); this module only
+marshals arguments and formats the table.  Latency = CUDA events around `--steps` calls after
+`--warmup` calls, rotating over 4 seeded token batches; the per-partition columns are the summed
+C~ ticks of the experts each partition keeps (stats.load) on the first batch.
+"""
+import argparse
+import statistics
+
+import torch
+
+from . import binding as B
+from . import workloads as wl
+from .layer import Layer
+
+
+def measure(L, xs, params, steps, warmup):
+    dev = L.device
+    y = torch.empty_like(xs[0])
+    stats = B.stats_buffer(dev)
+    for i in range(warmup):
+        L.forward(xs[i % len(xs)], params, y=y, stats=stats)
+    L.forward(xs[0], params, y=y, stats=stats)
+    torch.cuda.synchronize()
+    st0 = B.read_stats(stats)
+    ms = []
+    for i in range(steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        L.forward(xs[i % len(xs)], params, y=y, stats=stats)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    return statistics.median(ms) * 1e3, st0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", default="c3", choices=["c2", "c3", "c4"])
+    ap.add_argument("--tokens", default="8,32,64,128")
+    ap.add_argument("--thresh", default="0.3,0.6,0.8,1.0,1.2")
+    ap.add_argument("--cir", default="0.9,0.8,0.7")
+    ap.add_argument("--steps", type=int, default=12)
+    ap.add_argument("--warmup", type=int, default=3)
+    args = ap.parse_args()
+    cfg = wl.CONFIGS[args.workload.upper()]
+    Ts = [int(t) for t in args.tokens.split(",")]
+    dev = "cuda:0"
+    L = Layer(cfg, seed=0, max_tokens=max(max(Ts), 128), device=dev)
+    D = cfg.D
+    print(f"# Knob sweep, {cfg.name} (H={cfg.H} I={cfg.I} E={cfg.E}+{cfg.S} top-{cfg.k}, D={D} partitions, "
+          f"partition {cfg.straggler_part} costs 2x)\n")
+    print("| T | setting | step µs | vs dense | experts run | GB read | F_cost ticks (dense → kept) | per-partition load after pruning, % of the dense max |")
+    print("|---|---|---|---|---|---|---|---|")
+    try:
+        for T in Ts:
+            xs = [wl.hidden(cfg, T, 100 + i, dev) for i in range(4)]
+            base_us, st = measure(L, xs, None, args.steps, args.warmup)
+            # dense loads: THRESH θ = 0 keeps every activated expert and reports the loads
+            _, st_d = measure(L, xs, B.prune_params(B.CAEE_PRUNE_THRESH, 0.0), 1, 1)
+            fmax = max(1, st_d.F_cost_dense)
+            loads = " ".join(f"{100 * st_d.load[d] / fmax:.0f}" for d in range(D))
+            print(f"| {T} | dense | {base_us:.0f} | 1.000 | {st.n_run} | {st.weight_bytes / 1e9:.2f} | {st_d.F_cost_dense} | {loads} |")
+            grid = [("thresh", B.CAEE_PRUNE_THRESH, float(v)) for v in args.thresh.split(",") if v] + \
+                   [("cir", B.CAEE_PRUNE_CIR, float(v)) for v in args.cir.split(",") if v]
+            for name, mode, theta in grid:
+                us, s = measure(L, xs, B.prune_params(mode, theta), args.steps, args.warmup)
+                loads = " ".join(f"{100 * s.load[d] / fmax:.0f}" for d in range(D))
+                print(f"| {T} | {name} {theta:g} | {us:.0f} | {us / base_us:.3f} | {s.n_run} (kept {s.n_keep}/{s.n_act}) | "
+                      f"{s.weight_bytes / 1e9:.2f} | {s.F_cost_dense} → {s.F_cost} | {loads} |")
+    finally:
+        L.close()
+
+
+if __name__ == "__main__":
+    main()
