@@ -43,7 +43,7 @@ namespace {
 enum Dtype { DT_F32 = 0, DT_BF16 = 1, DT_E4M3 = 2 };
 enum ScoreFn { SCORE_SOFTMAX = 0, SCORE_SIGMOID = 1 };
 enum PruneMode { MODE_NONE = 0, MODE_THRESH = 1, MODE_CIR = 2, MODE_RANK = 3, MODE_FRAC = 4 };
-enum Flags { FLAG_COMP_ALL_TOKENS = 1, FLAG_KEEP_TOP1 = 2 };
+enum Flags { FLAG_COMP_ALL_TOKENS = 1, FLAG_KEEP_TOP1 = 2, FLAG_COMP_RANDOM = 4 };
 
 const double FIX_ONE = 1099511627776.0;  // 2^40, fixed-point unit of I_fix (reading R-fix)
 
@@ -342,6 +342,26 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
 // Affected tokens only (reading R14) unless FLAG_COMP_ALL_TOKENS; selection score
 // s' = s + corr_bias, no group limit (R13); exclusion, not numeric zero (R17);
 // min(k, |A_trans|) survivors (R15); gates renormalised over K_final (R16).
+//
+// FLAG_COMP_RANDOM is the ablation baseline of PAPER.md:250-256 / Fig. 9 ("we contrast a random
+// selection strategy with the proposed low-overhead compensation mechanism"; SURVEY.md 8(f)
+// NEXT-4).  The paper does not define it; reading R35: an affected token keeps the
+// picks that survived and fills the vacated slots with experts drawn uniformly without
+// replacement from the rest of A_trans.  Written as a Top-k over keys so that it reuses the same
+// selection: key(e) = 2 + u(t,e) for a surviving pick, u(t,e) otherwise, u in [0,1) from a
+// counter-based generator both sides implement (murmur3's 32-bit finalizer over t, e and a fixed
+// constant); gates as in R16 (unbiased scores of the chosen experts, renormalised).
+static uint32_t fmix32(uint32_t h) {
+  h ^= h >> 16; h *= 0x85ebca6bu; h ^= h >> 13; h *= 0xc2b2ae35u; h ^= h >> 16;
+  return h;
+}
+static float unit_draw(int t, int e) {
+  uint32_t h = fmix32(static_cast<uint32_t>(t) * 0x9e3779b1u + static_cast<uint32_t>(e) * 0x85ebca77u + 0x26062998u);
+  return static_cast<float>(h >> 8) * (1.0f / 16777216.0f);
+}
+extern "C" uint32_t oracle_fmix32(uint32_t h) { return fmix32(h); }
+extern "C" float oracle_unit_draw(int t, int e) { return unit_draw(t, e); }
+
 int oracle_compensate(const float* s, const float* corr_bias, const uint8_t* keep, int T, int E,
                       int k, int norm_topk, int flags, int32_t* idx, float* gate) {
   std::vector<float> sp(E);
@@ -353,6 +373,11 @@ int oracle_compensate(const float* s, const float* corr_bias, const uint8_t* kee
     if (!affected) continue;
     const float* sr = s + static_cast<size_t>(t) * E;
     for (int e = 0; e < E; ++e) sp[e] = corr_bias ? sr[e] + corr_bias[e] : sr[e];
+    if (flags & FLAG_COMP_RANDOM) {
+      for (int e = 0; e < E; ++e) sp[e] = unit_draw(t, e);
+      for (int j = 0; j < k; ++j)
+        if (ir[j] >= 0 && keep[ir[j]]) sp[ir[j]] = 2.0f + sp[ir[j]];
+    }
     int c = topk_select(sp.data(), keep, E, k, ir);
     for (int j = c; j < k; ++j) ir[j] = -1;
     gates_for_list(sr, ir, k, norm_topk, gate + static_cast<size_t>(t) * k);

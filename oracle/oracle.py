@@ -16,7 +16,7 @@ from . import build as _build
 DT_F32, DT_BF16, DT_E4M3 = 0, 1, 2
 SCORE_SOFTMAX, SCORE_SIGMOID = 0, 1
 MODE_NONE, MODE_THRESH, MODE_CIR, MODE_RANK, MODE_FRAC = 0, 1, 2, 3, 4
-FLAG_COMP_ALL_TOKENS, FLAG_KEEP_TOP1 = 1, 2
+FLAG_COMP_ALL_TOKENS, FLAG_KEEP_TOP1, FLAG_COMP_RANDOM = 1, 2, 4
 FIX_ONE = float(2 ** 40)
 
 _lib = None
@@ -30,6 +30,10 @@ def lib():
         _lib.oracle_cost_ticks.restype = C.c_int64
         _lib.oracle_cost_ticks.argtypes = [C.c_double, C.c_double, C.c_int64]
         _lib.oracle_e4m3_value.restype = C.c_double
+        _lib.oracle_fmix32.restype = C.c_uint32
+        _lib.oracle_fmix32.argtypes = [C.c_uint32]
+        _lib.oracle_unit_draw.restype = C.c_float
+        _lib.oracle_unit_draw.argtypes = [C.c_int, C.c_int]
     return _lib
 
 
