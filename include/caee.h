@@ -67,7 +67,10 @@ enum {
 };
 enum {
   CAEE_COMP_ALL_TOKENS = 1, /* re-select every token, not only those that lost an expert (R14)       */
-  CAEE_KEEP_TOP1 = 2        /* every token's first expert is mandatory (R23)                          */
+  CAEE_KEEP_TOP1 = 2,       /* every token's first expert is mandatory (R23)                          */
+  CAEE_COMP_RANDOM = 4      /* ablation baseline of PAPER.md:250-256 / Fig. 9 (R35): an affected token
+                               keeps its surviving picks and fills the vacated slots uniformly at random
+                               from the rest of A_trans (counter-based draws, reproducible)            */
 };
 enum { CAEE_KERNEL_AUTO = 0, CAEE_KERNEL_SIMT = 1, CAEE_KERNEL_UMMA = 2 };
 
@@ -107,7 +110,7 @@ typedef struct caee_expert_weights {
 
 typedef struct caee_prune_params {
   int32_t mode;  /* CAEE_PRUNE_*                                                                  */
-  int32_t flags; /* CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1                                         */
+  int32_t flags; /* CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM                      */
   double theta;  /* THRESH: theta in gate units (sum G = 1); CIR: theta_imp in (0,1];
                     RANK: budget b in 0..k; FRAC: p in [0,1]                                     */
 } caee_prune_params;

@@ -21,7 +21,7 @@ CAEE_OK, CAEE_EINVAL, CAEE_ESHAPE, CAEE_EDTYPE, CAEE_ENOMEM, CAEE_ECUDA, CAEE_ES
 CAEE_F32, CAEE_BF16, CAEE_E4M3 = 0, 1, 2
 CAEE_SCORE_SOFTMAX, CAEE_SCORE_SIGMOID = 0, 1
 CAEE_PRUNE_NONE, CAEE_PRUNE_THRESH, CAEE_PRUNE_CIR, CAEE_PRUNE_RANK, CAEE_PRUNE_FRAC = 0, 1, 2, 3, 4
-CAEE_COMP_ALL_TOKENS, CAEE_KEEP_TOP1 = 1, 2
+CAEE_COMP_ALL_TOKENS, CAEE_KEEP_TOP1, CAEE_COMP_RANDOM = 1, 2, 4
 CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",

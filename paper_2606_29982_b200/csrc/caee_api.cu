@@ -90,7 +90,7 @@ caee_status validate_prune(caee_ctx* c, const caee_prune_params* p) {
       break;
     default: return caee_fail(c, CAEE_EINVAL, "unknown prune mode %d", p->mode);
   }
-  if (p->flags & ~(CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1)) return caee_fail(c, CAEE_EINVAL, "unknown prune flags");
+  if (p->flags & ~(CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM)) return caee_fail(c, CAEE_EINVAL, "unknown prune flags");
   return CAEE_OK;
 }
 

@@ -148,7 +148,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
       const bool affected = __any_sync(0xffffffffu, bad) || (p.flags & CAEE_COMP_ALL_TOKENS);
       if (affected) {
         const float* sc = p.scores_in ? p.scores_in : p.scores;
-        caee_compensate_token<NV>(sc + (size_t)t * E, p.corr_bias != nullptr, cb, sm.keep, E, k, p.norm_topk, lane, ir, gr);
+        caee_compensate_token<NV>(sc + (size_t)t * E, p.corr_bias != nullptr, cb, sm.keep, E, k, p.norm_topk, lane, ir, gr,
+                                  (p.flags & CAEE_COMP_RANDOM) != 0, t);
         __syncwarp();
       }
     }

@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ sc
   float cb[NV];
   caee_load_vec<NV>(corr_bias, E, lane, cb);
   caee_compensate_token<NV>(scores + (size_t)t * E, corr_bias != nullptr, cb, keep, E, k, norm_topk, lane, ir,
-                            gate + (size_t)t * k);
+                            gate + (size_t)t * k, (flags & CAEE_COMP_RANDOM) != 0, t);
 }
 
 }  // namespace

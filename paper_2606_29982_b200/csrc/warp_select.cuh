@@ -239,11 +239,22 @@ __device__ __forceinline__ void caee_route_token(const float (&s)[NV], bool has_
   RSTAMP(3);
 }
 
+// Counter-based uniform draw in [0,1) for (token, expert): murmur3's 32-bit finalizer over t, e and
+// a fixed constant (CAEE_COMP_RANDOM, R35).
+__device__ __forceinline__ float caee_unit_draw(int t, int e) {
+  uint32_t h = (uint32_t)t * 0x9e3779b1u + (uint32_t)e * 0x85ebca77u + 0x26062998u;
+  h ^= h >> 16; h *= 0x85ebca6bu; h ^= h >> 13; h *= 0xc2b2ae35u; h ^= h >> 16;
+  return __fmul_rn((float)(h >> 8), 1.0f / 16777216.0f);
+}
+
 // S5 for one token: top-k of s' over the experts of A_trans only, no group limit (R13).
+// random (CAEE_COMP_RANDOM, the ablation baseline of PAPER.md:250-256): the selection key is
+// 2 + u(t,e) for a pick of idx_out that survived and u(t,e) otherwise, so the survivors stay and the
+// vacated slots are filled uniformly from the rest of A_trans; gates as always from s.
 template <int NV>
 __device__ __forceinline__ void caee_compensate_token(const float* __restrict__ scores_row, bool has_cb, const float (&cb)[NV],
                                                       const uint8_t* keep, int E, int k, int norm_topk, int lane,
-                                                      int32_t* idx_out, float* gate_out) {
+                                                      int32_t* idx_out, float* gate_out, bool random = false, int t = 0) {
   float s[NV], sp[NV];
   uint32_t ok = 0;
 #pragma unroll
@@ -252,6 +263,19 @@ __device__ __forceinline__ void caee_compensate_token(const float* __restrict__ 
     s[i] = e < E ? scores_row[e] : 0.f;
     sp[i] = (has_cb && e < E) ? __fadd_rn(s[i], cb[i]) : s[i];
     if (e < E && keep[e]) ok |= 1u << i;
+  }
+  if (random) {
+    const int mine = lane < k ? idx_out[lane] : -1;      // the token's current picks
+#pragma unroll
+    for (int i = 0; i < NV; ++i) sp[i] = caee_unit_draw(t, lane + 32 * i);
+    for (int j = 0; j < k; ++j) {
+      const int ej = __shfl_sync(0xffffffffu, mine, j);
+      if (ej >= 0 && (ej & 31) == lane) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i)
+          if (i == (ej >> 5) && ((ok >> i) & 1u)) sp[i] = __fadd_rn(2.0f, sp[i]);
+      }
+    }
   }
   __syncwarp();
   caee_warp_select<NV>(s, sp, ok, k, norm_topk, lane, idx_out, gate_out);

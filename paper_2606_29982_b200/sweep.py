@@ -40,6 +40,33 @@ def measure(L, xs, params, steps, warmup):
     return statistics.median(ms) * 1e3, st0
 
 
+def ablation(L, cfg, Ts, args):
+    """SURVEY.md §8(f) NEXT-4, PAPER.md:250-256 / Fig. 9: masked Top-k compensation against the random
+    selection baseline (CAEE_COMP_RANDOM).  Task accuracy needs the absent suites and weights; the
+    proxy is the relative L2 distance of the layer output from the dense (unpruned) layer's."""
+    dev = L.device
+    print(f"# Compensation ablation proxy, {cfg.name}: ||y - y_dense|| / ||y_dense|| over the batch\n")
+    print("| T | setting | experts kept | masked Top-k (paper) | random selection | ratio |")
+    print("|---|---|---|---|---|---|")
+    grid = [("cir", B.CAEE_PRUNE_CIR, float(v)) for v in args.cir.split(",") if v] + \
+           [("thresh", B.CAEE_PRUNE_THRESH, float(v)) for v in args.thresh.split(",") if v]
+    for T in Ts:
+        x = wl.hidden(cfg, T, 100, dev)
+        stats = B.stats_buffer(dev)
+        y0 = L.forward(x, None).float()
+        torch.cuda.synchronize()
+        n0 = float(y0.norm())
+        for name, mode, theta in grid:
+            errs = []
+            for flags in (0, B.CAEE_COMP_RANDOM):
+                y = L.forward(x, B.prune_params(mode, theta, flags), stats=stats).float()
+                torch.cuda.synchronize()
+                errs.append(float((y - y0).norm()) / n0)
+            s = B.read_stats(stats)
+            ratio = errs[1] / errs[0] if errs[0] > 0 else float("nan")
+            print(f"| {T} | {name} {theta:g} | {s.n_keep}/{s.n_act} | {errs[0]:.4f} | {errs[1]:.4f} | {ratio:.2f} |")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--workload", default="c3", choices=["c2", "c3", "c4"])
@@ -48,12 +75,19 @@ def main():
     ap.add_argument("--cir", default="0.9,0.8,0.7")
     ap.add_argument("--steps", type=int, default=12)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--ablation", action="store_true", help="compensation ablation proxy instead of the latency sweep")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.workload.upper()]
     Ts = [int(t) for t in args.tokens.split(",")]
     dev = "cuda:0"
     L = Layer(cfg, seed=0, max_tokens=max(max(Ts), 128), device=dev)
     D = cfg.D
+    if args.ablation:
+        try:
+            ablation(L, cfg, Ts, args)
+        finally:
+            L.close()
+        return
     print(f"# Knob sweep, {cfg.name} (H={cfg.H} I={cfg.I} E={cfg.E}+{cfg.S} top-{cfg.k}, D={D} partitions, "
           f"partition {cfg.straggler_part} costs 2x)\n")
     print("| T | setting | step µs | vs dense | experts run | GB read | F_cost ticks (dense → kept) | per-partition load after pruning, % of the dense max |")

@@ -67,7 +67,8 @@ def test_prune_compensate_compact_bit_exact(H, cfg, mode):
     try:
         for T in (1, 5, 16, 64, 300):
             m, theta = MODES[mode]
-            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS) if mode == "thresh" else (0,)):
+            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS, B.CAEE_COMP_RANDOM) if mode == "thresh" else
+                          (0, B.CAEE_COMP_RANDOM) if mode == "cir" else (0,)):
                 th = _thresh_theta(cfg, T) if theta is None else theta
                 x = wl.hidden(cfg, T, 11, L.device)
                 s = L.oracle_scores(x)
@@ -143,7 +144,8 @@ def test_forward_decisions_bit_exact_fused_and_standalone(H, cfg, mode):
     try:
         for T in (1, 7, 16, 17, 32, 129, 256, 257, 300):
             m, theta = MODES.get(mode, (0, 0.0))
-            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS) if mode == "thresh" else (0,)):
+            for flags in ((0, B.CAEE_KEEP_TOP1 | B.CAEE_COMP_ALL_TOKENS, B.CAEE_COMP_RANDOM) if mode == "thresh" else
+                          (0, B.CAEE_COMP_RANDOM) if mode == "cir" else (0,)):
                 th = _thresh_theta(cfg, T) if theta is None else theta
                 x = wl.hidden(cfg, T, 13, L.device)
                 s = L.oracle_scores(x)
