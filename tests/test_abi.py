@@ -77,6 +77,31 @@ def test_null_context_is_an_error_not_a_crash(B):
     assert lib.caee_create(None, None) == B.CAEE_EINVAL
 
 
+def test_cache_abi_argument_errors(B):
+    """caee_cache_* reject bad arguments without a GPU; an empty cache reports empty slots."""
+    lib = C.CDLL(B.LIB_PATH)
+    lib.caee_cache_create.argtypes = [C.c_int32, C.c_void_p]
+    assert lib.caee_cache_create(4, None) == B.CAEE_EINVAL
+    for bad in (0, -3):
+        with pytest.raises(B.CaeeError) as ei:
+            B.caee_cache_create(bad)
+        assert ei.value.code == B.CAEE_EINVAL
+    lib.caee_cache_attach.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+    assert lib.caee_cache_attach(None, None, 0) == B.CAEE_EINVAL
+    lib.caee_cache_read_stats.argtypes = [C.c_void_p, C.c_void_p]
+    assert lib.caee_cache_read_stats(None, None) == B.CAEE_EINVAL
+    cache = B.caee_cache_create(5)
+    try:
+        assert B.caee_cache_snapshot(cache, 5) == [None] * 5
+        st = B.caee_cache_read_stats(cache)
+        assert (st.hits, st.misses, st.evictions, st.h2d_bytes) == (0, 0, 0, 0)
+    finally:
+        B.caee_cache_destroy(cache)
+    lib.caee_cache_destroy.argtypes = [C.c_void_p]
+    lib.caee_cache_destroy.restype = None
+    lib.caee_cache_destroy(None)          # a no-op, not a crash
+
+
 def test_product_does_not_import_the_oracle():
     """The oracle is test infrastructure: nothing under the package may import, load or link it."""
     pkg = os.path.join(ROOT, "paper_2606_29982_b200")
