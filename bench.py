@@ -294,7 +294,8 @@ def run_caee(args, cfg, prune):
         launches_per_step = 2 + (1 if fp8 else 0) + 1 + 1
     else:
         # stand-alone decision kernels: logits, top-k, [prune, compensate], count/scan/fill, [split], expert, combine, stats
-        launches_per_step = 2 + (2 if prune is not None and prune[0] != 0 else (1 if prune is not None else 0)) + 3 + (1 if fp8 else 0) + 1 + 1 + 1
+        n_prune = 0 if prune is None else (1 if T <= 512 else 2)      # k_prune, or k_prune_accum + k_prune_from_acc
+        launches_per_step = 2 + n_prune + (1 if prune is not None and prune[0] != 0 else 0) + 3 + (1 if fp8 else 0) + 1 + 1 + 1
     if cfg.n_resident >= 0:
         launches_per_step += 1 + st.n_fetch          # k_stats + one expert launch per fetched expert (C5)
     out = {

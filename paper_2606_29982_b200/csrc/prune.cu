@@ -29,6 +29,34 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, do
   caee_prune_decide(sm, mode, theta, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
+// Large steps: S2 and the per-token rules by one warp per token over many CTAs, into the global
+// integer accumulators that k_decide also uses (decide_scratch: zero between steps) ...
+__global__ void __launch_bounds__(256) k_prune_accum(int mode, int flags, double theta, int T, int k,
+                                                     const int32_t* __restrict__ idx, const float* __restrict__ gate,
+                                                     unsigned long long* acc_I, unsigned char* acc_act, unsigned char* acc_must) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (t < T) caee_prune_token(mode, flags, theta, k, idx + (size_t)t * k, gate + (size_t)t * k, lane, acc_I, acc_act, acc_must);
+}
+
+// ... then one CTA takes the batch-global decision from them and zeroes them again.  Integer
+// sums and flag bytes: the same masks as the one-CTA k_prune, whatever the order of the atomics.
+__global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, double theta, int E, int D,
+                                                                  unsigned long long* acc_I, unsigned char* acc_act,
+                                                                  unsigned char* acc_must, const int64_t* __restrict__ w_eff,
+                                                                  const int32_t* __restrict__ part, uint8_t* __restrict__ act_o,
+                                                                  uint8_t* __restrict__ must_o, uint8_t* __restrict__ keep_o,
+                                                                  int64_t* __restrict__ I_o, int64_t* __restrict__ load_o,
+                                                                  int64_t* __restrict__ scalars) {
+  __shared__ caee_prune_smem sm;
+  for (int e = threadIdx.x; e < E; e += PRUNE_THREADS) {
+    sm.I[e] = __ldcg(acc_I + e); sm.act[e] = __ldcg(acc_act + e); sm.must[e] = __ldcg(acc_must + e);
+    acc_I[e] = 0; acc_act[e] = 0; acc_must[e] = 0;
+  }
+  __syncthreads();
+  caee_prune_decide(sm, mode, theta, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+}
+
 template <int NV>
 __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ scores, const float* __restrict__ corr_bias,
                                                     const uint8_t* __restrict__ keep, int flags, int T, int E, int k,
@@ -52,6 +80,17 @@ __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ sc
 void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx, const float* gate,
                        cudaStream_t st) {
   const caee_layer_desc& d = c->d;
+  if (T > 512) {
+    // the token pass of a prefill-size step takes ~100 us on one CTA: spread it over the GPU
+    const size_t E = d.E;
+    unsigned long long* acc_I = reinterpret_cast<unsigned long long*>(c->decide_scratch);   // layout: decide.cu
+    unsigned char* acc_act = c->decide_scratch + E * 8;
+    unsigned char* acc_must = c->decide_scratch + E * 9;
+    k_prune_accum<<<caee_ceil_div(T, 8), 256, 0, st>>>(mode, flags, theta, T, d.k, idx, gate, acc_I, acc_act, acc_must);
+    k_prune_from_acc<<<1, PRUNE_THREADS, 0, st>>>(mode, theta, d.E, d.D, acc_I, acc_act, acc_must, c->w_eff, c->part, c->act,
+                                                  c->must, c->keep, c->I_fix, c->load, c->scalars);
+    return;
+  }
   k_prune<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, T, d.E, d.k, d.D, idx, gate, c->w_eff, c->part, c->act,
                                        c->must, c->keep, c->I_fix, c->load, c->scalars);
 }

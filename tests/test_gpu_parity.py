@@ -102,7 +102,7 @@ def test_prune_compensate_compact_bit_exact(H, cfg, mode):
         L.close()
 
 
-@pytest.mark.parametrize("mode", ["none", "frac", "thresh"])
+@pytest.mark.parametrize("mode", ["none", "frac", "thresh", "cir"])
 def test_compact_large_step_segmented_fill(H, mode):
     """Steps of more than 4096 (token, slot) entries take the segmented fill of worklist.cu
     (per-block histograms + in-block ranks): lists must still be the oracle's, entry for entry.
@@ -122,7 +122,13 @@ def test_compact_large_step_segmented_fill(H, mode):
         B.caee_prune(L.ctx, B.prune_params(m, th), torch.from_numpy(s).to(L.device), T, idx, gate, out.struct)
         torch.cuda.synchronize()
         g = {k: v.cpu().numpy() for k, v in out.t.items()}
-        cp = d["compact"]
+        cp, pr = d["compact"], d["prune"]
+        # the token pass of S2 runs on many CTAs at this size (k_prune_accum): same integers
+        for name in ("act", "must", "keep"):
+            assert np.array_equal(g[name], pr[name]), name
+        assert np.array_equal(g["importance"], pr["I_fix"]) and np.array_equal(g["load"], pr["load"])
+        assert list(g["scalars"][:7]) == [pr["F_base"], pr["F_cost_dense"], pr["F_cost"], pr["F_imp_fix"],
+                                          pr["n_act"], pr["n_must"], pr["n_keep"]]
         assert np.array_equal(idx.cpu().numpy(), d["idx"])
         nr = int(g["n_run"][0])
         assert nr == cp["n_run"]
