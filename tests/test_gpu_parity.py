@@ -399,6 +399,36 @@ def test_forward_offload_small(H, mode):
         L.close()
 
 
+def test_forward_c5_full_size_sampled(H):
+    """Config 5 at full size (bf16 R1-shaped layer, 64 of 256 experts resident, 192 packed images of
+    88 MB in pinned host memory): decisions bit-exact, fetch accounting, y on sampled tokens, for
+    a dense and a CIR step of 8 tokens."""
+    from paper_2606_29982_b200 import binding as B
+    L = H.GpuLayer(wl.C5, seed=0, max_tokens=32, keep_raw=False)
+    try:
+        assert int(L.resident.sum()) == 64
+        T = 8
+        for mode in ("dense", "cir"):
+            m, theta = MODES.get(mode, (0, 0.0))
+            x = wl.hidden(L.cfg, T, 300, L.device)
+            s = L.oracle_scores(x)
+            d = L.oracle_decisions(s, None if mode == "dense" else m, theta)
+            params = None if mode == "dense" else B.prune_params(m, theta)
+            y, st = L.forward(x, params, torch.from_numpy(s).to(L.device), want_stats=True)
+            idx_g, _ = L.last_routing(T)
+            assert np.array_equal(idx_g, d["idx"])
+            run = set(int(e) for e in d["compact"]["expert_ids"])
+            want_fetch = sum(1 for e in run if not L.resident[e])
+            assert st.n_fetch == want_fetch and st.h2d_bytes == want_fetch * L.cfg.expert_bytes
+            if mode != "dense":
+                assert st.F_cost == d["prune"]["F_cost"] and st.n_keep == d["prune"]["n_keep"]
+            toks = [0, 3, T - 1]
+            r = H.check_y(y, L.oracle_y(x, d["idx"], d["gate"], toks), toks, H.TOL[L.cfg.w_dtype])
+            print(f"C5 T={T} {mode}: n_fetch={st.n_fetch} max|err|/RMS = {r:.3e}")
+    finally:
+        L.close()
+
+
 @pytest.mark.parametrize("mode", ["dense", "cir"])
 def test_lfu_cache_multi_layer_decode_loop(H, mode):
     """a two-layer decode loop over an LFU expert cache smaller than the two
