@@ -258,8 +258,9 @@ caee_status caee_profile_read(caee_ctx* ctx, float* expert_ms, int32_t* n_out);
  * one cudaMemcpyAsync each on a side stream while the hits compute (one host synchronisation per
  * step, as in the static offload path).  All layers of one cache must have the same packed
  * expert size and be driven from ONE stream.  A step whose executed experts outnumber the slots
- * fails with CAEE_ESTATE.  The cache must outlive its attached contexts' calls; destroy the
- * contexts first. */
+ * fails with CAEE_ESTATE.  caee_route / caee_prune on an attached context use the residency
+ * uploaded by its last caee_moe_forward*.  The cache must outlive its attached contexts' calls;
+ * destroy the contexts first. */
 typedef struct caee_cache caee_cache;
 typedef struct caee_cache_stats {
   int64_t hits, misses, evictions; /* per executed (layer, expert, step), since creation */
