@@ -484,32 +484,34 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
   }
 }
 
-// x rows of every run -> the run's token-operand stage images.  CTA (r, y): run r, stages
-// [y nsub / gridDim.y, (y + 1) nsub / gridDim.y); one thread per 16-byte chunk, rows >= n are zero.
+// x rows of every run -> the run's token-operand stage images (fp16).  CTA (r, y): run r; eight
+// threads share a row (one 16-byte chunk of every 128-byte piece each) and walk its 64-k stages in
+// order, so a row's 2H bytes are read front to back; rows >= n are written as zeros.
 __global__ void __launch_bounds__(256) k_gather_x(caee_worklist wl, const uint4* __restrict__ x, uint8_t* __restrict__ xg, int H,
                                                   int n_runs_arg) {
   const int n_runs = n_runs_arg >= 0 ? n_runs_arg : wl.meta[1];
   const int run = blockIdx.x;
   if (run >= n_runs) return;
   const int n = wl.run_n[run], start = wl.run_start[run], npad = (n + 15) & ~15;
-  const int nsub = H / kKSub;
-  const int s0 = (int)((long long)blockIdx.y * nsub / gridDim.y), s1 = (int)((long long)(blockIdx.y + 1) * nsub / gridDim.y);
+  const int nsub = H / kKSub, j = threadIdx.x & 7;
   uint8_t* img = xg + (size_t)wl.run_hrow[run] * H * 2;
-  const int total = (s1 - s0) * npad * 8;
-  for (int i = threadIdx.x; i < total; i += blockDim.x) {
-    const int j = i & 7, rs = i >> 3, rr = rs % npad, s = s0 + rs / npad;
-    uint4 v = make_uint4(0, 0, 0, 0);
-    if (rr < n) v = __ldg(x + ((size_t)wl.ent_tok[start + rr] * H + s * kKSub) / 8 + j);
-    if (kTokF16) {
+  for (int rr = blockIdx.y * 32 + (threadIdx.x >> 3); rr < npad; rr += gridDim.y * 32) {
+    const uint4* src = rr < n ? x + (size_t)wl.ent_tok[start + rr] * (H / 8) + j : nullptr;
+    uint8_t* dst = img + (rr >> 3) * 1024 + (rr & 7) * 128 + ((j ^ (rr & 7)) << 4);
+    const size_t sstride = (size_t)npad * 128;
+#pragma unroll 4
+    for (int s = 0; s < nsub; ++s) {
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (src) v = __ldg(src + s * 8);
       uint32_t* w = reinterpret_cast<uint32_t*>(&v);
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
+      for (int q = 0; q < 4; ++q) {   // bf16 pair -> fp16 pair, clamped to fp16's range
         const float lo = __uint_as_float(w[q] << 16), hi = __uint_as_float(w[q] & 0xffff0000u);
         const __half2 h2 = __floats2half2_rn(fminf(fmaxf(lo, -65504.f), 65504.f), fminf(fmaxf(hi, -65504.f), 65504.f));
         w[q] = *reinterpret_cast<const uint32_t*>(&h2);
       }
+      *reinterpret_cast<uint4*>(dst + s * sstride) = v;
     }
-    *reinterpret_cast<uint4*>(img + (size_t)s * npad * 128 + (rr >> 3) * 1024 + (rr & 7) * 128 + ((j ^ (rr & 7)) << 4)) = v;
   }
 }
 
