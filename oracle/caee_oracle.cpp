@@ -351,6 +351,8 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
 // selection: key(e) = 2 + u(t,e) for a surviving pick, u(t,e) otherwise, u in [0,1) from a
 // counter-based generator both sides implement (murmur3's 32-bit finalizer over t, e and a fixed
 // constant); gates as in R16 (unbiased scores of the chosen experts, renormalised).
+// PARITY UNPINNED by PAPER.md (the baseline is named, not defined); pinned by
+// tests/test_oracle_ablation.py (murmur3's published fmix32 values, uniformity, invariants).
 static uint32_t fmix32(uint32_t h) {
   h ^= h >> 16; h *= 0x85ebca6bu; h ^= h >> 13; h *= 0xc2b2ae35u; h ^= h >> 16;
   return h;

@@ -21,6 +21,10 @@ Everything else is a reading, listed as R30-R34 in DESIGN.md §3 and followed he
   R33  the cost model sees the cache as it is when the step starts (R(e,d) = 0 for a hit).
   R34  the cache starts empty.
 
+PARITY UNPINNED by PAPER.md beyond the word "LFU": the paper prints no trace, count or rule to
+check these readings against.  What pins this file is tests/test_oracle_lfu.py (a trace worked by
+hand from R30-R34, the slots >= keys special case, invariants).
+
 Plain Python on purpose: dictionaries and a linear scan, no heap, so that it can be checked against
 the rules above by eye.
 """
