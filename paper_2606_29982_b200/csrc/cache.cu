@@ -124,8 +124,16 @@ caee_status caee_cache_step(caee_ctx* c, const int32_t* executed, int n_executed
   std::vector<int64_t>& f = k->freq[l];
   std::vector<int32_t>& so = k->slot_of[l];
   std::vector<uint8_t> in_use(c->d.E, 0);
-  for (int i = 0; i < n_executed; ++i) { in_use[executed[i]] = 1; ++f[executed[i]]; }
+  for (int i = 0; i < n_executed; ++i) in_use[executed[i]] = 1;
   miss_slots->clear();
+  // a step that does not fit fails before anything changes: every miss needs a slot that is free
+  // or holds a key this step does not execute
+  int n_miss = 0, n_avail = 0;
+  for (int i = 0; i < n_executed; ++i) n_miss += so[executed[i]] < 0;
+  for (int s = 0; s < k->n_slots; ++s) n_avail += !(k->slot_layer[s] == l && in_use[k->slot_expert[s]]);
+  if (n_miss > n_avail)
+    return caee_fail(c, CAEE_ESTATE, "the step executes %d experts of layer %d: they do not fit the cache's %d slots", n_executed, l, k->n_slots);
+  for (int i = 0; i < n_executed; ++i) ++f[executed[i]];
   for (int i = 0; i < n_executed; ++i) {
     const int e = executed[i];
     if (so[e] >= 0) { ++k->st.hits; continue; }

@@ -486,6 +486,10 @@ def test_lfu_cache_too_small_is_an_error(H):
         with pytest.raises(B.CaeeError) as ei:
             L.forward(x)
         assert ei.value.code == B.CAEE_ESTATE
+        # ... and it fails before anything changes
+        assert B.caee_cache_snapshot(cache, 3) == [None] * 3
+        st = B.caee_cache_read_stats(cache)
+        assert (st.hits, st.misses, st.evictions) == (0, 0, 0)
     finally:
         L.close()
         B.caee_cache_destroy(cache)
