@@ -255,41 +255,19 @@ def run_caee(args, cfg, prune):
     ms_step = ms_total / K
     value = world * T / (ms_step * 1e-3)
 
-    # --- end to end through the public call with HOST buffers (pinned), copies inside the timed region.
-    # Every step copies its x from pinned host memory and its y back; the copies run on two side
-    # streams with double-buffered device tensors, so step i's D2H and step i+1's H2D overlap the
-    # layer's compute the way a serving loop would pipeline them.  The timed region ends only after
-    # the last step's y has landed in host memory.
+    # --- end to end through the public call with HOST buffers (caee_moe_forward_host): every step
+    # copies its x from pinned host memory and its y back inside the timed region.  The library
+    # runs the copies on two side streams with double-buffered device tensors, so step i's D2H and
+    # step i+1's H2D overlap the layer's compute; the timed region ends only after the last step's
+    # y has landed in host memory (caee_host_flush).
     xh = [x.cpu().pin_memory() for x in xs]
     yh = torch.empty_like(xh[0]).pin_memory()
-    xd2 = [torch.empty_like(xs[0]) for _ in range(2)]
-    yd2 = [torch.empty_like(xs[0]) for _ in range(2)]
-    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
-    ev_in = [torch.cuda.Event() for _ in range(2)]
-    ev_cmp = [torch.cuda.Event() for _ in range(2)]
-    ev_out = [torch.cuda.Event() for _ in range(2)]
-    for b in range(2):          # so that the first waits return at once
-        ev_cmp[b].record(stream)
-        ev_out[b].record(stream)
 
     def e2e_step(i):
-        b = i & 1
-        with torch.cuda.stream(s_in):
-            s_in.wait_event(ev_cmp[b])                 # the step that last read xd2[b] is done
-            xd2[b].copy_(xh[i % len(xh)], non_blocking=True)
-            ev_in[b].record(s_in)
-        stream.wait_event(ev_in[b])
-        stream.wait_event(ev_out[b])                   # yd2[b]'s previous copy to the host is done
-        L.forward(xd2[b], params, y=yd2[b])
-        ev_cmp[b].record(stream)
-        with torch.cuda.stream(s_out):
-            s_out.wait_event(ev_cmp[b])
-            yh.copy_(yd2[b], non_blocking=True)
-            ev_out[b].record(s_out)
+        B.caee_moe_forward_host(L.ctx, xh[i % len(xh)], T, params, yh)
 
     def e2e_finish():
-        stream.wait_event(ev_out[0])
-        stream.wait_event(ev_out[1])
+        B.caee_host_flush(L.ctx)
 
     for i in range(4):
         e2e_step(i)
@@ -335,7 +313,7 @@ def run_caee(args, cfg, prune):
                    "seed": 0},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                "copies": "every step: x from pinned host memory, y back to it; double-buffered on two side streams",
+                "call": "caee_moe_forward_host: x from pinned host memory, y back to it, every step; copies double-buffered on two side streams",
                 "ms_per_step": ms_e2e},
         "gpu_launches": launches_per_step * K,
         "roofline": {"bound": "hbm", "kernel": "k_expert_fp8" if fp8 else "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",

@@ -229,6 +229,17 @@ caee_status caee_moe_forward(caee_ctx* ctx, const void* x, int32_t T, const caee
 caee_status caee_moe_forward_from_scores(caee_ctx* ctx, const void* x, const float* scores, int32_t T,
                                          const caee_prune_params* p, void* y, caee_fwd_stats* stats,
                                          void* stream);
+/* The same step with HOST buffers (x_host, y_host: [T,H] act_dtype, pinned memory for the copies
+ * to be asynchronous).  The library copies x into one of two device staging tensors on its own
+ * copy-in stream, runs caee_moe_forward on `stream`, and copies y back on its copy-out stream; the
+ * staging tensors are double-buffered, so the copies of neighbouring steps overlap the compute.
+ * Enqueue-only like caee_moe_forward: x_host must stay unchanged until its copy has run and
+ * y_host is complete only after caee_host_flush(ctx, stream) — which makes `stream` wait for
+ * every outstanding copy-out — and a synchronisation of `stream`.  Contexts with an expert cache
+ * or offloaded experts synchronise `stream` inside the step as caee_moe_forward does. */
+caee_status caee_moe_forward_host(caee_ctx* ctx, const void* x_host, int32_t T, const caee_prune_params* p,
+                                  void* y_host, caee_fwd_stats* stats, void* stream);
+caee_status caee_host_flush(caee_ctx* ctx, void* stream);
 /* K_final of the last forward call on this context (dev -> dev copy, enqueued on stream). */
 caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gate, void* stream);
 

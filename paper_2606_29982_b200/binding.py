@@ -27,7 +27,7 @@ CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",
            "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_route",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
-           "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version",
+           "caee_moe_forward_host", "caee_host_flush", "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version",
            "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot"]
 
 
@@ -97,6 +97,9 @@ _lib.caee_moe_forward.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.POINTER(caee_
                                   C.c_void_p]
 _lib.caee_moe_forward_from_scores.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(caee_prune_params),
                                               C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.caee_moe_forward_host.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.POINTER(caee_prune_params), C.c_void_p, C.c_void_p,
+                                       C.c_void_p]
+_lib.caee_host_flush.argtypes = [_ctx_p, C.c_void_p]
 _lib.caee_last_routing.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_profile.argtypes = [_ctx_p, C.c_int32]
 _lib.caee_profile_read.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
@@ -215,6 +218,15 @@ def caee_moe_forward_from_scores(ctx, x, scores, T, params, y, stats=None, strea
     _check(_lib.caee_moe_forward_from_scores(ctx, _ptr(x), _ptr(scores), int(T),
                                              C.byref(params) if params is not None else None, _ptr(y), _ptr(stats),
                                              _stream(stream)), ctx)
+
+
+def caee_moe_forward_host(ctx, x_host, T, params, y_host, stats=None, stream=None):
+    _check(_lib.caee_moe_forward_host(ctx, _ptr(x_host), int(T), C.byref(params) if params is not None else None,
+                                      _ptr(y_host), _ptr(stats), _stream(stream)), ctx)
+
+
+def caee_host_flush(ctx, stream=None):
+    _check(_lib.caee_host_flush(ctx, _stream(stream)), ctx)
 
 
 def caee_last_routing(ctx, T, idx, gate, stream=None):

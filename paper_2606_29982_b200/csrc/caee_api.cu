@@ -134,6 +134,15 @@ void free_all(caee_ctx* c) {
   for (cudaEvent_t e : c->fetch_ev) cudaEventDestroy(e);
   if (c->host_meta) cudaFreeHost(c->host_meta);
   if (c->cache_up) cudaFreeHost(c->cache_up);
+  for (int b = 0; b < 2; ++b) {
+    if (c->hx_d[b]) cudaFree(c->hx_d[b]);
+    if (c->hy_d[b]) cudaFree(c->hy_d[b]);
+    if (c->ev_hin[b]) cudaEventDestroy(c->ev_hin[b]);
+    if (c->ev_hcmp[b]) cudaEventDestroy(c->ev_hcmp[b]);
+    if (c->ev_hout[b]) cudaEventDestroy(c->ev_hout[b]);
+  }
+  if (c->s_in) cudaStreamDestroy(c->s_in);
+  if (c->s_out) cudaStreamDestroy(c->s_out);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   c->prof_ev.clear();
   if (c->side_stream) cudaStreamDestroy(c->side_stream);
@@ -609,6 +618,53 @@ caee_status caee_moe_forward_from_scores(caee_ctx* c, const void* x, const float
                                          const caee_prune_params* p, void* y, caee_fwd_stats* stats, void* stream) {
   if (c && !scores && T > 0) return caee_fail(c, CAEE_EINVAL, "scores is NULL");
   return forward_impl(c, x, scores, T, p, y, stats, stream);
+}
+
+caee_status caee_moe_forward_host(caee_ctx* c, const void* x_host, int32_t T, const caee_prune_params* p, void* y_host,
+                                  caee_fwd_stats* stats, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if (T == 0) return CAEE_OK;
+  if (!x_host || !y_host) return caee_fail(c, CAEE_EINVAL, "x_host or y_host is NULL");
+  DeviceGuard g(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t esz = c->d.act_dtype == CAEE_F32 ? 4 : 2;
+  if (!c->s_in) {
+    const size_t cap = (size_t)c->d.max_tokens * c->d.H * esz;
+    for (int b = 0; b < 2; ++b) {
+      CAEE_CUDA(c, cudaMalloc(&c->hx_d[b], cap));
+      CAEE_CUDA(c, cudaMalloc(&c->hy_d[b], cap));
+      CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_hin[b], cudaEventDisableTiming));
+      CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_hcmp[b], cudaEventDisableTiming));
+      CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_hout[b], cudaEventDisableTiming));
+      CAEE_CUDA(c, cudaEventRecord(c->ev_hcmp[b], st));     // nothing to wait for yet
+      CAEE_CUDA(c, cudaEventRecord(c->ev_hout[b], st));
+    }
+    CAEE_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+    CAEE_CUDA(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+  }
+  const int b = (int)(c->host_step++ & 1u);
+  const size_t bytes = (size_t)T * c->d.H * esz;
+  CAEE_CUDA(c, cudaStreamWaitEvent(c->s_in, c->ev_hcmp[b], 0));      // the step that last read this x buffer is done
+  CAEE_CUDA(c, cudaMemcpyAsync(c->hx_d[b], x_host, bytes, cudaMemcpyHostToDevice, c->s_in));
+  CAEE_CUDA(c, cudaEventRecord(c->ev_hin[b], c->s_in));
+  CAEE_CUDA(c, cudaStreamWaitEvent(st, c->ev_hin[b], 0));
+  CAEE_CUDA(c, cudaStreamWaitEvent(st, c->ev_hout[b], 0));           // this y buffer's previous copy-out is done
+  rc = forward_impl(c, c->hx_d[b], nullptr, T, p, c->hy_d[b], stats, stream);
+  if (rc != CAEE_OK) return rc;
+  CAEE_CUDA(c, cudaEventRecord(c->ev_hcmp[b], st));
+  CAEE_CUDA(c, cudaStreamWaitEvent(c->s_out, c->ev_hcmp[b], 0));
+  CAEE_CUDA(c, cudaMemcpyAsync(y_host, c->hy_d[b], bytes, cudaMemcpyDeviceToHost, c->s_out));
+  CAEE_CUDA(c, cudaEventRecord(c->ev_hout[b], c->s_out));
+  return CAEE_OK;
+}
+
+caee_status caee_host_flush(caee_ctx* c, void* stream) {
+  if (!c) return CAEE_EINVAL;
+  if (!c->s_out) return CAEE_OK;
+  DeviceGuard g(c->device);
+  for (int b = 0; b < 2; ++b) CAEE_CUDA(c, cudaStreamWaitEvent((cudaStream_t)stream, c->ev_hout[b], 0));
+  return CAEE_OK;
 }
 
 caee_status caee_profile(caee_ctx* c, int32_t n_slots) {

@@ -145,6 +145,13 @@ struct caee_ctx {
   int32_t* host_meta = nullptr;          // pinned: meta[16] then run_expert[max_runs]
   bool any_offload = false;
 
+  // caee_moe_forward_host: double-buffered device staging and the two copy streams
+  void* hx_d[2] = {nullptr, nullptr};
+  void* hy_d[2] = {nullptr, nullptr};
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_hin[2] = {nullptr, nullptr}, ev_hcmp[2] = {nullptr, nullptr}, ev_hout[2] = {nullptr, nullptr};
+  unsigned host_step = 0;
+
   // LFU cache mode (cache.cu): residency, effective costs and image pointers change every step
   caee_cache* cache = nullptr;
   int cache_layer = -1;

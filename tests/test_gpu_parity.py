@@ -523,6 +523,34 @@ def test_forward_c4_prefill_4096_sampled(H, pairs, monkeypatch):
         L.close()
 
 
+def test_forward_host_buffers_match_device_path(H):
+    """caee_moe_forward_host (pinned host x / y, copies pipelined on side streams with double-buffered
+    staging) gives bit-identical outputs to caee_moe_forward on device tensors, step after step, and
+    y_host is complete after caee_host_flush + a stream synchronisation."""
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, R1S, max_tokens=64, kernel=B.CAEE_KERNEL_UMMA)
+    try:
+        params = B.prune_params(B.CAEE_PRUNE_CIR, 0.8)
+        T = 48
+        xs = [wl.hidden(L.cfg, T, 400 + i, L.device) for i in range(5)]
+        want = [L.forward(x, params).clone() for x in xs]
+        xh = [x.cpu().pin_memory() for x in xs]
+        yh = [torch.empty_like(xh[0]).pin_memory() for _ in xs]
+        for i in range(5):                      # all five steps in flight before any wait
+            B.caee_moe_forward_host(L.ctx, xh[i], T, params, yh[i])
+        B.caee_host_flush(L.ctx)
+        torch.cuda.synchronize()
+        for i in range(5):
+            assert torch.equal(yh[i], want[i].cpu()), i
+        # a shorter step afterwards reuses the staging buffers
+        B.caee_moe_forward_host(L.ctx, xh[0][:7].contiguous().pin_memory(), 7, None, yh[0])
+        B.caee_host_flush(L.ctx)
+        torch.cuda.synchronize()
+        assert torch.equal(yh[0][:7], L.forward(xs[0][:7].contiguous(), None).cpu())
+    finally:
+        L.close()
+
+
 def test_forward_is_cuda_graph_capturable(H):
     """The per-step calls only enqueue (include/caee.h): a decode step — router GEMM, the cooperative
     decision kernel, the expert kernel, the combine — can be captured once and replayed; the replay
