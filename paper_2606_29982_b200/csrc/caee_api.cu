@@ -190,6 +190,7 @@ caee_status create_impl(caee_ctx* c) {
   }
   A(c->obuf, Tm * (k + S) * d.H);
 #undef A
+  if (const char* v = getenv("CAEE_NO_PDL")) c->pdl = atoi(v) == 0;   // tuning aid
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
   CAEE_CUDA(c, cudaMemset(c->tile_ctr, 0, sizeof(int32_t) * ntile));
   CAEE_CUDA(c, cudaMemset(c->decide_scratch, 0, caee_decide_scratch_bytes(c)));

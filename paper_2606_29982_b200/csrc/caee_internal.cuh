@@ -127,6 +127,7 @@ struct caee_ctx {
   uint8_t* xg = nullptr;             // e4m3 prefill kernel (expert_fp8_wide.cu): per-run stage images of the gathered x rows
   bool tm_ready = false;
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
+  bool pdl = true;                   // programmatic dependent launches on the decode path (env CAEE_NO_PDL=1 switches them off)
   bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;

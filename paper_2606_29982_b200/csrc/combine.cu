@@ -19,6 +19,7 @@ template <typename YT>
 __global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf, const int32_t* __restrict__ idx,
                                                  const float* __restrict__ gate, YT* __restrict__ y, int H, int k, int S,
                                                  float routed_scale) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // programmatic dependent launch: the expert kernel is done
   const int t = blockIdx.y, c = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (c >= H) return;
   const int KS = k + S;
@@ -48,6 +49,19 @@ void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* ga
   const caee_layer_desc& d = c->d;
   if (T <= 0) return;
   dim3 grid(caee_ceil_div(d.H, 1024), T);
+  if (c->pdl && !c->any_offload && d.act_dtype != CAEE_F32) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_combine<__nv_bfloat16>, (const float*)c->obuf, idx, gate, (__nv_bfloat16*)y, (int)d.H, (int)d.k, (int)d.S,
+                       (float)d.routed_scale);
+    return;
+  }
   if (d.act_dtype == CAEE_F32)
     k_combine<float><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (float*)y, d.H, d.k, d.S, d.routed_scale);
   else

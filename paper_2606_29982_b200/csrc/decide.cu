@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   float* gr = s_gate[warp];
 
   STAMP(0);
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the expert kernel's CTAs may be scheduled (they wait for this grid)
   float bl[NV], cb[NV];
   caee_load_vec<NV>(p.scores_in ? nullptr : p.b_logit, E, lane, bl);
   caee_load_vec<NV>(p.corr_bias, E, lane, cb);

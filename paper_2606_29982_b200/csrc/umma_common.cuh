@@ -127,6 +127,13 @@ __device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
                : "memory");
 }
 
+// Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization
+// may start while its predecessor in the stream still runs; griddep_wait() returns once the
+// predecessor grid has completed and its writes are visible (at once if launched normally);
+// griddep_launch() lets the successor's CTAs be scheduled from now on.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // One lane of a converged warp (the warp must be converged: "elect.sync").  Code around it
 // stays warp-uniform, so descriptor arithmetic runs on the uniform datapath instead of being
 // moved lane-register -> uniform-register in front of every tcgen05 instruction.
