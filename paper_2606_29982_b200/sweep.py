@@ -73,6 +73,7 @@ def main():
     ap.add_argument("--tokens", default="8,32,64,128")
     ap.add_argument("--thresh", default="0.3,0.6,0.8,1.0,1.2")
     ap.add_argument("--cir", default="0.9,0.8,0.7")
+    ap.add_argument("--frac", default="", help="FRAC budgets p (BASELINE.json config 4: 0.1,0.25)")
     ap.add_argument("--steps", type=int, default=12)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--ablation", action="store_true", help="compensation ablation proxy instead of the latency sweep")
@@ -102,7 +103,8 @@ def main():
             loads = " ".join(f"{100 * st_d.load[d] / fmax:.0f}" for d in range(D))
             print(f"| {T} | dense | {base_us:.0f} | 1.000 | {st.n_run} | {st.weight_bytes / 1e9:.2f} | {st_d.F_cost_dense} | {loads} |")
             grid = [("thresh", B.CAEE_PRUNE_THRESH, float(v)) for v in args.thresh.split(",") if v] + \
-                   [("cir", B.CAEE_PRUNE_CIR, float(v)) for v in args.cir.split(",") if v]
+                   [("cir", B.CAEE_PRUNE_CIR, float(v)) for v in args.cir.split(",") if v] + \
+                   [("frac", B.CAEE_PRUNE_FRAC, float(v)) for v in args.frac.split(",") if v]
             for name, mode, theta in grid:
                 us, s = measure(L, xs, B.prune_params(mode, theta), args.steps, args.warmup)
                 loads = " ".join(f"{100 * s.load[d] / fmax:.0f}" for d in range(D))
