@@ -3,8 +3,8 @@
 // TEST INFRASTRUCTURE ONLY.  This file is the slow, plain, obviously-correct
 // restatement of what the hot path computes, written from the paper
 // (/root/reference/PAPER.md, cited as PAPER.md:<line>) and, where the paper is
-// silent, from the readings listed in DESIGN.md §3 (numbered R1..R28 after
-// SURVEY.md §8(c)).  Only tests/, __graft_entry__.smoke() and bench.py's
+// silent, from the readings listed in DESIGN.md §3 (R1..R28 after SURVEY.md §8(c),
+// R29.. added by the build).  Only tests/, __graft_entry__.smoke() and bench.py's
 // cpu_baseline / --impl reference legs may load it.  It shares no code, header,
 // table or helper with the CUDA path under paper_2606_29982_b200/csrc/.
 //
@@ -22,7 +22,9 @@
 //                    configs + invariants only)
 //   O2 importance  : sum_e I(e) = T, order independence
 //   O3 cost/F_cost : closed forms (3573 ns, 11.010 us), literal max-of-sums
-//   O4 prune       : brute force over all subsets, F_cost == F_base, maximality
+//   O4 prune       : brute force over all subsets, F_cost == F_base, maximality; hand-worked
+//                    fixtures for the CIR boundary / gate order (R9, R36), the equal-importance
+//                    tie (R7, R22) and the importance bound (R37) with a brute-force minimality pin
 //   O5 compensate  : K_final subset of A_trans, unaffected tokens untouched
 //   O6 compact     : inverse-permutation check against idx
 //   O7/O8 FFN      : torch fp64 SwiGLU MLP, linearity, concatenation identity,
@@ -43,7 +45,7 @@ namespace {
 enum Dtype { DT_F32 = 0, DT_BF16 = 1, DT_E4M3 = 2 };
 enum ScoreFn { SCORE_SOFTMAX = 0, SCORE_SIGMOID = 1 };
 enum PruneMode { MODE_NONE = 0, MODE_THRESH = 1, MODE_CIR = 2, MODE_RANK = 3, MODE_FRAC = 4 };
-enum Flags { FLAG_COMP_ALL_TOKENS = 1, FLAG_KEEP_TOP1 = 2, FLAG_COMP_RANDOM = 4 };
+enum Flags { FLAG_COMP_ALL_TOKENS = 1, FLAG_KEEP_TOP1 = 2, FLAG_COMP_RANDOM = 4, FLAG_IMP_BOUND = 8 };
 
 const double FIX_ONE = 1099511627776.0;  // 2^40, fixed-point unit of I_fix (reading R-fix)
 
@@ -245,7 +247,24 @@ int64_t oracle_cost_ticks(double slope_ns_per_byte, double intercept_ns, int64_t
 //   [3] F_imp_fix = sum_{e in A_act \ A_trans} I_fix(e)  [4] |A_act|  [5] |A_must| (step 1)
 //   [6] |A_trans|
 // must[] is the step-1 mandatory set, keep[] is A_trans, load[] = per-partition cost of A_trans.
-int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const float* gate, int T,
+//
+// Per-token rules (CIR, RANK, KEEP_TOP1) see the token's K_t "sorted by their gating scores
+// G(t)_e": positions ordered by (gate descending, expert id ascending) — reading
+// R36.  The route's list order is by the biased selection score s' = s + corr_bias and differs
+// from it whenever corr_bias != 0.
+//
+// FLAG_IMP_BOUND (reading R37): the constraint F_imp(X) <= eps of the objective
+// ("strictly bounding the importance loss" :154).  After step 3, while the
+// pruned importance exceeds eps, the pruned expert of largest I(e) (ties -> lower id) is put
+// back into A_trans; F_cost may then exceed F_base and is reported as it is.
+static void gate_order(const int32_t* ir, const float* gr, int k, std::vector<int>& ord) {
+  ord.clear();
+  for (int j = 0; j < k; ++j)
+    if (ir[j] >= 0) ord.push_back(j);
+  std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return before(gr[a], ir[a], gr[b], ir[b]); });
+}
+
+int oracle_prune(int mode, double theta, int flags, double eps, const int32_t* idx, const float* gate, int T,
                  int E, int k, const int64_t* w, const int32_t* part, int D, uint8_t* act,
                  int64_t* I_fix, uint8_t* must, uint8_t* keep, int64_t* load, int64_t* scalars) {
   oracle_importance(idx, gate, T, E, k, act, I_fix);
@@ -254,6 +273,7 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
 
   // Step 1: mandatory set by mode.
   std::fill(must, must + E, 0);
+  std::vector<int> ord;
   if (mode == MODE_NONE) {
     for (int e = 0; e < E; ++e) must[e] = act[e];
   } else if (mode == MODE_THRESH) {  // I(e) >= theta
@@ -264,13 +284,12 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
     for (int t = 0; t < T; ++t) {
       const int32_t* ir = idx + static_cast<size_t>(t) * k;
       const float* gr = gate + static_cast<size_t>(t) * k;
-      float pk = 0.0f;
-      for (int j = 0; j < k; ++j)
-        if (ir[j] >= 0) pk = pk + gr[j];
-      float rhs = th * pk;
+      gate_order(ir, gr, k, ord);
+      float pk = 0.0f;  // sum_{j=1..K} G(t)_{e_j}, in the sorted order
+      for (int j : ord) pk = pk + gr[j];
+      float rhs = th * pk;  // CIR(m) >= theta_imp  <=>  p_m >= theta_imp * p_K (no division, R9)
       float pm = 0.0f;
-      for (int j = 0; j < k; ++j) {
-        if (ir[j] < 0) break;
+      for (int j : ord) {
         must[ir[j]] = 1;
         pm = pm + gr[j];
         if (pm >= rhs) break;
@@ -278,11 +297,11 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
     }
   } else if (mode == MODE_RANK) {  // budget b experts/token (BASELINE.json config 1)
     int b = static_cast<int>(theta);
-    for (int t = 0; t < T; ++t)
-      for (int j = 0; j < k - b; ++j) {
-        int e = idx[static_cast<size_t>(t) * k + j];
-        if (e >= 0) must[e] = 1;
-      }
+    for (int t = 0; t < T; ++t) {
+      const int32_t* ir = idx + static_cast<size_t>(t) * k;
+      gate_order(ir, gate + static_cast<size_t>(t) * k, k, ord);
+      for (int m = 0; m < static_cast<int>(ord.size()) && m < k - b; ++m) must[ir[ord[m]]] = 1;
+    }
   } else if (mode == MODE_FRAC) {  // budget p of activated experts (BASELINE.json config 4)
     std::vector<int> a;
     for (int e = 0; e < E; ++e)
@@ -294,8 +313,11 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
     return -1;
   }
   if ((flags & FLAG_KEEP_TOP1) && mode != MODE_NONE)
-    for (int t = 0; t < T; ++t)
-      if (idx[static_cast<size_t>(t) * k] >= 0) must[idx[static_cast<size_t>(t) * k]] = 1;
+    for (int t = 0; t < T; ++t) {
+      const int32_t* ir = idx + static_cast<size_t>(t) * k;
+      gate_order(ir, gate + static_cast<size_t>(t) * k, k, ord);
+      if (!ord.empty()) must[ir[ord[0]]] = 1;
+    }
   int n_must = 0;
   for (int e = 0; e < E; ++e) n_must += must[e];
 
@@ -316,6 +338,20 @@ int oracle_prune(int mode, double theta, int flags, const int32_t* idx, const fl
     if (l[part[e]] + w[e] <= F_base) {
       keep[e] = 1;
       l[part[e]] += w[e];
+    }
+  }
+
+  // Importance bound (reading R37): F_imp(X) = sum_{pruned} I(e) <= eps.
+  if (flags & FLAG_IMP_BOUND) {
+    int64_t eps_fix = static_cast<int64_t>(std::floor(eps * FIX_ONE));
+    int64_t lost = 0;
+    for (int e = 0; e < E; ++e)
+      if (act[e] && !keep[e]) lost += I_fix[e];
+    for (int e : cand) {  // still in descending I(e), ties -> lower id
+      if (lost <= eps_fix) break;
+      if (keep[e]) continue;
+      keep[e] = 1;
+      lost -= I_fix[e];
     }
   }
 

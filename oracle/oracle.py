@@ -16,7 +16,7 @@ from . import build as _build
 DT_F32, DT_BF16, DT_E4M3 = 0, 1, 2
 SCORE_SOFTMAX, SCORE_SIGMOID = 0, 1
 MODE_NONE, MODE_THRESH, MODE_CIR, MODE_RANK, MODE_FRAC = 0, 1, 2, 3, 4
-FLAG_COMP_ALL_TOKENS, FLAG_KEEP_TOP1, FLAG_COMP_RANDOM = 1, 2, 4
+FLAG_COMP_ALL_TOKENS, FLAG_KEEP_TOP1, FLAG_COMP_RANDOM, FLAG_IMP_BOUND = 1, 2, 4, 8
 FIX_ONE = float(2 ** 40)
 
 _lib = None
@@ -108,7 +108,7 @@ def cost_ticks(slope_ns_per_byte, intercept_ns, nbytes):
     return int(lib().oracle_cost_ticks(float(slope_ns_per_byte), float(intercept_ns), int(nbytes)))
 
 
-def prune(mode, theta, flags, idx, gate, E, w, part, D):
+def prune(mode, theta, flags, idx, gate, E, w, part, D, eps=0.0):
     idx = _c(idx, np.int32)
     gate = _c(gate, np.float32)
     w = _c(w, np.int64)
@@ -120,7 +120,7 @@ def prune(mode, theta, flags, idx, gate, E, w, part, D):
     keep = np.empty(E, np.uint8)
     load = np.empty(D, np.int64)
     sc = np.empty(7, np.int64)
-    rc = lib().oracle_prune(int(mode), C.c_double(theta), int(flags), _p(idx), _p(gate), T, E, k, _p(w),
+    rc = lib().oracle_prune(int(mode), C.c_double(theta), int(flags), C.c_double(eps), _p(idx), _p(gate), T, E, k, _p(w),
                             _p(part), D, _p(act), _p(I_fix), _p(must), _p(keep), _p(load), _p(sc))
     assert rc == 0
     return dict(act=act, I_fix=I_fix, must=must, keep=keep, load=load, F_base=int(sc[0]),

@@ -123,12 +123,15 @@ def _must_reference(mode, theta, idx, gate, E):
     act = np.isin(np.arange(E), idx)
     if mode == MODE_THRESH:
         return act & (I >= theta)
+    # per-token rules see K_t sorted by gate (R36): an independent numpy sort
+    order = np.stack([np.lexsort((idx[t], -gate[t].astype(np.float64))) for t in range(T)])
+    idx_s, gate_s = np.take_along_axis(idx, order, 1), np.take_along_axis(gate, order, 1).astype(np.float64)
     if mode == MODE_RANK:
-        return np.isin(np.arange(E), idx[:, :k - int(theta)])
+        return np.isin(np.arange(E), idx_s[:, :k - int(theta)])
     if mode == MODE_CIR:
-        cir = np.cumsum(gate.astype(np.float64), 1) / gate.astype(np.float64).sum(1, keepdims=True)
+        cir = np.cumsum(gate_s, 1) / gate_s.sum(1, keepdims=True)
         m = (cir >= theta).argmax(1) + 1
-        keep = [idx[t, :m[t]] for t in range(T)]
+        keep = [idx_s[t, :m[t]] for t in range(T)]
         return np.isin(np.arange(E), np.concatenate(keep))
     if mode == MODE_FRAC:
         ids = np.flatnonzero(act)
@@ -160,7 +163,8 @@ def test_prune_bruteforce_over_all_subsets(orc, mode, thetas, uniform_cost, resi
             if mode == MODE_THRESH:
                 margin_ok = np.all(np.abs(I[act] / FIX - theta) > 1e-5)
             if mode == MODE_CIR:
-                cir = np.cumsum(gate.astype(np.float64), 1) / gate.astype(np.float64).sum(1, keepdims=True)
+                gs = -np.sort(-gate.astype(np.float64), 1)
+                cir = np.cumsum(gs, 1) / gs.sum(1, keepdims=True)
                 margin_ok = np.all(np.abs(cir - theta) > 1e-5)
             if mode == MODE_FRAC:
                 margin_ok = len(set(I[act].tolist())) == act.sum()
@@ -247,6 +251,124 @@ def test_keep_top1_flag(orc):
     assert r["n_must"] == 0 and r["n_keep"] == int((w[idx[0]] == 0).sum())       # faithful: may empty A_must (reading R23)
     r = orc.prune(MODE_THRESH, 5.0, 2, idx, gate, 8, w, part, 2)
     assert r["must"][idx[0, 0]] == 1
+
+
+def _golden_case(name):
+    g = read_golden(name)
+    E, D, k = int(g["E"][0]), int(g["D"][0]), int(g["k"][0])
+    idx = np.array(g["idx"], np.int32).reshape(-1, k)
+    gate = np.array(g["gate"], np.float32).reshape(-1, k)
+    return g, E, D, idx, gate, np.array(g["w"], np.int64), np.array(g["part"], np.int32)
+
+
+def _check_golden(r, g, keep_key="keep"):
+    assert list(r["must"]) == [int(v) for v in g["must"]]
+    assert list(r["keep"]) == [int(v) for v in g[keep_key]]
+
+
+def test_cir_boundary_and_gate_order_hand_example(orc):
+    """R9 (the boundary is '>=') and R36 (K_t sorted by gate, equal gates -> lower id)."""
+    g, E, D, idx, gate, w, part = _golden_case("cir_boundary_example.txt")
+    r = orc.prune(MODE_CIR, g["theta_imp"][0], 0, idx, gate, E, w, part, D)
+    _check_golden(r, g)
+    assert (r["F_base"], r["F_cost_dense"], r["F_cost"]) == (int(g["F_base"][0]), int(g["F_cost_dense"][0]), int(g["F_cost"][0]))
+    assert r["F_imp_fix"] == int(g["F_imp"][0] * FIX)
+    r = orc.prune(MODE_RANK, g["rank_budget"][0], 0, idx, gate, E, w, part, D)
+    assert list(r["must"]) == [int(v) for v in g["must"]]
+    r = orc.prune(MODE_THRESH, 5.0, 2, idx, gate, E, w, part, D)
+    assert list(r["must"]) == [int(v) for v in g["top1_must"]]
+
+
+def test_equal_importance_tie_hand_example(orc):
+    """R7 / R22: equal I(e) -> the lower expert id is visited (and promoted) first."""
+    g, E, D, idx, gate, w, part = _golden_case("prune_tie_example.txt")
+    r = orc.prune(MODE_THRESH, g["theta"][0], 0, idx, gate, E, w, part, D)
+    assert r["I_fix"][1] == r["I_fix"][2]
+    _check_golden(r, g)
+    assert (r["F_base"], r["F_cost_dense"], r["F_cost"]) == (int(g["F_base"][0]), int(g["F_cost_dense"][0]), int(g["F_cost"][0]))
+    assert r["F_imp_fix"] == int(g["F_imp"][0] * FIX)
+
+
+def test_per_token_rules_use_gate_order_not_list_order(orc):
+    """With a selection bias the route lists K_t by s' = s + corr_bias; CIR / RANK / KEEP_TOP1 must
+    still see it sorted by the gate (R36).  The reference sorts independently with numpy."""
+    rng = np.random.default_rng(77)
+    E, D, k = 16, 4, 4
+    differs = 0
+    for trial in range(120):
+        s, part, w, T = tiny_instance(rng, E, D, T=int(rng.integers(1, 9)), k=k, softmax=False)
+        cb = rng.normal(scale=0.3, size=E).astype(np.float32)
+        idx, gate = orc.route(s, cb, k)
+        differs += int((np.diff(gate, axis=1) > 0).any())
+        for mode, theta in ((MODE_CIR, 0.83), (MODE_CIR, 0.61), (MODE_RANK, 1), (MODE_RANK, 3)):
+            if mode == MODE_CIR:
+                gs = -np.sort(-gate.astype(np.float64), 1)
+                if not np.all(np.abs(np.cumsum(gs, 1) / gs.sum(1, keepdims=True) - theta) > 1e-5):
+                    continue
+            r = orc.prune(mode, theta, 0, idx, gate, E, w, part, D)
+            assert np.array_equal(r["must"].astype(bool), _must_reference(mode, theta, idx, gate, E)), (trial, mode, theta)
+        r = orc.prune(MODE_THRESH, 100.0, 2, idx, gate, E, w, part, D)
+        top = idx[np.arange(T), np.argmax(gate, 1)]          # np.argmax: first maximum
+        assert np.array_equal(r["must"].astype(bool), np.isin(np.arange(E), top))
+    assert differs > 60          # the instances really do have non-descending gate lists
+
+
+# ---------------------------------------------------------------- importance bound (R37)
+def test_importance_bound_hand_example(orc):
+    g, E, D, idx, gate, w, part = _golden_case("imp_bound_example.txt")
+    r0 = orc.prune(MODE_THRESH, g["theta"][0], 0, idx, gate, E, w, part, D)
+    _check_golden(r0, g, "keep_unbounded")
+    assert r0["F_imp_fix"] == int(g["F_imp_unbounded"][0] * FIX)
+    for eps in (g["eps"][0], g["eps_boundary"][0]):
+        r = orc.prune(MODE_THRESH, g["theta"][0], 8, idx, gate, E, w, part, D, eps=eps)
+        _check_golden(r, g)
+        assert (r["F_base"], r["F_cost"]) == (int(g["F_base"][0]), int(g["F_cost"][0]))
+        assert r["F_imp_fix"] == int(g["F_imp"][0] * FIX)
+    r = orc.prune(MODE_THRESH, g["theta"][0], 8, idx, gate, E, w, part, D, eps=0.0)
+    assert np.array_equal(r["keep"], r["act"]) and r["F_imp_fix"] == 0 and r["F_cost"] == r["F_cost_dense"]
+
+
+@pytest.mark.parametrize("mode,theta", [(MODE_THRESH, 0.9), (MODE_CIR, 0.6), (MODE_FRAC, 0.7), (MODE_RANK, 1)])
+def test_importance_bound_bruteforce(orc, mode, theta):
+    """F_imp <= eps holds; the bound only ever restores (A_trans grows); the restored
+    set R is the smallest set of pruned experts whose return meets the bound (brute force over all
+    subsets of the unbounded pruned set), hence the pruned set is inclusion-maximal under the bound;
+    a bound that already holds changes nothing."""
+    rng = np.random.default_rng(300 + mode)
+    E, D, k = 8, 2, 2
+    hit = 0
+    for trial in range(80):
+        s, part, w, T = tiny_instance(rng, E, D, T=int(rng.integers(2, 9)), k=k)
+        idx, gate = orc.route(s, None, k)
+        r0 = orc.prune(mode, theta, 0, idx, gate, E, w, part, D)
+        I = r0["I_fix"]
+        pruned0 = np.flatnonzero(r0["act"].astype(bool) & ~r0["keep"].astype(bool))
+        for eps in (0.0, 0.05, 0.3, 0.8, 100.0):
+            r = orc.prune(mode, theta, 8, idx, gate, E, w, part, D, eps=eps)
+            eps_fix = int(np.floor(eps * FIX))
+            assert r["F_imp_fix"] <= eps_fix
+            keep0, keep1 = r0["keep"].astype(bool), r["keep"].astype(bool)
+            assert not (keep0 & ~keep1).any() and np.array_equal(r["must"], r0["must"]) and r["F_base"] == r0["F_base"]
+            assert r["F_cost"] == F_literal(keep1, w, part, D) >= r["F_base"]
+            assert r["F_imp_fix"] == int(I[r["act"].astype(bool) & ~keep1].sum())
+            restored = np.flatnonzero(keep1 & ~keep0)
+            if r0["F_imp_fix"] <= eps_fix:
+                assert len(restored) == 0
+                continue
+            hit += 1
+            best = None
+            for bits_ in itertools.product([0, 1], repeat=len(pruned0)):
+                sel = pruned0[np.array(bits_, bool)]
+                if int(I[pruned0].sum() - I[sel].sum()) <= eps_fix and (best is None or len(sel) < best):
+                    best = len(sel)
+            assert len(restored) == best
+            # greedy by importance: every restored expert is at least as important as every expert left pruned
+            left = np.setdiff1d(pruned0, restored)
+            if len(left) and len(restored):
+                assert I[restored].min() >= I[left].max()
+            for e in restored:             # dropping any restored expert breaks the bound
+                assert r["F_imp_fix"] + int(I[e]) > eps_fix
+    assert hit > 40
 
 
 # ---------------------------------------------------------------- O5
