@@ -2,7 +2,7 @@
  * decode hot path on one NVIDIA B200 (sm_100a).
  *
  * Citations are to /root/reference/PAPER.md ("PAPER.md:<line>") and to the readings
- * R1..R29 listed in DESIGN.md §3.  The paper's "devices" are logical expert
+ * R1..R37 listed in DESIGN.md §3.  The paper's "devices" are logical expert
  * partitions on one GPU whose costs are aggregated by max.
  *
  * Conventions
@@ -63,14 +63,21 @@ enum {
   CAEE_PRUNE_THRESH = 1, /* I(e) = sum_t G(t)_e >= theta        (on-device setup)  */
   CAEE_PRUNE_CIR = 2,    /* per token, minimal m* with CIR(m*) >= theta (offloading)    */
   CAEE_PRUNE_RANK = 3,   /* per token, the first k - theta of K_t    (BASELINE.json config 1 budget) */
+                         /* CIR, RANK and KEEP_TOP1 see K_t "sorted by their gating scores":
+                            by (gate descending, expert id ascending), R36 — not in the route's list order,
+                            which is by the biased selection score                                       */
   CAEE_PRUNE_FRAC = 4    /* all but the floor(theta*|A_act|) least important (config 4 budget)       */
 };
 enum {
   CAEE_COMP_ALL_TOKENS = 1, /* re-select every token, not only those that lost an expert (R14)       */
   CAEE_KEEP_TOP1 = 2,       /* every token's first expert is mandatory (R23)                          */
-  CAEE_COMP_RANDOM = 4      /* ablation baseline of PAPER.md:250-256 / Fig. 9 (R35): an affected token
+  CAEE_COMP_RANDOM = 4,     /* ablation baseline of PAPER.md:250-256 / Fig. 9 (R35): an affected token
                                keeps its surviving picks and fills the vacated slots uniformly at random
                                from the rest of A_trans (counter-based draws, reproducible)            */
+  CAEE_IMP_BOUND = 8        /* enforce the objective's constraint F_imp(X) <= eps (R37):
+                               after the cost-invariant expansion, while the pruned importance exceeds
+                               eps the pruned expert of largest I(e) (ties -> lower id) returns to A_trans;
+                               F_cost may then exceed F_base and is reported as it is                  */
 };
 enum { CAEE_KERNEL_AUTO = 0, CAEE_KERNEL_SIMT = 1, CAEE_KERNEL_UMMA = 2 };
 
@@ -110,9 +117,11 @@ typedef struct caee_expert_weights {
 
 typedef struct caee_prune_params {
   int32_t mode;  /* CAEE_PRUNE_*                                                                  */
-  int32_t flags; /* CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM                      */
+  int32_t flags; /* CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM | CAEE_IMP_BOUND     */
   double theta;  /* THRESH: theta in gate units (sum G = 1); CIR: theta_imp in (0,1];
                     RANK: budget b in 0..k; FRAC: p in [0,1]                                     */
+  double eps;    /* with CAEE_IMP_BOUND: bound on F_imp = sum of pruned I(e), in gate units
+                    (sum_e I(e) = T), in [0, 1e6]; ignored otherwise                              */
 } caee_prune_params;
 
 /* Optional device outputs of caee_prune; any pointer may be NULL.  scalars[8] =
@@ -201,6 +210,16 @@ caee_status caee_set_cost_table(caee_ctx* ctx, const int64_t* ticks_resident, co
  * t = slope*bytes + intercept, and with opts->apply fills the cost table with
  * round(slope*S_e + intercept) ns per tier.  Blocking.  opts may be NULL (defaults, apply=1). */
 caee_status caee_calibrate_cost(caee_ctx* ctx, const caee_calib_opts* opts, caee_cost_fit out_fit[2]);
+/* The points the last caee_calibrate_cost on this context timed for tier 0 (HBM) or 1 (H2D): transfer
+ * sizes in bytes and the median duration of each in ns (host arrays of capacity cap), their number in
+ * *n_out (0 if the tier was not measured).  They are exactly what the fit was computed from, so a
+ * caller can check the least squares of PAPER.md:139 independently. */
+caee_status caee_calibrate_points(const caee_ctx* ctx, int32_t tier, int32_t cap, double* bytes, double* ns,
+                                  int32_t* n_out);
+/* The cost table in force (host arrays [E]; either may be NULL): as set by caee_set_cost_table or
+ * applied by caee_calibrate_cost, ticks = llround(slope * S_e + intercept) per tier (clamped at 0),
+ * S_e = 3*H*I*sizeof(w) + the e4m3 block scales. */
+caee_status caee_get_cost_table(const caee_ctx* ctx, int64_t* ticks_resident, int64_t* ticks_miss);
 
 /* S0+S1: scores s = act(x W_r^T + b_logit) and the top-k set K_t with gates.
  * x dev [T,H] act dtype; scores dev [T,E] fp32 or NULL; idx dev [T,k] int32 in descending
@@ -221,7 +240,7 @@ caee_status caee_prune(caee_ctx* ctx, const caee_prune_params* p, const float* s
  * compute; stats->n_fetch / h2d_bytes count them) -> grouped SwiGLU FFN over the surviving
  * experts only -> combine
  *   y_t = routed_scale * sum_{e in K_final} G(t)_e E_e(t) + sum_shared E_sh(t).
- * x, y dev [T,H] act dtype; stats dev or NULL. */
+ * x, y dev [T,H] act dtype, 16-byte aligned; stats dev or NULL. */
 caee_status caee_moe_forward(caee_ctx* ctx, const void* x, int32_t T, const caee_prune_params* p, void* y,
                              caee_fwd_stats* stats, void* stream);
 /* Same, with the router's scores supplied by the caller (dev [T,E] fp32) instead of
@@ -240,6 +259,9 @@ caee_status caee_moe_forward_from_scores(caee_ctx* ctx, const void* x, const flo
 caee_status caee_moe_forward_host(caee_ctx* ctx, const void* x_host, int32_t T, const caee_prune_params* p,
                                   void* y_host, caee_fwd_stats* stats, void* stream);
 caee_status caee_host_flush(caee_ctx* ctx, void* stream);
+/* Kernels of this library that the per-step calls (caee_route*, caee_prune, caee_moe_forward*) have
+ * enqueued on this context since it was created (host counter, incremented at each launch site). */
+caee_status caee_launch_count(const caee_ctx* ctx, int64_t* n_out);
 /* K_final of the last forward call on this context (dev -> dev copy, enqueued on stream). */
 caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gate, void* stream);
 

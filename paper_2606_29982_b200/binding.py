@@ -21,11 +21,12 @@ CAEE_OK, CAEE_EINVAL, CAEE_ESHAPE, CAEE_EDTYPE, CAEE_ENOMEM, CAEE_ECUDA, CAEE_ES
 CAEE_F32, CAEE_BF16, CAEE_E4M3 = 0, 1, 2
 CAEE_SCORE_SOFTMAX, CAEE_SCORE_SIGMOID = 0, 1
 CAEE_PRUNE_NONE, CAEE_PRUNE_THRESH, CAEE_PRUNE_CIR, CAEE_PRUNE_RANK, CAEE_PRUNE_FRAC = 0, 1, 2, 3, 4
-CAEE_COMP_ALL_TOKENS, CAEE_KEEP_TOP1, CAEE_COMP_RANDOM = 1, 2, 4
+CAEE_COMP_ALL_TOKENS, CAEE_KEEP_TOP1, CAEE_COMP_RANDOM, CAEE_IMP_BOUND = 1, 2, 4, 8
 CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",
-           "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_route",
+           "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_calibrate_points",
+           "caee_get_cost_table", "caee_launch_count", "caee_route",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
            "caee_moe_forward_host", "caee_host_flush", "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version",
            "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot"]
@@ -43,7 +44,7 @@ class caee_expert_weights(C.Structure):
 
 
 class caee_prune_params(C.Structure):
-    _fields_ = [("mode", C.c_int32), ("flags", C.c_int32), ("theta", C.c_double)]
+    _fields_ = [("mode", C.c_int32), ("flags", C.c_int32), ("theta", C.c_double), ("eps", C.c_double)]
 
 
 class caee_prune_out(C.Structure):
@@ -89,6 +90,9 @@ _lib.caee_set_partitions.argtypes = [_ctx_p, C.c_void_p, C.c_int32]
 _lib.caee_set_residency.argtypes = [_ctx_p, C.c_void_p]
 _lib.caee_set_cost_table.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
 _lib.caee_calibrate_cost.argtypes = [_ctx_p, C.POINTER(caee_calib_opts), C.POINTER(caee_cost_fit)]
+_lib.caee_calibrate_points.argtypes = [_ctx_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.caee_get_cost_table.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
+_lib.caee_launch_count.argtypes = [_ctx_p, C.c_void_p]
 _lib.caee_route.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_route_from_scores.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_prune.argtypes = [_ctx_p, C.POINTER(caee_prune_params), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
@@ -196,6 +200,26 @@ def caee_calibrate_cost(ctx, opts: caee_calib_opts = None):
     return fits[0], fits[1]
 
 
+def caee_calibrate_points(ctx, tier, cap=16):
+    """(bytes[n], ns[n]) of the last calibration's timed points for a tier."""
+    b, t = np.zeros(cap, np.float64), np.zeros(cap, np.float64)
+    n = C.c_int32(0)
+    _check(_lib.caee_calibrate_points(ctx, int(tier), int(cap), _ptr(b), _ptr(t), C.addressof(n)), ctx)
+    return b[:n.value].copy(), t[:n.value].copy()
+
+
+def caee_get_cost_table(ctx, E):
+    tr, tm = np.zeros(E, np.int64), np.zeros(E, np.int64)
+    _check(_lib.caee_get_cost_table(ctx, _ptr(tr), _ptr(tm)), ctx)
+    return tr, tm
+
+
+def caee_launch_count(ctx):
+    n = C.c_int64(0)
+    _check(_lib.caee_launch_count(ctx, C.addressof(n)), ctx)
+    return n.value
+
+
 def caee_route(ctx, x, T, scores, idx, gate, stream=None):
     _check(_lib.caee_route(ctx, _ptr(x), int(T), _ptr(scores), _ptr(idx), _ptr(gate), _stream(stream)), ctx)
 
@@ -287,8 +311,11 @@ def caee_kernel_is_simt(cfg, kernel):
     return kernel == CAEE_KERNEL_SIMT or (kernel == CAEE_KERNEL_AUTO and not umma_ok)
 
 
-def prune_params(mode, theta=0.0, flags=0):
-    return caee_prune_params(int(mode), int(flags), float(theta))
+def prune_params(mode, theta=0.0, flags=0, eps=None):
+    """eps (a bound on F_imp in gate units) switches CAEE_IMP_BOUND on."""
+    if eps is not None:
+        flags |= CAEE_IMP_BOUND
+    return caee_prune_params(int(mode), int(flags), float(theta), 0.0 if eps is None else float(eps))
 
 
 class PruneOut:

@@ -90,7 +90,8 @@ caee_status validate_prune(caee_ctx* c, const caee_prune_params* p) {
       break;
     default: return caee_fail(c, CAEE_EINVAL, "unknown prune mode %d", p->mode);
   }
-  if (p->flags & ~(CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM)) return caee_fail(c, CAEE_EINVAL, "unknown prune flags");
+  if (p->flags & ~(CAEE_COMP_ALL_TOKENS | CAEE_KEEP_TOP1 | CAEE_COMP_RANDOM | CAEE_IMP_BOUND)) return caee_fail(c, CAEE_EINVAL, "unknown prune flags");
+  if ((p->flags & CAEE_IMP_BOUND) && (!(p->eps >= 0.0) || p->eps > 1e6)) return caee_fail(c, CAEE_EINVAL, "IMP_BOUND: eps must be in [0, 1e6]");
   return CAEE_OK;
 }
 
@@ -224,7 +225,7 @@ caee_status enqueue_decisions(caee_ctx* c, const void* x, const float* scores_in
   }
   const int mode = p ? p->mode : CAEE_PRUNE_NONE;
   if (p) {
-    caee_launch_prune(c, mode, p->flags, p->theta, T, idx, gate, st);
+    caee_launch_prune(c, mode, p->flags, p->theta, p->eps, T, idx, gate, st);
     if (mode != CAEE_PRUNE_NONE && T > 0) caee_launch_compensate(c, p->flags, scores, T, idx, gate, st);
   }
   caee_launch_worklist(c, T, idx, gate, st);
@@ -455,6 +456,29 @@ caee_status caee_calibrate_cost(caee_ctx* c, const caee_calib_opts* opts, caee_c
   return CAEE_OK;
 }
 
+caee_status caee_calibrate_points(const caee_ctx* c, int32_t tier, int32_t cap, double* bytes, double* ns, int32_t* n_out) {
+  if (!c || !n_out || tier < 0 || tier > 1 || cap < 0 || (cap > 0 && (!bytes || !ns))) return CAEE_EINVAL;
+  const int n = (int)c->calib_bytes[tier].size();
+  *n_out = n;
+  for (int i = 0; i < n && i < cap; ++i) { bytes[i] = c->calib_bytes[tier][i]; ns[i] = c->calib_ns[tier][i]; }
+  return CAEE_OK;
+}
+
+caee_status caee_get_cost_table(const caee_ctx* c, int64_t* ticks_resident, int64_t* ticks_miss) {
+  if (!c) return CAEE_EINVAL;
+  for (int e = 0; e < c->d.E; ++e) {
+    if (ticks_resident) ticks_resident[e] = c->ticks_res_h[e];
+    if (ticks_miss) ticks_miss[e] = c->ticks_miss_h[e];
+  }
+  return CAEE_OK;
+}
+
+caee_status caee_launch_count(const caee_ctx* c, int64_t* n_out) {
+  if (!c || !n_out) return CAEE_EINVAL;
+  *n_out = c->n_launches;
+  return CAEE_OK;
+}
+
 caee_status caee_route(caee_ctx* c, const void* x, int32_t T, float* scores, int32_t* idx, float* gate, void* stream) {
   caee_status rc = check_call(c, T);
   if (rc != CAEE_OK) return rc;
@@ -488,7 +512,7 @@ caee_status caee_prune(caee_ctx* c, const caee_prune_params* p, const float* sco
   if (prunes && T > 0 && !scores) return caee_fail(c, CAEE_EINVAL, "scores is NULL but compensation needs them");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  caee_prune_params none = {CAEE_PRUNE_NONE, 0, 0.0};
+  caee_prune_params none = {CAEE_PRUNE_NONE, 0, 0.0, 0.0};
   c->wl.run_cap = CAEE_RUN_TOKENS;
   rc = enqueue_decisions(c, nullptr, scores, T, p ? p : &none, idx, gate, nullptr, false, st);
   if (rc != CAEE_OK) return rc;
@@ -515,6 +539,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (p && p->mode != CAEE_PRUNE_NONE && !c->have_cost) return caee_fail(c, CAEE_ESTATE, "pruning requested before caee_set_cost_table / caee_calibrate_cost");
   if (T == 0) return CAEE_OK;
   if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
+  if (((uintptr_t)x | (uintptr_t)y) & 15) return caee_fail(c, CAEE_EINVAL, "x and y must be 16-byte aligned");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
   // decode steps (T <= 128) use 64-token runs: the smaller token operand leaves room for a deeper
@@ -555,7 +580,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   } else if (!c->any_offload) {
     caee_launch_umma_prepare(c, x, T, st);
     if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
-    caee_launch_expert_umma(c, x, T, 0, -1, 0, st);
+    if ((rc = caee_launch_expert_umma(c, x, T, 0, -1, 0, st)) != CAEE_OK) return rc;
   } else {
     // S9 (Fig. 8): only the non-resident experts that survived pruning are
     // fetched, one cudaMemcpyAsync each on the side stream, while the resident experts (first
@@ -598,10 +623,10 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     }
     n_fetch = (int)segs.size();
     if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
-    if (n_res > 0) caee_launch_expert_umma(c, x, T, 0, n_res, 0, st);
+    if (n_res > 0 && (rc = caee_launch_expert_umma(c, x, T, 0, n_res, 0, st)) != CAEE_OK) return rc;
     for (size_t i = 0; i < segs.size(); ++i) {
       CAEE_CUDA(c, cudaStreamWaitEvent(st, c->fetch_ev[i], 0));
-      caee_launch_expert_umma(c, x, T, segs[i].begin, segs[i].count, 1 + (int)i, st);
+      if ((rc = caee_launch_expert_umma(c, x, T, segs[i].begin, segs[i].count, 1 + (int)i, st)) != CAEE_OK) return rc;
     }
   }
   if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);

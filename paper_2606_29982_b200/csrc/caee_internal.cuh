@@ -126,11 +126,17 @@ struct caee_ctx {
   alignas(64) unsigned char tm_x[128] = {0}, tm_h[128] = {0};  // CUtensorMap of xq / hq (row gathers), see expert_fp8.cu
   uint8_t* xg = nullptr;             // e4m3 prefill kernel (expert_fp8_wide.cu): per-run stage images of the gathered x rows
   bool tm_ready = false;
+  int wide_max_pairs = -1;           // co-resident CTA pairs of the e4m3 prefill kernel on this device (-1: not asked yet)
+  unsigned attr_done = 0;            // bit i: this context's device has kernel i's MaxDynamicSharedMemorySize (a per-device attribute)
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
   bool pdl = true;                   // programmatic dependent launches on the decode path (env CAEE_NO_PDL=1 switches them off)
   bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
+
+  long long n_launches = 0;          // kernels of this library enqueued by the per-step calls (caee_launch_count)
+  // the timed points of the last caee_calibrate_cost (caee_calibrate_points): [tier] -> sizes in bytes, medians in ns
+  std::vector<double> calib_bytes[2], calib_ns[2];
 
   // optional expert-kernel timing (caee_profile)
   std::vector<cudaEvent_t> prof_ev;  // 2 per slot
@@ -182,7 +188,7 @@ size_t caee_decide_scratch_bytes(const caee_ctx* c);
 cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* p, caee_fwd_stats* stats,
                                cudaStream_t s);
 // prune.cu
-void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx,
+void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, double eps, int T, const int32_t* idx,
                        const float* gate, cudaStream_t s);
 void caee_launch_compensate(caee_ctx* c, int flags, const float* scores, int T, int32_t* idx, float* gate,
                             cudaStream_t s);
@@ -198,7 +204,7 @@ size_t caee_umma_packed_bytes(const caee_ctx* c);
 void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst_dev, const void* g, const void* u, const void* d,
                              const float* sg, const float* su, const float* sd, cudaStream_t s);
 void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
-void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
+caee_status caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // expert_fp8.cu
 caee_status caee_fp8_supported(const caee_ctx* c, std::string* why);
 size_t caee_fp8_packed_bytes(const caee_ctx* c);

@@ -68,6 +68,7 @@ caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost
   if (n_sizes < 2 || n_sizes > 16 || iters < 1 || iters > 1000 || lo < 4096 || hi <= lo || hi > (4LL << 30))
     return caee_fail(c, CAEE_EINVAL, "bad calibration options");
   memset(fit, 0, sizeof(caee_cost_fit) * 2);
+  for (int t = 0; t < 2; ++t) { c->calib_bytes[t].clear(); c->calib_ns[t].clear(); }
   std::vector<int64_t> sizes(n_sizes);
   for (int i = 0; i < n_sizes; ++i) {
     double f = (double)i / (n_sizes - 1);
@@ -111,6 +112,7 @@ caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost
       Tm.push_back(median(ms) * 1e6);
     }
     ols(S, Tm, &fit[0]);
+    c->calib_bytes[0] = S; c->calib_ns[0] = Tm;
   }
   {
     // tier 1: pinned host -> device copies (the paper's H2D transfer of a cache-miss expert)
@@ -136,6 +138,7 @@ caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost
         Tm.push_back(median(ms) * 1e6);
       }
       ols(S, Tm, &fit[1]);
+      c->calib_bytes[1] = S; c->calib_ns[1] = Tm;
     }
   }
 done:

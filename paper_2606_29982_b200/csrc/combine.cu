@@ -48,6 +48,7 @@ __global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_
 void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   if (T <= 0) return;
+  ++c->n_launches;
   dim3 grid(caee_ceil_div(d.H, 1024), T);
   if (c->pdl && !c->any_offload && d.act_dtype != CAEE_F32) {
     cudaLaunchConfig_t cfg = {};
@@ -76,6 +77,7 @@ long long caee_expert_bytes(const caee_ctx* c) {
 
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t st) {
   if (!stats) return;
+  ++c->n_launches;
   const long long bpe = caee_expert_bytes(c);
   k_stats<<<1, 64, 0, st>>>(stats, c->scalars, c->load, c->wl.meta, c->d.D, c->d.S, pruned, bpe, n_fetch);
 }

@@ -52,7 +52,7 @@ struct DecideParams {
   float* gate;             // [T,k] out
   int T, E, k, S, D, n_group, topk_group, score_fn, norm_topk;
   int has_prune, mode, flags;
-  double theta;
+  double theta, eps;
   const int64_t* w_eff;
   const int32_t* part;
   const uint8_t* resident;
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
       sm.must[e] = __ldcg(p.acc_must + e);
     }
     __syncthreads();
-    caee_prune_decide(sm, p.mode, p.theta, E, p.D, p.w_eff, p.part, blockIdx.x == 0, p.act, p.must, p.keep, p.I_fix, p.load,
+    caee_prune_decide(sm, p.mode, p.flags, p.theta, p.eps, E, p.D, p.w_eff, p.part, blockIdx.x == 0, p.act, p.must, p.keep, p.I_fix, p.load,
                       p.scalars);
     STAMP(3);
     // ---- C: S5 — a token that lost an expert re-selects inside A_trans
@@ -217,7 +217,7 @@ cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const
   p.T = T; p.E = d.E; p.k = d.k; p.S = d.S; p.D = d.D; p.n_group = d.n_group; p.topk_group = d.topk_group;
   p.score_fn = d.score_fn; p.norm_topk = d.norm_topk;
   p.has_prune = pp != nullptr; p.mode = pp ? pp->mode : CAEE_PRUNE_NONE; p.flags = pp ? pp->flags : 0;
-  p.theta = pp ? pp->theta : 0.0;
+  p.theta = pp ? pp->theta : 0.0; p.eps = pp ? pp->eps : 0.0;
   p.w_eff = c->w_eff; p.part = c->part; p.resident = c->resident;
   p.act = c->act; p.must = c->must; p.keep = c->keep; p.I_fix = c->I_fix; p.load = c->load; p.scalars = c->scalars;
   p.wl = c->wl; p.n_sched = c->wl.n_tickets + c->wl.max_runs;
@@ -237,5 +237,6 @@ cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const
                    : nv <= 8 ? (const void*)k_decide<8>
                              : (const void*)k_decide<16>;
   void* args[] = {&p};
+  ++c->n_launches;
   return cudaLaunchCooperativeKernel(fn, dim3(caee_ceil_div(T, kWarps)), dim3(kThreads), args, 0, st);
 }

@@ -545,6 +545,7 @@ caee_status caee_fp8_make_tensor_maps(caee_ctx* c) {
 // Once per step, before the first expert launch: x -> its two e4m3 terms and block scales.
 void caee_launch_fp8_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (T <= 0) return;
+  ++c->n_launches;
   const size_t n_blocks = (size_t)T * (c->d.H / kKBlock);
   const size_t TH = (size_t)c->d.max_tokens * c->d.H;
   k_act_split<<<(unsigned)((n_blocks + 7) / 8), 256, 0, st>>>((const __nv_bfloat16*)x, c->xq, c->xq + TH, c->xs, n_blocks);
@@ -577,10 +578,10 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
   const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers / amax buffers
   p.n_stages = std::min(kMaxStages, (max_dyn - 1024) / p.stage_bytes);
   const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(c->attr_done & 2u)) {
     cudaFuncSetAttribute(k_expert_fp8, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
-    attr_set = true;
+    c->attr_done |= 2u;
   }
+  ++c->n_launches;
   k_expert_fp8<<<c->num_sms, kThreads, dyn, st>>>(p);
 }

@@ -350,7 +350,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
           for (int j = 0; j < 16; ++j) {
             if (c + j < c_hi) {
               const float gv = __uint_as_float(g[j]) * inv, uv = __uint_as_float(u[j]) * inv;
-              const float hv = __fdividef(gv, 1.0f + __expf(-gv)) * uv;
+              // fp16 token operand: clamp like x (|h| > 65504 would become inf and then NaN in y)
+              const float hv = fminf(fmaxf(__fdividef(gv, 1.0f + __expf(-gv)) * uv, -65504.f), 65504.f);
               const int cc = c + j;
               *reinterpret_cast<uint16_t*>(hrun + cc * 128 + ((chunk ^ (cc & 7)) << 4)) =
                   kTokF16 ? __half_as_ushort(__float2half_rn(hv)) : __bfloat16_as_ushort(__float2bfloat16_rn(hv));
@@ -524,6 +525,7 @@ size_t caee_fp8_wide_xg_bytes(const caee_ctx* c) { return c->h_rows_cap * (size_
 // Once per step, after the work list is built: the x rows of every run, laid out for bulk copies.
 void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (T <= 0) return;
+  ++c->n_launches;
   k_gather_x<<<dim3((unsigned)c->wl.max_runs, 8), 256, 0, st>>>(c->wl, (const uint4*)x, c->xg, c->d.H, -1);
 }
 
@@ -531,6 +533,7 @@ void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_
 // tickets from wl.sched[ticket].  Runs hold up to CAEE_RUN_TOKENS_WIDE tokens.
 void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
   (void)T;
+  ++c->n_launches;
   const caee_layer_desc& d = c->d;
   WideParams p;
   p.wl = c->wl;
@@ -545,11 +548,10 @@ void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_coun
   p.sc_off = (int)((size_t)3 * d.H * d.I);
   p.t2_off = p.P1 * p.KB1 * 2;
   p.norm_off = (int)caee_fp8_norm_offset(c);
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(c->attr_done & 4u)) {
     cudaFuncSetAttribute(k_expert_fp8_wide<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
     cudaFuncSetAttribute(k_expert_fp8_wide<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
-    attr_set = true;
+    c->attr_done |= 4u;
   }
   // CTA pairs (cta_group::2) need an even number of tiles per run in both phases
   // (opt-in, caee_ctx::fp8_wide_pairs: on this pool's B200s the kernel runs into the 1000 W power cap
@@ -566,8 +568,9 @@ void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_coun
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     // the static schedule needs every pair resident at once (a phase-2 tile waits for phase-1 tiles of other pairs)
-    static int max_pairs = -1;
+    int max_pairs = c->wide_max_pairs;
     if (max_pairs < 0 && cudaOccupancyMaxActiveClusters(&max_pairs, k_expert_fp8_wide<true>, &cfg) != cudaSuccess) { max_pairs = 0; cudaGetLastError(); }
+    c->wide_max_pairs = max_pairs;
     if (max_pairs * 2 >= (int)cfg.gridDim.x) {
       cudaLaunchKernelEx(&cfg, k_expert_fp8_wide<true>, p);
       return;

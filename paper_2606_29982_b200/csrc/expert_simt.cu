@@ -142,6 +142,7 @@ void launch(caee_ctx* c, const void* x, cudaStream_t st) {
 
 void caee_launch_expert_simt(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   (void)T;
+  c->n_launches += 2;
   switch (c->d.w_dtype) {
     case CAEE_F32: launch<float>(c, x, st); break;
     case CAEE_BF16: launch<__nv_bfloat16>(c, x, st); break;

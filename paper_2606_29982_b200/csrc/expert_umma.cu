@@ -333,13 +333,14 @@ void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st
 
 // runs [run_begin, run_begin + run_count) (run_count < 0: every run of the work list), tile
 // tickets from wl.sched[ticket].
-void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
+caee_status caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   if (d.w_dtype == CAEE_E4M3) {
     if (c->wl.run_cap == CAEE_RUN_TOKENS_WIDE) caee_launch_expert_fp8_wide(c, T, run_begin, run_count, ticket, st);
     else caee_launch_expert_fp8(c, T, run_begin, run_count, ticket, st);
-    return;
+    return CAEE_OK;
   }
+  ++c->n_launches;
   UmmaParams p;
   p.wl = c->wl;
   p.packed = c->packed.dev_ptrs;
@@ -352,9 +353,12 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
   p.run_begin = run_begin; p.run_count = run_count; p.ticket = ticket;
   // x is the caller's buffer: its map is encoded per call (host-side, ~1 us); h is ours
   if (!c->tm_ready) {
-    if (encode_row_gather_map(c->tm_h, c->hbuf_b16, (size_t)d.I * 2, c->h_rows_cap)) c->tm_ready = true;
+    if (!encode_row_gather_map(c->tm_h, c->hbuf_b16, (size_t)d.I * 2, c->h_rows_cap))
+      return caee_fail(c, CAEE_ECUDA, "cuTensorMapEncodeTiled failed for the h scratch");
+    c->tm_ready = true;
   }
-  encode_row_gather_map(&p.tm_x, x, (size_t)d.H * 2, (size_t)T);
+  if (!encode_row_gather_map(&p.tm_x, x, (size_t)d.H * 2, (size_t)T))
+    return caee_fail(c, CAEE_EINVAL, "cuTensorMapEncodeTiled refused x (it must be 16-byte aligned device memory)");
   memcpy(&p.tm_h, c->tm_h, sizeof(CUtensorMap));
   const int ncap = std::min((int)c->wl.run_cap, (T + 15) & ~15);
   p.b_stage_bytes = ncap * kKBlock * 2;
@@ -362,10 +366,9 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
   const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers
   p.n_stages = std::min(kMaxStages, (max_dyn - 1024) / p.stage_bytes);
   const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(c->attr_done & 1u)) {
     cudaFuncSetAttribute(k_expert_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
-    attr_set = true;
+    c->attr_done |= 1u;
   }
   if (c->pdl && !c->any_offload) {
     // programmatic dependent launch: the CTAs are scheduled while the decision kernel still runs
@@ -379,7 +382,8 @@ void caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, i
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, k_expert_umma, p);
-    return;
+    return CAEE_OK;
   }
   k_expert_umma<<<c->num_sms, kThreads, dyn, st>>>(p);
+  return CAEE_OK;
 }

@@ -13,7 +13,7 @@ namespace {
 
 constexpr int PRUNE_THREADS = 512;
 
-__global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, double theta, int T, int E, int k, int D,
+__global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, double theta, double eps, int T, int E, int k, int D,
                                                          const int32_t* __restrict__ idx, const float* __restrict__ gate,
                                                          const int64_t* __restrict__ w_eff, const int32_t* __restrict__ part,
                                                          uint8_t* __restrict__ act_o, uint8_t* __restrict__ must_o,
@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, do
   for (int t = warp; t < T; t += PRUNE_THREADS / 32)
     caee_prune_token(mode, flags, theta, k, idx + (size_t)t * k, gate + (size_t)t * k, lane, sm.I, sm.act, sm.must);
   __syncthreads();
-  caee_prune_decide(sm, mode, theta, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
 // Large steps: S2 and the per-token rules by one warp per token over many CTAs, into the global
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) k_prune_accum(int mode, int flags, double
 
 // ... then one CTA takes the batch-global decision from them and zeroes them again.  Integer
 // sums and flag bytes: the same masks as the one-CTA k_prune, whatever the order of the atomics.
-__global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, double theta, int E, int D,
+__global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, int flags, double theta, double eps, int E, int D,
                                                                   unsigned long long* acc_I, unsigned char* acc_act,
                                                                   unsigned char* acc_must, const int64_t* __restrict__ w_eff,
                                                                   const int32_t* __restrict__ part, uint8_t* __restrict__ act_o,
@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, doub
     acc_I[e] = 0; acc_act[e] = 0; acc_must[e] = 0;
   }
   __syncthreads();
-  caee_prune_decide(sm, mode, theta, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
 template <int NV>
@@ -77,9 +77,10 @@ __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ sc
 
 }  // namespace
 
-void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, const int32_t* idx, const float* gate,
-                       cudaStream_t st) {
+void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, double eps, int T, const int32_t* idx,
+                       const float* gate, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
+  c->n_launches += T > 512 ? 2 : 1;
   if (T > 512) {
     // the token pass of a prefill-size step takes ~100 us on one CTA: spread it over the GPU
     const size_t E = d.E;
@@ -87,17 +88,18 @@ void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, int T, co
     unsigned char* acc_act = c->decide_scratch + E * 8;
     unsigned char* acc_must = c->decide_scratch + E * 9;
     k_prune_accum<<<caee_ceil_div(T, 8), 256, 0, st>>>(mode, flags, theta, T, d.k, idx, gate, acc_I, acc_act, acc_must);
-    k_prune_from_acc<<<1, PRUNE_THREADS, 0, st>>>(mode, theta, d.E, d.D, acc_I, acc_act, acc_must, c->w_eff, c->part, c->act,
+    k_prune_from_acc<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, d.E, d.D, acc_I, acc_act, acc_must, c->w_eff, c->part, c->act,
                                                   c->must, c->keep, c->I_fix, c->load, c->scalars);
     return;
   }
-  k_prune<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, T, d.E, d.k, d.D, idx, gate, c->w_eff, c->part, c->act,
+  k_prune<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, T, d.E, d.k, d.D, idx, gate, c->w_eff, c->part, c->act,
                                        c->must, c->keep, c->I_fix, c->load, c->scalars);
 }
 
 void caee_launch_compensate(caee_ctx* c, int flags, const float* scores, int T, int32_t* idx, float* gate,
                             cudaStream_t st) {
   const caee_layer_desc& d = c->d;
+  ++c->n_launches;
   int nv = caee_ceil_div(d.E, 32);
   dim3 grid(caee_ceil_div(T, 4));
 #define CAEE_COMP(NV) \

@@ -34,6 +34,9 @@ struct caee_prune_smem {
 
 // S2 + per-token rules of step 1 for one token (all 32 lanes call it).  ir/gr: the token's
 // K_t and gates; I/act/must: accumulators in shared or global memory.
+// The per-token rules (CIR, RANK, KEEP_TOP1) see K_t "sorted by their gating scores"
+// (PAPER.md:244): by (gate descending, expert id ascending), R36 — the route's list order is by
+// the biased selection score and differs from it when corr_bias != 0.
 __device__ __forceinline__ void caee_prune_token(int mode, int flags, double theta, int k, const int32_t* ir, const float* gr,
                                                  int lane, unsigned long long* I, unsigned char* act, unsigned char* must) {
   int e = -1;
@@ -44,29 +47,48 @@ __device__ __forceinline__ void caee_prune_token(int mode, int flags, double the
     // exact in fp32: power-of-two scale, then truncation
     atomicAdd(&I[e], (unsigned long long)__float2ll_rz(__fmul_rn(g, CAEE_FIX_ONE_F)));
   }
+  const bool top1 = (flags & CAEE_KEEP_TOP1) && mode != CAEE_PRUNE_NONE;
+  if (mode != CAEE_PRUNE_CIR && mode != CAEE_PRUNE_RANK && !top1) return;
+  // lane m <- the m-th entry of K_t by (gate desc, id asc); empty slots go last
+  const float kg = e >= 0 ? g : -INFINITY;
+  const int kid = e >= 0 ? e : (1 << 30) + lane;
+  int rank = 0;
+  for (int j = 0; j < k; ++j) {
+    const float gj = __shfl_sync(0xffffffffu, kg, j);
+    const int ij = __shfl_sync(0xffffffffu, kid, j);
+    rank += (gj > kg) | ((gj == kg) & (ij < kid));
+  }
+  int se = -1;
+  float sg = 0.f;
+  for (int m = 0; m < k; ++m) {
+    const int src = __ffs(__ballot_sync(0xffffffffu, lane < k && rank == m)) - 1;
+    const float gv = __shfl_sync(0xffffffffu, g, src);
+    const int ev = __shfl_sync(0xffffffffu, e, src);
+    if (lane == m) { sg = gv; se = ev; }
+  }
   if (mode == CAEE_PRUNE_CIR) {
-    // minimal m* with p_m >= theta_imp * p_k, sums in list order (R9); k <= 32 values live in the lanes
+    // minimal m* with p_m >= theta_imp * p_k, sums in sorted order (R9); k <= 32 values live in the lanes
     float pk = 0.f;
     for (int j = 0; j < k; ++j) {
-      const float gj = __shfl_sync(0xffffffffu, g, j);
-      const int ej = __shfl_sync(0xffffffffu, e, j);
+      const float gj = __shfl_sync(0xffffffffu, sg, j);
+      const int ej = __shfl_sync(0xffffffffu, se, j);
       if (ej >= 0) pk = __fadd_rn(pk, gj);
     }
     const float rhs = __fmul_rn((float)theta, pk);
     float pm = 0.f;
     bool open = true;    // slot j is within the first m*
     for (int j = 0; j < k; ++j) {
-      const float gj = __shfl_sync(0xffffffffu, g, j);
-      const int ej = __shfl_sync(0xffffffffu, e, j);
+      const float gj = __shfl_sync(0xffffffffu, sg, j);
+      const int ej = __shfl_sync(0xffffffffu, se, j);
       if (ej < 0) open = false;
-      if (open && lane == j) must[e] = 1;
+      if (open && lane == j) must[se] = 1;
       pm = __fadd_rn(pm, gj);
       if (pm >= rhs) open = false;
     }
   } else if (mode == CAEE_PRUNE_RANK) {
-    if (e >= 0 && lane < k - (int)theta) must[e] = 1;
+    if (se >= 0 && lane < k - (int)theta) must[se] = 1;
   }
-  if ((flags & CAEE_KEEP_TOP1) && mode != CAEE_PRUNE_NONE && lane == 0 && e >= 0) must[e] = 1;
+  if (top1 && lane == 0 && se >= 0) must[se] = 1;
 }
 
 __device__ __forceinline__ long long caee_warp_sum_ll(long long v) {
@@ -98,7 +120,7 @@ __device__ __forceinline__ int caee_warp_rank(const unsigned long long* key, con
 // the CTA is synchronised.  With `out` set the CTA also writes the result arrays (else only
 // shared memory is filled: several CTAs may take the same decision redundantly).
 // On return (synchronised) sm.keep, sm.load, sm.F_*, sm.cnt are valid.
-__device__ __forceinline__ void caee_prune_decide(caee_prune_smem& sm, int mode, double theta, int E, int D,
+__device__ __forceinline__ void caee_prune_decide(caee_prune_smem& sm, int mode, int flags, double theta, double eps, int E, int D,
                                                   const int64_t* __restrict__ w_eff, const int32_t* __restrict__ part, bool out,
                                                   uint8_t* __restrict__ act_o, uint8_t* __restrict__ must_o,
                                                   uint8_t* __restrict__ keep_o, int64_t* __restrict__ I_o,
@@ -201,6 +223,35 @@ __device__ __forceinline__ void caee_prune_decide(caee_prune_smem& sm, int mode,
     sm.load[tid] = l;
   }
   __syncthreads();
+  if (flags & CAEE_IMP_BOUND) {
+    // importance bound F_imp(X) <= eps (R37): the pruned experts return in
+    // descending (I, id asc) order while the pruned importance exceeds eps, i.e. expert e returns
+    // iff the importance of the pruned experts from e onwards in that order exceeds eps
+    const long long eps_fix = (long long)floor(eps * 1099511627776.0);
+    for (int e = tid; e < E; e += nth) sm.key[e] = (sm.act[e] && !sm.keep[e]) ? sm.I[e] + 1 : 0ull;
+    __syncthreads();
+    for (int e = warp; e < E; e += nwarps) {
+      const unsigned long long ke = sm.key[e];
+      if (ke == 0) continue;
+      long long tail = 0;
+      for (int f = lane; f < E; f += 32) {
+        const unsigned long long kf = sm.key[f];
+        const bool from_e = kf != 0 && (kf < ke || (kf == ke && f >= e));
+        tail += from_e ? (long long)(kf - 1) : 0;
+      }
+      tail = caee_warp_sum_ll(tail);
+      if (lane == 0 && tail > eps_fix) sm.keep[e] = 1;
+    }
+    __syncthreads();
+    for (int d = warp; d < D; d += nwarps) {
+      long long l = 0;
+      for (int e = lane; e < E; e += 32)
+        if (sm.prt[e] == d && sm.keep[e]) l += sm.w[e];
+      l = caee_warp_sum_ll(l);
+      if (lane == 0) sm.load[d] = l;
+    }
+    __syncthreads();
+  }
 
   PSTAMP(6);
   // step 4 + reporting

@@ -228,6 +228,7 @@ template <typename XT>
 void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   int tt, ks;
+  ++c->n_launches;
   caee_router_shape(c, T, &tt, &ks);
   const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), KC) * KC;
   dim3 grid(caee_ceil_div(d.E, TE), caee_ceil_div(T, tt), ks);
@@ -255,6 +256,7 @@ void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t s
 
 void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate,
                             cudaStream_t st) {
+  ++c->n_launches;
   int nv = caee_ceil_div(c->d.E, 32);
   if (nv <= 1) launch_topk<1>(c, scores_in, T, scores_out, idx, gate, st);
   else if (nv <= 2) launch_topk<2>(c, scores_in, T, scores_out, idx, gate, st);

@@ -114,6 +114,7 @@ void caee_launch_worklist(caee_ctx* c, int T, const int32_t* idx, const float* g
   cudaMemsetAsync(c->wl.counts, 0, sizeof(int32_t) * d.E, st);
   cudaMemsetAsync(c->wl.sched, 0, sizeof(int32_t) * (c->wl.n_tickets + c->wl.max_runs), st);
   int n = T * d.k;
+  c->n_launches += n > 0 ? 3 : 2;   // the two memsets are copy-engine work, not kernels of ours
   if (n > 4096 && c->wl_hist) {
     const int nb = caee_ceil_div(n, kFillSeg);
     k_wl_hist<<<nb, kFillSeg, sizeof(int) * d.E, st>>>(idx, n, d.E, c->wl.counts, c->wl_hist);
@@ -136,5 +137,6 @@ void caee_launch_export_worklist(caee_ctx* c, int T, const caee_prune_out* out, 
   if (out) o = *out;
   int n = T * c->d.k;
   int blocks = n > 0 ? caee_ceil_div(n, 256) : 1;
+  ++c->n_launches;
   k_wl_export<<<blocks > 64 ? 64 : blocks, 256, 0, st>>>(c->wl, o, c->d.E, c->scalars);
 }

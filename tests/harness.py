@@ -33,14 +33,17 @@ class GpuLayer(Layer):
     def oracle_scores(self, x):
         return orc.scores(wl.bits(x), self.Wr.cpu().numpy(), self.b_logit.cpu().numpy(), self.cfg.score_fn)
 
-    def oracle_decisions(self, s, mode=None, theta=0.0, flags=0):
-        """route -> prune -> compensate -> compact on scores s.  mode None = dense top-k."""
+    def oracle_decisions(self, s, mode=None, theta=0.0, flags=0, eps=None):
+        """route -> prune -> compensate -> compact on scores s.  mode None = dense top-k.
+        eps: bound on F_imp (switches the oracle's FLAG_IMP_BOUND on)."""
         c = self.cfg
         cb = None if self.corr_bias is None else self.corr_bias.cpu().numpy()
         idx, gate = orc.route(s, cb, c.k, c.n_group, c.topk_group, c.norm_topk)
         out = dict(idx0=idx.copy(), gate0=gate.copy())
         if mode is not None:
-            pr = orc.prune(mode, theta, flags, idx, gate, c.E, self.w_eff(), self.part, c.D)
+            if eps is not None:
+                flags |= orc.FLAG_IMP_BOUND
+            pr = orc.prune(mode, theta, flags, idx, gate, c.E, self.w_eff(), self.part, c.D, eps=0.0 if eps is None else eps)
             if mode != 0:
                 idx, gate = orc.compensate(s, cb, pr["keep"], idx, gate, c.norm_topk, flags)
             out["prune"] = pr
@@ -48,7 +51,16 @@ class GpuLayer(Layer):
         out["compact"] = orc.compact(idx, gate, c.E)
         return out
 
-    def oracle_y(self, x, idx, gate, tokens):
+    def oracle_y(self, x, idx, gate, tokens, chunk=None):
+        """chunk: evaluate that many tokens at a time and drop the host copies of the experts in between
+        (a full-size expert is 44-88 MB on the host; 32 tokens touch up to ~200 of them)."""
+        tokens = list(tokens)
+        if chunk is not None and len(tokens) > chunk:
+            out = []
+            for i in range(0, len(tokens), chunk):
+                out.append(self.oracle_y(x, idx, gate, tokens[i:i + chunk]))
+                self._host.clear()
+            return np.concatenate(out)
         c = self.cfg
         n = c.E + c.S
         used = set(int(e) for t in tokens for e in idx[t] if e >= 0) | set(range(c.E, n))

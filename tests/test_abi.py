@@ -36,7 +36,7 @@ def test_library_exports_every_declared_symbol(B):
 
 def test_struct_layouts_match_header(B):
     assert C.sizeof(B.caee_layer_desc) == 16 * 4
-    assert C.sizeof(B.caee_prune_params) == 16
+    assert C.sizeof(B.caee_prune_params) == 24
     assert C.sizeof(B.caee_expert_weights) == 6 * 8 and C.sizeof(B.caee_prune_out) == 12 * 8
     assert C.sizeof(B.caee_fwd_stats) == 6 * 8 + 4 * 4 + 64 * 8
     assert C.sizeof(B.caee_calib_opts) == 32 and C.sizeof(B.caee_cost_fit) == 40
