@@ -182,6 +182,8 @@ def moe_tokens(x, tokens, idx, gate, Wg, Wu, Wd, E, S, routed_scale, sg=None, su
     gate = _c(gate, np.float32)
     k = idx.shape[1]
     tokens = _c(tokens, np.int32)
+    if all(a is None for a in Wg):          # no listed token uses any expert (everything pruned, S = 0): empty sums
+        return np.zeros((len(tokens), H), np.float64)
     first = next(a for a in Wg if a is not None)
     I = first.shape[0]
     wdt = w_dtype_of(first)
