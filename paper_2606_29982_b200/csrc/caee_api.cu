@@ -95,6 +95,21 @@ caee_status validate_prune(caee_ctx* c, const caee_prune_params* p) {
   return CAEE_OK;
 }
 
+// E_d as lists: experts grouped by partition, ascending id inside a partition
+caee_status upload_partitions(caee_ctx* c) {
+  const int E = c->d.E, D = c->d.D;
+  std::vector<int32_t> start(D + 1, 0), list(E);
+  for (int e = 0; e < E; ++e) ++start[c->part_h[e] + 1];
+  c->part_max = 0;
+  for (int d = 0; d < D; ++d) { c->part_max = std::max(c->part_max, start[d + 1]); start[d + 1] += start[d]; }
+  std::vector<int32_t> fill(start.begin(), start.end() - 1);
+  for (int e = 0; e < E; ++e) list[fill[c->part_h[e]]++] = e;
+  CAEE_CUDA(c, cudaMemcpy(c->part, c->part_h.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->pl_experts, list.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->pl_start, start.data(), sizeof(int32_t) * (D + 1), cudaMemcpyHostToDevice));
+  return CAEE_OK;
+}
+
 caee_status upload_costs(caee_ctx* c) {
   const int E = c->d.E;
   std::vector<int64_t> w(E);
@@ -118,7 +133,7 @@ caee_status after_launch(caee_ctx* c, const char* what) {
 }
 
 void free_all(caee_ctx* c) {
-  void* ptrs[] = {c->part, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->logits, c->tile_ctr, c->decide_scratch, c->scores, c->idx,
+  void* ptrs[] = {c->part, c->pl_experts, c->pl_start, c->resident, c->w_eff, c->wg, c->wu, c->wd, c->sg, c->su, c->sd, c->partial, c->decide_scratch, c->scores, c->idx,
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
@@ -154,18 +169,17 @@ void free_all(caee_ctx* c) {
 caee_status create_impl(caee_ctx* c) {
   const caee_layer_desc& d = c->d;
   const size_t Tm = d.max_tokens, E = d.E, k = d.k, S = d.S;
-  size_t prow = 1, ntile = 1;
+  size_t prow = 1;
   for (int T = 1; T <= d.max_tokens; ++T) {
     int tt, ks;
-    caee_router_shape(c, T, &tt, &ks);
+    caee_router_shape(c, T, &tt, &ks, nullptr);
     prow = std::max(prow, (size_t)ks * T);
-    ntile = std::max(ntile, (size_t)caee_ceil_div(d.E, 64) * caee_ceil_div(T, tt));
   }
   caee_status rc;
 #define A(ptr, n) if ((rc = dev_alloc(c, &(ptr), (n))) != CAEE_OK) return rc
-  A(c->part, E); A(c->resident, E); A(c->w_eff, E);
+  A(c->part, E); A(c->pl_experts, E); A(c->pl_start, CAEE_MAX_D + 1); A(c->resident, E); A(c->w_eff, E);
   A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
-  A(c->partial, prow * E); A(c->logits, Tm * E); A(c->tile_ctr, ntile); A(c->decide_scratch, caee_decide_scratch_bytes(c)); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
+  A(c->partial, prow * E); A(c->decide_scratch, caee_decide_scratch_bytes(c)); A(c->scores, Tm * E); A(c->idx, Tm * k); A(c->gate, Tm * k);
   A(c->act, E); A(c->must, E); A(c->keep, E); A(c->I_fix, E); A(c->load, CAEE_MAX_D); A(c->scalars, 8);
   c->wl.max_runs = (int)(E + (Tm * k + CAEE_RUN_TOKENS_MIN - 1) / CAEE_RUN_TOKENS_MIN +
                          S * ((Tm + CAEE_RUN_TOKENS_MIN - 1) / CAEE_RUN_TOKENS_MIN));
@@ -193,7 +207,6 @@ caee_status create_impl(caee_ctx* c) {
 #undef A
   if (const char* v = getenv("CAEE_NO_PDL")) c->pdl = atoi(v) == 0;   // tuning aid
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
-  CAEE_CUDA(c, cudaMemset(c->tile_ctr, 0, sizeof(int32_t) * ntile));
   CAEE_CUDA(c, cudaMemset(c->decide_scratch, 0, caee_decide_scratch_bytes(c)));
   CAEE_CUDA(c, cudaMemset(c->scalars, 0, sizeof(int64_t) * 8));
   CAEE_CUDA(c, cudaMemset(c->load, 0, sizeof(int64_t) * CAEE_MAX_D));
@@ -201,7 +214,7 @@ caee_status create_impl(caee_ctx* c) {
   c->part_h.resize(E); c->resident_h.assign(E, 1); c->ticks_res_h.assign(E, 1); c->ticks_miss_h.assign(E, 1);
   const int per = (int)((E + d.D - 1) / d.D);
   for (size_t e = 0; e < E; ++e) c->part_h[e] = (int32_t)(e / per);
-  CAEE_CUDA(c, cudaMemcpy(c->part, c->part_h.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  if ((rc = upload_partitions(c)) != CAEE_OK) return rc;
   if ((rc = upload_costs(c)) != CAEE_OK) return rc;
   CAEE_CUDA(c, cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking));
   CAEE_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
@@ -317,8 +330,7 @@ caee_status caee_set_partitions(caee_ctx* c, const int32_t* part, int32_t D) {
   DeviceGuard g(c->device);
   CAEE_CUDA(c, cudaDeviceSynchronize());
   c->part_h.assign(part, part + c->d.E);
-  CAEE_CUDA(c, cudaMemcpy(c->part, part, sizeof(int32_t) * c->d.E, cudaMemcpyHostToDevice));
-  return CAEE_OK;
+  return upload_partitions(c);
 }
 
 caee_status caee_set_residency(caee_ctx* c, const uint8_t* resident) {

@@ -87,6 +87,9 @@ struct caee_ctx {
   std::vector<uint8_t> resident_h;
   std::vector<int64_t> ticks_res_h, ticks_miss_h;
   int32_t* part = nullptr;      // dev [E]
+  int32_t* pl_experts = nullptr;  // dev [E]   the experts grouped by partition (ascending id inside E_d)
+  int32_t* pl_start = nullptr;    // dev [D+1] where each E_d starts in pl_experts
+  int part_max = 0;               // largest |E_d|: <= 32 lets the decision run one warp per partition (prune_dev.cuh)
   uint8_t* resident = nullptr;  // dev [E]
   int64_t* w_eff = nullptr;     // dev [E] = resident ? ticks_resident : ticks_miss
 
@@ -102,10 +105,8 @@ struct caee_ctx {
   caee_packed packed;
 
   // scratch
-  float* partial = nullptr;  // [ksplit, T, E] split-K partial logits (sized for the worst T)
-  float* logits = nullptr;   // [Tmax, E] x W_r^T
+  float* partial = nullptr;  // [ksplit, T, E] split-K partial logits of x W_r^T (sized for the worst T)
   uint8_t* decide_scratch = nullptr;  // k_decide's self-cleaning accumulators, membership matrix, barriers
-  int32_t* tile_ctr = nullptr;  // per output tile of the router GEMM: CTAs finished (self-resetting)
   float* scores = nullptr;   // [Tmax, E]
   int32_t* idx = nullptr;    // [Tmax, k]
   float* gate = nullptr;     // [Tmax, k]
@@ -178,7 +179,7 @@ caee_status caee_check_cuda(caee_ctx* c, cudaError_t e, const char* what);
 static inline int caee_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 // router.cu
-void caee_router_shape(const caee_ctx* c, int T, int* token_tile, int* ksplit);
+void caee_router_shape(const caee_ctx* c, int T, int* token_tile, int* ksplit, int* k_chunk);
 void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate,
                             cudaStream_t s);

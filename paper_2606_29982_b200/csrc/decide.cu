@@ -43,7 +43,8 @@ constexpr int kWarps = kThreads / 32;         // tokens per CTA
 constexpr int kWords = CAEE_DECIDE_MAX_TOKENS / 32;
 
 struct DecideParams {
-  const float* logits;     // [T,E] x W_r^T (k_router_logits), or NULL with scores_in
+  const float* logits;     // [n_part][T,E] split-K partials of x W_r^T (k_router_logits), or NULL with scores_in
+  int n_part;
   const float* b_logit;
   const float* scores_in;  // [T,E] caller's post-activation scores, or NULL
   const float* corr_bias;
@@ -55,6 +56,8 @@ struct DecideParams {
   double theta, eps;
   const int64_t* w_eff;
   const int32_t* part;
+  const int32_t *pl_experts, *pl_start;   // E_d as lists (prune_dev.cuh)
+  int fast;                               // one warp per partition (largest E_d <= 32)
   const uint8_t* resident;
   uint8_t *act, *must, *keep;
   int64_t *I_fix, *load, *scalars;
@@ -88,7 +91,10 @@ __device__ __forceinline__ void grid_barrier(int* ctr, int G) {
   __syncthreads();
 }
 
-template <int NV>
+// kSingle: the whole step fits ONE CTA (T <= 16).  The accumulators and the membership matrix then
+// live in shared memory, the two grid barriers are block barriers, nothing has to be cleaned up
+// for the next step, and the kernel needs no cooperative launch.
+template <int NV, bool kSingle>
 __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   __shared__ caee_prune_smem sm;
   __shared__ int32_t s_idx[kWarps][32];
@@ -96,6 +102,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   __shared__ int32_t s_est[CAEE_MAX_E];
   __shared__ int s_scan[33 * 6];
   __shared__ int s_last;
+  __shared__ uint32_t s_M[kSingle ? CAEE_MAX_E : 1];     // one 32-bit word per expert covers the <= 16 tokens
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x;
   const int T = p.T, E = p.E, k = p.k;
   const int t = blockIdx.x * kWarps + warp;   // this warp's token
@@ -103,12 +110,25 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   const bool prunes = p.has_prune && p.mode != CAEE_PRUNE_NONE;
   int32_t* ir = s_idx[warp];
   float* gr = s_gate[warp];
+  unsigned long long* acc_I = kSingle ? sm.I : p.acc_I;
+  unsigned char* acc_act = kSingle ? sm.act : p.acc_act;
+  unsigned char* acc_must = kSingle ? sm.must : p.acc_must;
+  uint32_t* M = kSingle ? s_M : p.M;
+  const int mwords = kSingle ? 1 : kWords;
 
   STAMP(0);
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the expert kernel's CTAs may be scheduled (they wait for this grid)
+  // everything up to the first read of the router's partial logits touches only per-layer tables:
+  // with a programmatic dependent launch it overlaps the router GEMM's tail
   float bl[NV], cb[NV];
   caee_load_vec<NV>(p.scores_in ? nullptr : p.b_logit, E, lane, bl);
   caee_load_vec<NV>(p.corr_bias, E, lane, cb);
+  if (p.has_prune && p.fast) caee_prune_preload(sm, E, p.D, p.w_eff, p.part, p.pl_experts, p.pl_start);
+  if (kSingle) {
+    for (int e = tid; e < E; e += kThreads) { sm.I[e] = 0; sm.act[e] = 0; sm.must[e] = 0; s_M[e] = 0; }
+    __syncthreads();
+  }
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the expert kernel's CTAs may be scheduled (they wait for this grid)
   if (blockIdx.x == 0)
     for (int i = tid; i < p.n_sched; i += kThreads) p.wl.sched[i] = 0;
 
@@ -116,7 +136,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   if (live) {
     float s[NV];
     caee_token_scores<NV>(p.scores_in ? p.scores_in + (size_t)t * E : nullptr, p.logits ? p.logits + (size_t)t * E : nullptr,
-                          p.b_logit != nullptr, bl, E, p.score_fn, lane, s);
+                          p.n_part, (size_t)T * E, p.b_logit != nullptr, bl, E, p.score_fn, lane, s);
     if (!p.scores_in && prunes) {
 #pragma unroll
       for (int i = 0; i < NV; ++i) {
@@ -126,21 +146,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
     }
     caee_route_token<NV>(s, p.corr_bias != nullptr, cb, E, k, p.n_group, p.topk_group, p.norm_topk, lane, ir, gr);
     __syncwarp();
-    if (p.has_prune) caee_prune_token(p.mode, p.flags, p.theta, k, ir, gr, lane, p.acc_I, p.acc_act, p.acc_must);
+    if (p.has_prune) caee_prune_token(p.mode, p.flags, p.theta, k, ir, gr, lane, acc_I, acc_act, acc_must);
   }
   STAMP(1);
   if (p.has_prune) {
-    grid_barrier(p.bar + 0, G);
+    if (kSingle) __syncthreads();
+    else grid_barrier(p.bar + 0, G);
     STAMP(2);
     // ---- B: S2-S4 for the batch, redundantly per CTA; CTA 0 writes the result arrays
-    for (int e = tid; e < E; e += kThreads) {
-      sm.I[e] = __ldcg(p.acc_I + e);
-      sm.act[e] = __ldcg(p.acc_act + e);
-      sm.must[e] = __ldcg(p.acc_must + e);
+    if (!kSingle) {
+      for (int e = tid; e < E; e += kThreads) {
+        sm.I[e] = __ldcg(p.acc_I + e);
+        sm.act[e] = __ldcg(p.acc_act + e);
+        sm.must[e] = __ldcg(p.acc_must + e);
+      }
+      __syncthreads();
     }
-    __syncthreads();
-    caee_prune_decide(sm, p.mode, p.flags, p.theta, p.eps, E, p.D, p.w_eff, p.part, blockIdx.x == 0, p.act, p.must, p.keep, p.I_fix, p.load,
-                      p.scalars);
+    if (p.fast)
+      caee_prune_decide_fast(sm, p.mode, p.flags, p.theta, p.eps, E, p.D, blockIdx.x == 0, p.act, p.must, p.keep, p.I_fix, p.load,
+                             p.scalars);
+    else
+      caee_prune_decide(sm, p.mode, p.flags, p.theta, p.eps, E, p.D, p.w_eff, p.part, blockIdx.x == 0, p.act, p.must, p.keep,
+                        p.I_fix, p.load, p.scalars);
     STAMP(3);
     // ---- C: S5 — a token that lost an expert re-selects inside A_trans
     if (live && prunes) {
@@ -160,28 +187,34 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
     const int e = ir[lane];
     p.idx[(size_t)t * k + lane] = e;
     p.gate[(size_t)t * k + lane] = gr[lane];
-    if (e >= 0) atomicOr(p.M + (size_t)e * kWords + (t >> 5), 1u << (t & 31));
+    if (e >= 0) atomicOr(M + (size_t)e * mwords + (t >> 5), 1u << (t & 31));
   }
   STAMP(4);
-  grid_barrier(p.bar + 1, G);
+  if (kSingle) __syncthreads();
+  else grid_barrier(p.bar + 1, G);
   STAMP(5);
 
   // ---- D: S6 — counts and scans per CTA, entries per token, runs/meta/stats by CTA 0
   int cnt = 0;
   if (tid < E) {
-    const uint4* row = reinterpret_cast<const uint4*>(p.M + (size_t)tid * kWords);
+    if (kSingle) {
+      cnt = __popc(s_M[tid]);
+    } else {
+      const uint4* row = reinterpret_cast<const uint4*>(p.M + (size_t)tid * kWords);
 #pragma unroll
-    for (int q = 0; q < kWords / 4; ++q) {
-      const uint4 v = __ldcg(row + q);
-      cnt += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
+      for (int q = 0; q < kWords / 4; ++q) {
+        const uint4 v = __ldcg(row + q);
+        cnt += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
+      }
     }
   }
   caee_wl_scan_block(p.wl, cnt, s_est, p.resident, T, E, p.S, k, blockIdx.x == 0, s_scan);
   __syncthreads();
   STAMP(6);
-  if (live) caee_wl_fill_token(p.wl, p.M, kWords, s_est, ir, gr, t, T, E, p.S, k, lane);
+  if (live) caee_wl_fill_token<kSingle>(p.wl, M, mwords, s_est, ir, gr, t, T, E, p.S, k, lane);
   if (blockIdx.x == 0 && p.stats && tid < 64)
     caee_stats_fill(p.stats, p.scalars, p.load, p.wl.meta, p.D, p.S, p.has_prune, p.bytes_per_expert, 0, tid, 64);
+  if (kSingle) return;
 
   // ---- exit: the last CTA out clears the scratch for the next step
   __syncthreads();
@@ -211,7 +244,8 @@ cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const
                                cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   DecideParams p;
-  p.logits = scores_in ? nullptr : c->logits;
+  p.logits = scores_in ? nullptr : c->partial;
+  { int tt; caee_router_shape(c, T, &tt, &p.n_part, nullptr); }
   p.b_logit = c->b_logit; p.scores_in = scores_in; p.corr_bias = c->corr_bias;
   p.scores = c->scores; p.idx = c->idx; p.gate = c->gate;
   p.T = T; p.E = d.E; p.k = d.k; p.S = d.S; p.D = d.D; p.n_group = d.n_group; p.topk_group = d.topk_group;
@@ -230,13 +264,32 @@ cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const
   const size_t m_off = (E * 10 + 15) & ~(size_t)15;
   p.M = reinterpret_cast<uint32_t*>(z + m_off);
   p.bar = reinterpret_cast<int*>(z + m_off + E * kWords * 4);
+  p.pl_experts = c->pl_experts; p.pl_start = c->pl_start; p.fast = c->part_max <= 32;
   const int nv = caee_ceil_div(d.E, 32);
-  const void* fn = nv <= 1   ? (const void*)k_decide<1>
-                   : nv <= 2 ? (const void*)k_decide<2>
-                   : nv <= 4 ? (const void*)k_decide<4>
-                   : nv <= 8 ? (const void*)k_decide<8>
-                             : (const void*)k_decide<16>;
   void* args[] = {&p};
   ++c->n_launches;
+  if (T <= kWarps) {
+    // one CTA: an ordinary launch, programmatically dependent on the router GEMM (its set-up overlaps that kernel's tail)
+    const void* fn = nv <= 1   ? (const void*)k_decide<1, true>
+                     : nv <= 2 ? (const void*)k_decide<2, true>
+                     : nv <= 4 ? (const void*)k_decide<4, true>
+                     : nv <= 8 ? (const void*)k_decide<8, true>
+                               : (const void*)k_decide<16, true>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(kThreads);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = c->pdl ? 1 : 0;
+    return cudaLaunchKernelExC(&cfg, fn, args);
+  }
+  const void* fn = nv <= 1   ? (const void*)k_decide<1, false>
+                   : nv <= 2 ? (const void*)k_decide<2, false>
+                   : nv <= 4 ? (const void*)k_decide<4, false>
+                   : nv <= 8 ? (const void*)k_decide<8, false>
+                             : (const void*)k_decide<16, false>;
   return cudaLaunchCooperativeKernel(fn, dim3(caee_ceil_div(T, kWarps)), dim3(kThreads), args, 0, st);
 }

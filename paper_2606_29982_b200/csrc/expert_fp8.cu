@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     // ===== weight producer: claims tiles; one 32 KB bulk copy per 128-k stage from the packed image
     if (lane == 0) {
       int stage = 0, ph = 0, q = 0, qph = 0;
+      const uint64_t pol = l2_evict_first_policy();
       for (;;) {
         mbar_wait(qempty0 + 8 * q, qph ^ 1);
         const int i = atomicAdd(p.wl.sched + p.ticket, 1);
@@ -234,7 +235,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, ph ^ 1);
           mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
-          bulk_g2s(smem_base + stage * p.stage_bytes, src + (size_t)kb * kAStageBytes, kAStageBytes, full0 + 8 * stage);
+          bulk_g2s_stream(smem_base + stage * p.stage_bytes, src + (size_t)kb * kAStageBytes, kAStageBytes, full0 + 8 * stage, pol);
           if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
         }
       }

@@ -13,20 +13,29 @@ namespace {
 
 constexpr int PRUNE_THREADS = 512;
 
+struct PartLists {
+  const int32_t* experts;   // [E] experts grouped by partition
+  const int32_t* start;     // [D+1]
+  int fast;                 // largest partition <= 32 experts: one warp per partition (caee_prune_decide_fast)
+};
+
 __global__ void __launch_bounds__(PRUNE_THREADS) k_prune(int mode, int flags, double theta, double eps, int T, int E, int k, int D,
                                                          const int32_t* __restrict__ idx, const float* __restrict__ gate,
                                                          const int64_t* __restrict__ w_eff, const int32_t* __restrict__ part,
+                                                         const PartLists pl,
                                                          uint8_t* __restrict__ act_o, uint8_t* __restrict__ must_o,
                                                          uint8_t* __restrict__ keep_o, int64_t* __restrict__ I_o,
                                                          int64_t* __restrict__ load_o, int64_t* __restrict__ scalars) {
   __shared__ caee_prune_smem sm;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int e = tid; e < E; e += PRUNE_THREADS) { sm.I[e] = 0; sm.act[e] = 0; sm.must[e] = 0; }
+  if (pl.fast) caee_prune_preload(sm, E, D, w_eff, part, pl.experts, pl.start);
   __syncthreads();
   for (int t = warp; t < T; t += PRUNE_THREADS / 32)
     caee_prune_token(mode, flags, theta, k, idx + (size_t)t * k, gate + (size_t)t * k, lane, sm.I, sm.act, sm.must);
   __syncthreads();
-  caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  if (pl.fast) caee_prune_decide_fast(sm, mode, flags, theta, eps, E, D, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  else caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
 // Large steps: S2 and the per-token rules by one warp per token over many CTAs, into the global
@@ -44,7 +53,8 @@ __global__ void __launch_bounds__(256) k_prune_accum(int mode, int flags, double
 __global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, int flags, double theta, double eps, int E, int D,
                                                                   unsigned long long* acc_I, unsigned char* acc_act,
                                                                   unsigned char* acc_must, const int64_t* __restrict__ w_eff,
-                                                                  const int32_t* __restrict__ part, uint8_t* __restrict__ act_o,
+                                                                  const int32_t* __restrict__ part, const PartLists pl,
+                                                                  uint8_t* __restrict__ act_o,
                                                                   uint8_t* __restrict__ must_o, uint8_t* __restrict__ keep_o,
                                                                   int64_t* __restrict__ I_o, int64_t* __restrict__ load_o,
                                                                   int64_t* __restrict__ scalars) {
@@ -53,8 +63,10 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_prune_from_acc(int mode, int 
     sm.I[e] = __ldcg(acc_I + e); sm.act[e] = __ldcg(acc_act + e); sm.must[e] = __ldcg(acc_must + e);
     acc_I[e] = 0; acc_act[e] = 0; acc_must[e] = 0;
   }
+  if (pl.fast) caee_prune_preload(sm, E, D, w_eff, part, pl.experts, pl.start);
   __syncthreads();
-  caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  if (pl.fast) caee_prune_decide_fast(sm, mode, flags, theta, eps, E, D, true, act_o, must_o, keep_o, I_o, load_o, scalars);
+  else caee_prune_decide(sm, mode, flags, theta, eps, E, D, w_eff, part, true, act_o, must_o, keep_o, I_o, load_o, scalars);
 }
 
 template <int NV>
@@ -80,6 +92,7 @@ __global__ void __launch_bounds__(128) k_compensate(const float* __restrict__ sc
 void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, double eps, int T, const int32_t* idx,
                        const float* gate, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
+  const PartLists pl = {c->pl_experts, c->pl_start, c->part_max <= 32};
   c->n_launches += T > 512 ? 2 : 1;
   if (T > 512) {
     // the token pass of a prefill-size step takes ~100 us on one CTA: spread it over the GPU
@@ -88,11 +101,11 @@ void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, double ep
     unsigned char* acc_act = c->decide_scratch + E * 8;
     unsigned char* acc_must = c->decide_scratch + E * 9;
     k_prune_accum<<<caee_ceil_div(T, 8), 256, 0, st>>>(mode, flags, theta, T, d.k, idx, gate, acc_I, acc_act, acc_must);
-    k_prune_from_acc<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, d.E, d.D, acc_I, acc_act, acc_must, c->w_eff, c->part, c->act,
+    k_prune_from_acc<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, d.E, d.D, acc_I, acc_act, acc_must, c->w_eff, c->part, pl, c->act,
                                                   c->must, c->keep, c->I_fix, c->load, c->scalars);
     return;
   }
-  k_prune<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, T, d.E, d.k, d.D, idx, gate, c->w_eff, c->part, c->act,
+  k_prune<<<1, PRUNE_THREADS, 0, st>>>(mode, flags, theta, eps, T, d.E, d.k, d.D, idx, gate, c->w_eff, c->part, pl, c->act,
                                        c->must, c->keep, c->I_fix, c->load, c->scalars);
 }
 

@@ -1,8 +1,9 @@
 // router.cu — S0 router scores and S1 group-limited top-k + gates (router
 // form per DESIGN.md reading R1).  Plain fp32 ALUs: E <= 512 and the GEMV is a few MB.
 //
-//  k_router_logits : split-K partial logits  partial[ks][t][e] = sum_{h in chunk ks} x[t,h] W_r[e,h],
-//                    reduced in ascending ks by the last CTA of each tile (deterministic scores)
+//  k_router_logits : split-K partial logits  partial[ks][t][e] = sum_{h in chunk ks} x[t,h] W_r[e,h];
+//                    the consumer (caee_token_scores, warp_select.cuh) adds the partials of its token
+//                    in ascending ks: deterministic scores, no reduction tail in this kernel
 //  k_route_topk    : one warp per token: activation, selection, gates (steps > 256 tokens and
 //                    caee_route; decode-size steps run the same code inside k_decide, decide.cu).
 #include "caee_internal.cuh"
@@ -38,21 +39,17 @@ __device__ __forceinline__ void cp_async16(void* dst, const void* src, bool vali
 
 // Split-K router GEMM  logit[t,e] = sum_h x[t,h] W_r[e,h]  (S0).
 // Grid (E/64, T/TT, ksplit); CTA tile 64 experts x TT tokens, thread tile 4 x TT/16, fp32 FMAs in
-// ascending h.  W_r and x tiles stream through a cp.async ring (3-4 stages in flight: the
-// weights are cold in L2 every step, the expert stream has flushed them).  Each CTA writes its
-// partial tile; the LAST CTA of a tile to finish (ticket counter) adds the ksplit partials in
-// ascending ks and writes the logits, so the result does not depend on which CTA came last:
-// scores are deterministic.
+// ascending h.  W_r and x tiles stream through a cp.async ring (3-4 stages in flight).  Each CTA
+// writes its partial tile and is done.
 template <typename XT, int TT>
 __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x, const float* __restrict__ Wr,
-                                                       float* __restrict__ partial, float* __restrict__ logits,
-                                                       int* __restrict__ tile_ctr, int T, int H, int E, int Hs) {
+                                                       float* __restrict__ partial, int T, int H, int E, int Hs) {
   using XR = XTraits<XT>;
   constexpr int TPT = TT / 16, NS = TT >= 64 ? (sizeof(XT) == 4 ? 2 : 3) : XR::kStages;   // static shared memory stays below 48 KB
   constexpr int kStageBytes = TE * WROW + TT * XR::kRow;
   __shared__ __align__(16) uint8_t ring[NS * kStageBytes];
-  __shared__ int last_s;
-  const int e0 = blockIdx.x * TE, t0 = blockIdx.y * TT, ks = blockIdx.z, ksplit = gridDim.z;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the decision kernel may set itself up (it waits for this grid)
+  const int e0 = blockIdx.x * TE, t0 = blockIdx.y * TT, ks = blockIdx.z;
   const int h_lo = ks * Hs, h_hi = min(H, h_lo + Hs);
   const int n_it = h_hi > h_lo ? (h_hi - h_lo + KC - 1) / KC : 0;
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -112,7 +109,7 @@ __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x,
   }
   asm volatile("cp.async.wait_group 0;" ::: "memory");
   // thread (tx, ty) holds experts e0 + tx + 16 j, tokens t0 + ty*TPT + i
-  float* out = ksplit == 1 ? logits : partial + (size_t)ks * T * E;
+  float* out = partial + (size_t)ks * T * E;
 #pragma unroll
   for (int i = 0; i < TPT; ++i) {
     const int t = t0 + ty * TPT + i;
@@ -122,79 +119,10 @@ __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x,
       if (t < T && e < E) out[(size_t)t * E + e] = acc[i][j];
     }
   }
-  if (ksplit == 1) return;
-  // tile ticket: the last CTA to arrive reduces the tile (threadFenceReduction pattern)
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) {
-    int* ctr = tile_ctr + blockIdx.y * gridDim.x + blockIdx.x;
-    const int prev = atomicAdd(ctr, 1);
-    last_s = prev == ksplit - 1;
-    if (last_s) *ctr = 0;   // ready for the next step
-  }
-  __syncthreads();
-  if (!last_s) return;
-  __threadfence();
-  // fixed summation tree: R threads per output quad each add a contiguous range of ks in
-  // ascending order, then the R range sums are added in ascending order
-  const int nt = min(TT, T - t0), items = nt * (TE / 4);
-  int R = 1;
-  while (R * 2 * items <= 256 && R * 2 <= ksplit) R *= 2;
-  const int L = (ksplit + R - 1) / R;
-  float4* part_s = reinterpret_cast<float4*>(ring);
-  if ((E & 3) == 0) {
-    for (int u = tid; u < items * R; u += 256) {
-      const int i = u / R, r = u - i * R;
-      const int t = t0 + i / (TE / 4), e = e0 + (i % (TE / 4)) * 4;
-      float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (e + 3 < E) {
-        const int s_lo = r * L, s_hi = min(ksplit, s_lo + L);
-        const float* src = partial + (size_t)t * E + e;
-        const size_t stride = (size_t)T * E;
-        int sk = s_lo;
-        for (; sk + 4 <= s_hi; sk += 4) {
-          const float4 v0 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 0) * stride));
-          const float4 v1 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 1) * stride));
-          const float4 v2 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 2) * stride));
-          const float4 v3 = __ldcg(reinterpret_cast<const float4*>(src + (sk + 3) * stride));
-          a.x += v0.x; a.y += v0.y; a.z += v0.z; a.w += v0.w;
-          a.x += v1.x; a.y += v1.y; a.z += v1.z; a.w += v1.w;
-          a.x += v2.x; a.y += v2.y; a.z += v2.z; a.w += v2.w;
-          a.x += v3.x; a.y += v3.y; a.z += v3.z; a.w += v3.w;
-        }
-        for (; sk < s_hi; ++sk) {
-          const float4 v = __ldcg(reinterpret_cast<const float4*>(src + sk * stride));
-          a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
-        }
-      }
-      if (R == 1) { if (e + 3 < E) *reinterpret_cast<float4*>(logits + (size_t)t * E + e) = a; }
-      else part_s[u] = a;
-    }
-    if (R > 1) {
-      __syncthreads();
-      for (int i = tid; i < items; i += 256) {
-        const int t = t0 + i / (TE / 4), e = e0 + (i % (TE / 4)) * 4;
-        float4 a = part_s[i * R];
-        for (int r = 1; r < R; ++r) {
-          const float4 v = part_s[i * R + r];
-          a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
-        }
-        if (e + 3 < E) *reinterpret_cast<float4*>(logits + (size_t)t * E + e) = a;
-      }
-    }
-  } else {
-    for (int i = tid; i < nt * TE; i += 256) {
-      const int t = t0 + i / TE, e = e0 + i % TE;
-      if (e >= E) continue;
-      float a = 0.f;
-      for (int sk = 0; sk < ksplit; ++sk) a += __ldcg(partial + ((size_t)sk * T + t) * E + e);
-      logits[(size_t)t * E + e] = a;
-    }
-  }
 }
 
 template <int NV>
-__global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ logits, const float* __restrict__ b_logit,
+__global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ logits, int n_part, const float* __restrict__ b_logit,
                                                     const float* __restrict__ scores_in,
                                                     const float* __restrict__ corr_bias, float* __restrict__ scores_out,
                                                     int32_t* __restrict__ idx, float* __restrict__ gate, int T, int E, int k,
@@ -206,7 +134,7 @@ __global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ lo
   caee_load_vec<NV>(b_logit, E, lane, bl);
   caee_load_vec<NV>(corr_bias, E, lane, cb);
   caee_token_scores<NV>(scores_in ? scores_in + (size_t)t * E : nullptr, logits ? logits + (size_t)t * E : nullptr,
-                        b_logit != nullptr, bl, E, score_fn, lane, s);
+                        n_part, (size_t)T * E, b_logit != nullptr, bl, E, score_fn, lane, s);
   if (scores_out) {
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
@@ -220,33 +148,39 @@ __global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ lo
 template <int NV>
 void launch_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
-  k_route_topk<NV><<<caee_ceil_div(T, 4), 128, 0, st>>>(c->logits, c->b_logit, scores_in, c->corr_bias, scores_out, idx, gate,
+  int tt, ks;
+  caee_router_shape(c, T, &tt, &ks, nullptr);
+  k_route_topk<NV><<<caee_ceil_div(T, 4), 128, 0, st>>>(c->partial, ks, c->b_logit, scores_in, c->corr_bias, scores_out, idx, gate,
                                                          T, d.E, d.k, d.n_group, d.topk_group, d.score_fn, d.norm_topk);
 }
 
 template <typename XT>
 void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
-  int tt, ks;
+  int tt, ks, Hs;
   ++c->n_launches;
-  caee_router_shape(c, T, &tt, &ks);
-  const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), KC) * KC;
+  caee_router_shape(c, T, &tt, &ks, &Hs);
   dim3 grid(caee_ceil_div(d.E, TE), caee_ceil_div(T, tt), ks);
-  if (tt == 16) k_router_logits<XT, 16><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
-  else if (tt == 64) k_router_logits<XT, 64><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
-  else k_router_logits<XT, 32><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, c->logits, c->tile_ctr, T, d.H, d.E, Hs);
+  if (tt == 16) k_router_logits<XT, 16><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
+  else if (tt == 64) k_router_logits<XT, 64><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
+  else k_router_logits<XT, 32><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
 }
 
 }  // namespace
 
-// Token tile and split-K factor for a T-token step: about two CTAs per SM, K chunks >= 128.
-void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit) {
+// Token tile and split-K factor for a T-token step: about one CTA per SM for decode-size steps (every
+// partial is read back by the step's decision kernel), two for larger ones; K chunks >= 128.  The
+// split actually used is the number of non-empty chunks of Hs = ceil(H / ksplit) rounded up to KC.
+void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit, int* hs) {
   const caee_layer_desc& d = c->d;
   *tt = T <= 16 ? 16 : (T >= 1024 ? 64 : 32);   // prefill-size steps: 4 x 4 outputs per thread (more FMAs per shared-memory load)
   const int tiles = caee_ceil_div(d.E, TE) * caee_ceil_div(T, *tt);
-  const int want = caee_ceil_div(2 * c->num_sms, tiles);
+  const int want = caee_ceil_div((T <= 256 ? 1 : 2) * c->num_sms, tiles);
   const int maxk = d.H / 128 > 0 ? d.H / 128 : 1;
-  *ksplit = want < 1 ? 1 : (want > maxk ? maxk : want);
+  int ks = want < 1 ? 1 : (want > maxk ? maxk : want);
+  const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), KC) * KC;
+  *ksplit = caee_ceil_div(d.H, Hs);
+  if (hs) *hs = Hs;
 }
 
 void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t st) {

@@ -19,13 +19,15 @@ __device__ __forceinline__ bool caee_before(float va, int ia, float vb, int ib) 
   return va > vb || (va == vb && ia < ib);
 }
 
-__device__ __forceinline__ void caee_warp_argmax(float& v, int& id) {
-#pragma unroll
-  for (int o = 16; o; o >>= 1) {
-    float ov = __shfl_xor_sync(0xffffffffu, v, o);
-    int oi = __shfl_xor_sync(0xffffffffu, id, o);
-    if (caee_before(ov, oi, v, id)) { v = ov; id = oi; }
-  }
+// Order-preserving map float -> uint32 (a > b  <=>  key(a) > key(b), a == b <=> key(a) == key(b) for
+// non-NaN values; -0 is folded into +0 first).  Keys of real scores are >= 1, so 0 can mean "none".
+// It lets a warp take a maximum with ONE redux.sync instead of a five-step shuffle butterfly.
+__device__ __forceinline__ uint32_t caee_okey(float v) {
+  const uint32_t u = __float_as_uint(__fadd_rn(v, 0.0f));
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float caee_okey_inv(uint32_t k) {
+  return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
 // Group-limited routing: group score = sum of the two largest s' in the group; the
@@ -39,6 +41,41 @@ __device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint3
 #pragma unroll
   for (int i = 0; i < NV; ++i) grp[i] = ((ok >> i) & 1u) ? (lane + 32 * i) / gs : -1;
   float my_gscore = -INFINITY;  // lane g holds the score of group g
+  if (gs == 32 && n_group <= NV) {
+    // Register slot i is exactly group i.  The two largest s' of a group by two warp maxima over
+    // order-preserving keys (redux.sync), written branch-free so that the NV groups' reductions
+    // issue back to back; the sum of two floats does not depend on their order.  The results are
+    // warp-uniform, so every lane ranks "its" group (lane g < n_group) against all of them without a
+    // shuffle, and with slot == group the allowed-slot mask is the ballot of the kept groups itself.
+    uint32_t key[NV], m1[NV], m2[NV];
+    bool dup[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) key[i] = grp[i] >= 0 ? caee_okey(sp[i]) : 0u;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) m1[i] = __reduce_max_sync(0xffffffffu, key[i]);
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const unsigned eq = __ballot_sync(0xffffffffu, key[i] == m1[i]);
+      dup[i] = (eq & (eq - 1u)) != 0u;                 // the maximum occurs at least twice
+    }
+#pragma unroll
+    for (int i = 0; i < NV; ++i) m2[i] = __reduce_max_sync(0xffffffffu, key[i] == m1[i] ? 0u : key[i]);
+    float gsc[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const uint32_t second = dup[i] ? m1[i] : m2[i];
+      const float a = caee_okey_inv(m1[i]), bsum = __fadd_rn(a, caee_okey_inv(second));
+      gsc[i] = m1[i] == 0u ? -INFINITY : (second == 0u ? a : bsum);
+    }
+    float mine = -INFINITY;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) mine = lane == i ? gsc[i] : mine;
+    int before = 0;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) before += (i < n_group) & ((gsc[i] > mine) | ((gsc[i] == mine) & (i < lane)));
+    const uint32_t gsel = __ballot_sync(0xffffffffu, lane < n_group && before < topk_group);
+    return gsel & ok;
+  }
   // top-2 merge of two (m1 >= m2) pairs
 #define CAEE_TOP2_MERGE(m1, m2, o1, o2)                   \
   do {                                                    \
@@ -120,31 +157,44 @@ __device__ __forceinline__ uint32_t caee_group_mask(const float (&sp)[NV], uint3
 
 // Top-k of sp over the allowed slots, listed in descending order; gates from s.
 // Writes idx_out[0..k) (-1 for empty slots) and gate_out[0..k).  k <= 32.
+// Each of the k rounds is: per-lane maximum over its slots (strict '>' keeps the lower slot = lower
+// id on ties), one redux.sync max over the warp, one redux.sync min over the ids that hold it
+// (ties -> lower id, R22), one shuffle for the winner's unbiased score.
 template <int NV>
 __device__ __forceinline__ void caee_warp_select(const float (&s)[NV], const float (&sp)[NV], uint32_t ok, int k,
                                                  int norm_topk, int lane, int32_t* idx_out, float* gate_out) {
+  uint32_t key[NV];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) key[i] = ((ok >> i) & 1u) ? caee_okey(sp[i]) : 0u;
   int sel_e = -1;
   float sel_s = 0.f;
   for (int j = 0; j < k; ++j) {
-    float bv = -INFINITY;
-    int bi = CAEE_NONE_ID;
+    // per-lane maximum as a tree; on equal keys the lower slot (= lower id) stays
+    uint32_t tk[NV];
+    int ti[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) { tk[i] = key[i]; ti[i] = i; }
+#pragma unroll
+    for (int w = 1; w < NV; w *= 2) {
+#pragma unroll
+      for (int i = 0; i + w < NV; i += 2 * w) {
+        const bool up = tk[i + w] > tk[i];
+        tk[i] = up ? tk[i + w] : tk[i];
+        ti[i] = up ? ti[i + w] : ti[i];
+      }
+    }
+    const uint32_t m = __reduce_max_sync(0xffffffffu, tk[0]);
+    // m == 0: nothing left (fewer than k allowed experts) — win = 0xffffffff then matches no lane and no slot
+    const uint32_t win = __reduce_min_sync(0xffffffffu, (tk[0] == m && m != 0u) ? (uint32_t)(lane + 32 * ti[0]) : 0xffffffffu);
+    float mine = 0.f;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      int e = lane + 32 * i;
-      if (((ok >> i) & 1u) && caee_before(sp[i], e, bv, bi)) { bv = sp[i]; bi = e; }
+      const bool hit = win == (uint32_t)(lane + 32 * i);
+      mine = hit ? s[i] : mine;
+      key[i] = hit ? 0u : key[i];
     }
-    caee_warp_argmax(bv, bi);
-    float ws = 0.f;
-    if (bi != CAEE_NONE_ID) {
-      int owner = bi & 31, slot = bi >> 5;
-      float mine = 0.f;
-#pragma unroll
-      for (int i = 0; i < NV; ++i)
-        if (i == slot) mine = s[i];
-      ws = __shfl_sync(0xffffffffu, mine, owner);
-      if (lane == owner) ok &= ~(1u << slot);
-    }
-    if (lane == j) { sel_e = bi == CAEE_NONE_ID ? -1 : bi; sel_s = ws; }
+    const float ws = __shfl_sync(0xffffffffu, mine, win & 31);
+    if (lane == j) { sel_e = (int)win; sel_s = ws; }      // 0xffffffff == -1: an empty slot
   }
   float sum = 0.f;
   for (int j = 0; j < k; ++j) {
@@ -171,10 +221,13 @@ __device__ __forceinline__ void caee_load_vec(const float* __restrict__ p, int E
   }
 }
 
+// logits_row: the token's row of the first split-K partial of the router GEMM; n_part partials lie
+// part_stride floats apart and are added here in ascending order (a fixed order: the scores are a
+// deterministic function of x and W_r whatever the schedule of the GEMM's CTAs was).
 template <int NV>
 __device__ __forceinline__ void caee_token_scores(const float* __restrict__ scores_row, const float* __restrict__ logits_row,
-                                                  bool has_bl, const float (&bl)[NV], int E, int score_fn, int lane,
-                                                  float (&s)[NV]) {
+                                                  int n_part, size_t part_stride, bool has_bl, const float (&bl)[NV], int E,
+                                                  int score_fn, int lane, float (&s)[NV]) {
   RSTAMP(0);
   if (scores_row) {
 #pragma unroll
@@ -189,7 +242,33 @@ __device__ __forceinline__ void caee_token_scores(const float* __restrict__ scor
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     int e = lane + 32 * i;
-    l[i] = e < E ? logits_row[e] : 0.f;
+    l[i] = e < E ? __ldcg(logits_row + e) : 0.f;
+  }
+  // four partials' loads in flight at a time, added in ascending order
+  int q = 1;
+  for (; q + 4 <= n_part; q += 4) {
+    float v[4][NV];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const float* pr = logits_row + (size_t)(q + u) * part_stride;
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        int e = lane + 32 * i;
+        v[u][i] = e < E ? __ldcg(pr + e) : 0.f;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int i = 0; i < NV; ++i) l[i] = __fadd_rn(l[i], v[u][i]);
+  }
+  for (; q < n_part; ++q) {
+    const float* pr = logits_row + (size_t)q * part_stride;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      int e = lane + 32 * i;
+      if (e < E) l[i] = __fadd_rn(l[i], __ldcg(pr + e));
+    }
   }
 #pragma unroll
   for (int i = 0; i < NV; ++i) {

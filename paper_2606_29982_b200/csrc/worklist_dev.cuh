@@ -130,6 +130,8 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
 // Decode-size fill (T <= 256): M is the E x W bit matrix "expert e is in K_final of token t"
 // (W = 8 words per expert), so an entry's place in its expert's list is a popcount.
 // One warp, one token: lanes j < k place the token's routed entries, lanes s < S the shared ones.
+// kShared: M lives in shared memory (the one-CTA step), else in global memory behind a grid barrier.
+template <bool kShared>
 __device__ __forceinline__ void caee_wl_fill_token(const caee_worklist& wl, const uint32_t* M, int W, const int32_t* estart,
                                                    const int32_t* ir, const float* gr, int t, int T, int E, int S, int k,
                                                    int lane) {
@@ -139,8 +141,8 @@ __device__ __forceinline__ void caee_wl_fill_token(const caee_worklist& wl, cons
     if (e >= 0) {
       const uint32_t* row = M + (size_t)e * W;
       int pos = estart[e];
-      for (int w = 0; w < (t >> 5); ++w) pos += __popc(__ldcg(row + w));
-      pos += __popc(__ldcg(row + (t >> 5)) & ((1u << (t & 31)) - 1u));
+      for (int w = 0; w < (t >> 5); ++w) pos += __popc(kShared ? row[w] : __ldcg(row + w));
+      pos += __popc((kShared ? row[t >> 5] : __ldcg(row + (t >> 5))) & ((1u << (t & 31)) - 1u));
       wl.ent_tok[pos] = t;
       wl.ent_slot[pos] = lane;
       wl.ent_wt[pos] = gr[lane];

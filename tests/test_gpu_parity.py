@@ -64,9 +64,11 @@ def test_route_scores_and_selection(H, cfg):
 
 
 R1B = wl.scaled(R1S, name="R1-small-bias", corr_bias_std=0.3)    # the route's list order != gate order on most tokens (R36)
+# one partition of 64 experts: partitions of more than 32 experts take the block-wide decision code, the others one warp per partition
+C2W = wl.scaled(wl.C2, name="C2-one-partition", H=256, I=128, S=0, D=1)
 
 
-@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, R1B], ids=lambda c: c.name)
+@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, R1B, C2W], ids=lambda c: c.name)
 @pytest.mark.parametrize("mode", list(MODES))
 def test_prune_compensate_compact_bit_exact(H, cfg, mode):
     from paper_2606_29982_b200 import binding as B
@@ -199,7 +201,7 @@ def test_compact_large_step_segmented_fill(H, mode):
         L.close()
 
 
-@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, R1B, wl.scaled(wl.C3, name="R1-router", H=256, I=128)], ids=lambda c: c.name)
+@pytest.mark.parametrize("cfg", [wl.C1, C2S, R1S, R1B, C2W, wl.scaled(wl.C3, name="R1-router", H=256, I=128)], ids=lambda c: c.name)
 @pytest.mark.parametrize("mode", ["dense"] + list(MODES))
 def test_forward_decisions_bit_exact_fused_and_standalone(H, cfg, mode):
     """caee_moe_forward takes the one-kernel decision path (decide.cu) up to 256 tokens and the
