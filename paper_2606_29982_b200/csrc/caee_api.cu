@@ -575,6 +575,10 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs, dp, sizeof(void*) * n, cudaMemcpyHostToDevice, st));
   }
   const bool fused = caee_decide_fits(c, T);
+  // e4m3 decode steps: the split of x into its two e4m3 terms depends on x alone, so it goes first and
+  // the chain router GEMM -> decision kernel -> expert kernel stays free for programmatic dependent launches
+  const bool early_prep = c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && c->wl.run_cap != CAEE_RUN_TOKENS_WIDE;
+  if (early_prep) caee_launch_umma_prepare(c, x, T, st);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
     if (!scores) caee_launch_router_logits(c, x, T, st);
@@ -590,7 +594,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
     caee_launch_expert_simt(c, x, T, st);
   } else if (!c->any_offload) {
-    caee_launch_umma_prepare(c, x, T, st);
+    if (!early_prep) caee_launch_umma_prepare(c, x, T, st);
     if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
     if ((rc = caee_launch_expert_umma(c, x, T, 0, -1, 0, st)) != CAEE_OK) return rc;
   } else {
@@ -598,7 +602,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     // fetched, one cudaMemcpyAsync each on the side stream, while the resident experts (first
     // in the run list) are already computing on the caller's stream.  The host has to learn
     // which experts survived: this is the one host synchronisation of an offloading step.
-    caee_launch_umma_prepare(c, x, T, st);
+    if (!early_prep) caee_launch_umma_prepare(c, x, T, st);
     CAEE_CUDA(c, cudaMemcpyAsync(c->host_meta, c->wl.meta, sizeof(int32_t) * 16, cudaMemcpyDeviceToHost, st));
     CAEE_CUDA(c, cudaMemcpyAsync(c->host_meta + 16, c->wl.run_expert, sizeof(int32_t) * c->wl.max_runs, cudaMemcpyDeviceToHost, st));
     CAEE_CUDA(c, cudaStreamSynchronize(st));

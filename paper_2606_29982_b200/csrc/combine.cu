@@ -19,15 +19,26 @@ template <typename YT>
 __global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf, const int32_t* __restrict__ idx,
                                                  const float* __restrict__ gate, YT* __restrict__ y, int H, int k, int S,
                                                  float routed_scale) {
-  asm volatile("griddepcontrol.wait;" ::: "memory");   // programmatic dependent launch: the expert kernel is done
+  // K_final and the gates were complete before the expert kernel started: fetch them while it still runs
+  __shared__ int s_idx[32];
+  __shared__ float s_gate[32];
   const int t = blockIdx.y, c = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (threadIdx.x < k) {
+    const int e = idx[(size_t)t * k + threadIdx.x];
+    s_idx[threadIdx.x] = e;
+    s_gate[threadIdx.x] = e >= 0 ? gate[(size_t)t * k + threadIdx.x] : 0.f;
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // programmatic dependent launch: the expert kernel is done
   if (c >= H) return;
   const int KS = k + S;
   float4 acc = {0.f, 0.f, 0.f, 0.f};
+  const float* orow = obuf + (size_t)t * KS * H + c;
+#pragma unroll 4
   for (int j = 0; j < k; ++j) {
-    if (idx[(size_t)t * k + j] < 0) continue;
-    const float g = gate[(size_t)t * k + j];
-    const float4 o = *reinterpret_cast<const float4*>(obuf + ((size_t)t * KS + j) * H + c);
+    if (s_idx[j] < 0) continue;            // an empty slot's row was never written
+    const float g = s_gate[j];
+    const float4 o = *reinterpret_cast<const float4*>(orow + (size_t)j * H);
     acc.x = fmaf(g, o.x, acc.x); acc.y = fmaf(g, o.y, acc.y); acc.z = fmaf(g, o.z, acc.z); acc.w = fmaf(g, o.w, acc.w);
   }
   acc.x *= routed_scale; acc.y *= routed_scale; acc.z *= routed_scale; acc.w *= routed_scale;

@@ -187,7 +187,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
   const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[kMaxStages]);
   const uint32_t tfull0 = smem_u32(&bars[2 * kMaxStages]), tempty0 = smem_u32(&bars[2 * kMaxStages + 2]);
   const uint32_t qfull0 = smem_u32(&bars[2 * kMaxStages + 4]), qempty0 = smem_u32(&bars[2 * kMaxStages + 4 + kQueue]);
-  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < p.n_stages; ++s) {
@@ -214,6 +213,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  // everything above touched only shared memory and TMEM: with a programmatic dependent launch it
+  // overlaps the decision kernel's tail; the work list exists from here on
+  griddep_wait();
+  griddep_launch();
+  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
   TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
   Tile t;
 
@@ -584,5 +588,19 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
     c->attr_done |= 2u;
   }
   ++c->n_launches;
+  if (c->pdl && !c->any_offload) {
+    // programmatic dependent launch behind the decision kernel (the x split runs before the router GEMM)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)c->num_sms);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = dyn;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k_expert_fp8, p);
+    return;
+  }
   k_expert_fp8<<<c->num_sms, kThreads, dyn, st>>>(p);
 }

@@ -121,6 +121,83 @@ __global__ void __launch_bounds__(256) k_router_logits(const XT* __restrict__ x,
   }
 }
 
+// The same partial logits for steps of at most 4 tokens, where the tile kernel above would spend its
+// time on padding tokens: a bandwidth-shaped GEMV.  CTA tile 16 experts x TT tokens; a stage holds 128
+// k of the 16 rows (8 KB, cp.async ring); thread (tx = expert, ty = one of 16 k-octets of the stage)
+// multiplies its 8 k in ascending order; the 16 octet sums of an output are added in ascending ty
+// through shared memory at the end (a fixed order).  Grid (E/16, ksplit): about one CTA per SM, and
+// only ~8 partials for the decision kernel to add.
+constexpr int SE = 16, SKC = 128, SWROW = SKC * 4 + 16, SNS = 4;
+template <typename XT, int TT>
+__global__ void __launch_bounds__(256) k_router_small(const XT* __restrict__ x, const float* __restrict__ Wr,
+                                                      float* __restrict__ partial, int T, int H, int E, int Hs) {
+  constexpr int kXRow = SKC * (int)sizeof(XT) + 16;
+  constexpr int kStageBytes = SE * SWROW + TT * kXRow;
+  __shared__ __align__(16) uint8_t ring[SNS * kStageBytes];
+  __shared__ float red[16][TT][SE + 1];
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the decision kernel may set itself up (it waits for this grid)
+  const int e0 = blockIdx.x * SE, ks = blockIdx.y;
+  const int h_lo = ks * Hs, h_hi = min(H, h_lo + Hs);
+  const int n_it = h_hi > h_lo ? (h_hi - h_lo + SKC - 1) / SKC : 0;
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  float acc[TT];
+#pragma unroll
+  for (int t = 0; t < TT; ++t) acc[t] = 0.f;
+  auto issue = [&](int it) {
+    if (it < n_it) {
+      uint8_t* st = ring + (it % SNS) * kStageBytes;
+      const int h0 = h_lo + it * SKC;
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {   // W tile: 16 rows x 32 chunks of 4 floats
+        const int i = tid + 256 * q, r = i >> 5, c = i & 31;
+        const int e = e0 + r, h = h0 + c * 4;
+        const bool ok = e < E && h < h_hi;
+        cp_async16(st + r * SWROW + c * 16, ok ? Wr + (size_t)e * H + h : Wr, ok);
+      }
+      constexpr int kXChunks = SKC * (int)sizeof(XT) / 16;
+      if (tid < TT * kXChunks) {      // x tile: TT rows of 128 k
+        const int r = tid / kXChunks, c = tid % kXChunks;
+        const int t = r, h = h0 + c * (16 / (int)sizeof(XT));
+        const bool ok = t < T && h < h_hi;
+        cp_async16(st + SE * SWROW + r * kXRow + c * 16, ok ? x + (size_t)t * H + h : x, ok);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+#pragma unroll
+  for (int s = 0; s < SNS - 1; ++s) issue(s);
+  for (int it = 0; it < n_it; ++it) {
+    asm volatile("cp.async.wait_group %0;" ::"n"(SNS - 2) : "memory");
+    __syncthreads();
+    issue(it + SNS - 1);
+    const uint8_t* st = ring + (it % SNS) * kStageBytes;
+    const float4 w0 = *reinterpret_cast<const float4*>(st + tx * SWROW + ty * 32);
+    const float4 w1 = *reinterpret_cast<const float4*>(st + tx * SWROW + ty * 32 + 16);
+#pragma unroll
+    for (int t = 0; t < TT; ++t) {
+      float xv[4], xw[4];
+      const uint8_t* xr = st + SE * SWROW + t * kXRow + ty * 8 * (int)sizeof(XT);
+      XTraits<XT>::ld4(xr, xv);
+      XTraits<XT>::ld4(xr + 4 * (int)sizeof(XT), xw);
+      float a = acc[t];
+      a = fmaf(xv[0], w0.x, a); a = fmaf(xv[1], w0.y, a); a = fmaf(xv[2], w0.z, a); a = fmaf(xv[3], w0.w, a);
+      a = fmaf(xw[0], w1.x, a); a = fmaf(xw[1], w1.y, a); a = fmaf(xw[2], w1.z, a); a = fmaf(xw[3], w1.w, a);
+      acc[t] = a;
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+  for (int t = 0; t < TT; ++t) red[ty][t][tx] = acc[t];
+  __syncthreads();
+  if (tid < TT * SE) {
+    const int t = tid / SE, e = tid % SE;
+    float a = red[0][t][e];
+#pragma unroll
+    for (int q = 1; q < 16; ++q) a += red[q][t][e];
+    if (t < T && e0 + e < E) partial[((size_t)ks * T + t) * E + e0 + e] = a;
+  }
+}
+
 template <int NV>
 __global__ void __launch_bounds__(128) k_route_topk(const float* __restrict__ logits, int n_part, const float* __restrict__ b_logit,
                                                     const float* __restrict__ scores_in,
@@ -160,6 +237,13 @@ void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
   int tt, ks, Hs;
   ++c->n_launches;
   caee_router_shape(c, T, &tt, &ks, &Hs);
+  if (tt <= 4) {
+    dim3 grid(caee_ceil_div(d.E, SE), ks);
+    if (tt == 1) k_router_small<XT, 1><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
+    else if (tt == 2) k_router_small<XT, 2><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
+    else k_router_small<XT, 4><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
+    return;
+  }
   dim3 grid(caee_ceil_div(d.E, TE), caee_ceil_div(T, tt), ks);
   if (tt == 16) k_router_logits<XT, 16><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
   else if (tt == 64) k_router_logits<XT, 64><<<grid, 256, 0, st>>>(x, c->Wr, c->partial, T, d.H, d.E, Hs);
@@ -170,15 +254,18 @@ void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
 
 // Token tile and split-K factor for a T-token step: about one CTA per SM for decode-size steps (every
 // partial is read back by the step's decision kernel), two for larger ones; K chunks >= 128.  The
-// split actually used is the number of non-empty chunks of Hs = ceil(H / ksplit) rounded up to KC.
+// split actually used is the number of non-empty chunks of Hs = ceil(H / ksplit) rounded up to the
+// stage depth.  Steps of at most 4 tokens take the GEMV-shaped kernel (token tile 1, 2 or 4).
 void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit, int* hs) {
   const caee_layer_desc& d = c->d;
-  *tt = T <= 16 ? 16 : (T >= 1024 ? 64 : 32);   // prefill-size steps: 4 x 4 outputs per thread (more FMAs per shared-memory load)
-  const int tiles = caee_ceil_div(d.E, TE) * caee_ceil_div(T, *tt);
+  const bool small = T <= 4;
+  *tt = small ? (T <= 1 ? 1 : (T <= 2 ? 2 : 4)) : (T <= 16 ? 16 : (T >= 1024 ? 64 : 32));   // prefill-size steps: 4 x 4 outputs per thread
+  const int tiles = small ? caee_ceil_div(d.E, SE) : caee_ceil_div(d.E, TE) * caee_ceil_div(T, *tt);
   const int want = caee_ceil_div((T <= 256 ? 1 : 2) * c->num_sms, tiles);
   const int maxk = d.H / 128 > 0 ? d.H / 128 : 1;
   int ks = want < 1 ? 1 : (want > maxk ? maxk : want);
-  const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), KC) * KC;
+  const int kc = small ? SKC : KC;
+  const int Hs = caee_ceil_div(caee_ceil_div(d.H, ks), kc) * kc;
   *ksplit = caee_ceil_div(d.H, Hs);
   if (hs) *hs = Hs;
 }
