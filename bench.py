@@ -8,7 +8,13 @@ BASELINE.json config 3, the DeepSeek-R1-shaped bf16 layer (H 7168, 256+1 experts
 I 2048, 22.5 GB of expert weights in HBM) at a 128-token decode batch.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3] [--tokens 128]
-                    [--prune thresh:0.6] [--impl caee|reference]
+                    [--prune thresh:0.6] [--eps-frac 0.10] [--impl caee|reference]
+
+Default operating point: the paper's on-device knob THRESH theta = 0.6 under the objective's
+importance bound F_imp <= eps with eps = 0.10 T (R37): at most 10% of the batch's
+gate mass may be re-routed, the batch-level counterpart of the paper's theta_imp = 0.9 retention point
+(Table III).  `value` is that step; the same batches without pruning are reported beside it
+under "dense".
 
 N > 1 (under torchrun) runs N independent replicas ("replicas only").
 """
@@ -36,8 +42,10 @@ def parse_prune(s):
     return MODE_IDS[name], float(val or 0)
 
 
-def workload_name(cfg, T, prune):
-    p = "dense top-k" if prune is None else f"CAEE prune {prune}"
+def workload_name(cfg, T, prune, eps=None):
+    p = "dense top-k" if prune in (None, "dense", "off") else f"CAEE prune {prune}"
+    if eps is not None and prune not in (None, "dense", "off"):
+        p += f" under the importance bound F_imp <= {eps:g} (= {eps / T:g} T, PAPER.md:150-152)"
     return (f"{cfg.name}: H={cfg.H} I={cfg.I} E={cfg.E}+{cfg.S} top-{cfg.k} groups {cfg.n_group}/{cfg.topk_group} "
             f"D={cfg.D}, decode batch T={T}, {p}")
 
@@ -108,72 +116,83 @@ def dist_env():
 
 
 # --------------------------------------------------------------------------- CPU oracle legs
-def oracle_sample_run(cfg, T, prune, seed, n_sample, device_for_inputs, layer=None, min_seconds=0.0):
-    """Times the oracle as it stands on the host cores: decisions on all T tokens, FFN + combine on
-    n_sample of them; returns (tokens_per_s extrapolated to T, seconds of CPU work, cores)."""
-    import numpy as np
-    from oracle import oracle as orc
-    from paper_2606_29982_b200 import workloads as wl
-    cores = len(os.sched_getaffinity(0))
-    x = wl.hidden(cfg, T, seed + 100, device_for_inputs)
-    Wr, b_logit, cb = (layer.Wr, layer.b_logit, layer.corr_bias) if layer is not None else wl.router(cfg, seed, device_for_inputs)
-    xb, Wr_h, b_h = wl.bits(x), Wr.cpu().numpy(), b_logit.cpu().numpy()
-    cb_h = None if cb is None else cb.cpu().numpy()
-    part = wl.partitions(cfg)
-    w_eff = orc.effective_cost(wl.residency(cfg, seed), *wl.cost_tables(cfg))
-    t0 = time.perf_counter()
-    s = orc.scores(xb, Wr_h, b_h, cfg.score_fn)
-    idx, gate = orc.route(s, cb_h, cfg.k, cfg.n_group, cfg.topk_group, cfg.norm_topk)
-    if prune is not None:
-        pr = orc.prune(prune[0], prune[1], 0, idx, gate, cfg.E, w_eff, part, cfg.D)
-        if prune[0] != 0:
-            idx, gate = orc.compensate(s, cb_h, pr["keep"], idx, gate, cfg.norm_topk, 0)
-    orc.compact(idx, gate, cfg.E)
-    t_dec = time.perf_counter() - t0
-    tokens = list(range(0, T, max(1, T // n_sample)))[:n_sample]
-    n = cfg.E + cfg.S
-    used = sorted(set(int(e) for t in tokens for e in idx[t] if e >= 0) | set(range(cfg.E, n)))
-    tabs = {k: [None] * n for k in ("gate", "up", "down", "gate_scale", "up_scale", "down_scale")}
-    for e in used:                                   # untimed: fetch the exact bits of the needed experts
-        r = wl.expert_weights(cfg, seed, e, device_for_inputs)
-        for k_, v in r.items():
-            tabs[k_][e] = wl.bits(v)
-    fp8 = cfg.w_dtype == wl.DT_E4M3
-    reps, t_all = 0, 0.0
-    while reps == 0 or (t_all < min_seconds and reps < 64):    # repeat the same sample up to the time budget
+class OracleLayer:
+    """The CPU oracle on the bench workload, as it stands: one timed call = the whole layer step on ALL T
+    tokens (scores -> route -> prune -> compensation -> compaction -> expert FFNs -> combine).  Set-up
+    (drawing x, the router and the exact bits of the experts the step touches) is not timed."""
+
+    def __init__(self, cfg, T, prune, eps, seed, device, layer=None):
+        import numpy as np
+        from oracle import oracle as orc
+        from paper_2606_29982_b200 import workloads as wl
+        self.cfg, self.T, self.prune, self.eps, self.orc, self.wl, self.np = cfg, T, prune, eps, orc, wl, np
+        self.cores = len(os.sched_getaffinity(0))
+        x = wl.hidden(cfg, T, seed * 1000 + 100, device)
+        Wr, b_logit, cb = (layer.Wr, layer.b_logit, layer.corr_bias) if layer is not None else wl.router(cfg, seed, device)
+        self.xb, self.Wr, self.b = wl.bits(x), Wr.cpu().numpy(), b_logit.cpu().numpy()
+        self.cb = None if cb is None else cb.cpu().numpy()
+        self.part = wl.partitions(cfg)
+        self.w_eff = orc.effective_cost(wl.residency(cfg, seed), *wl.cost_tables(cfg))
+        idx, _ = self.decisions()[:2]
+        n = cfg.E + cfg.S
+        used = sorted(set(int(e) for e in idx.ravel() if e >= 0) | set(range(cfg.E, n)))
+        self.tabs = {k: [None] * n for k in ("gate", "up", "down", "gate_scale", "up_scale", "down_scale")}
+        for e in used:                                   # untimed: the exact bits of the needed experts
+            for k_, v in wl.expert_weights(cfg, seed, e, device).items():
+                self.tabs[k_][e] = wl.bits(v)
+        self.n_experts = len(used)
+
+    def decisions(self):
+        orc, cfg = self.orc, self.cfg
+        s = orc.scores(self.xb, self.Wr, self.b, cfg.score_fn)
+        idx, gate = orc.route(s, self.cb, cfg.k, cfg.n_group, cfg.topk_group, cfg.norm_topk)
+        if self.prune is not None:
+            flags = orc.FLAG_IMP_BOUND if self.eps is not None else 0
+            pr = orc.prune(self.prune[0], self.prune[1], flags, idx, gate, cfg.E, self.w_eff, self.part, cfg.D,
+                           eps=0.0 if self.eps is None else self.eps)
+            if self.prune[0] != 0:
+                idx, gate = orc.compensate(s, self.cb, pr["keep"], idx, gate, cfg.norm_topk, 0)
+        c = orc.compact(idx, gate, cfg.E)
+        return idx, gate, c
+
+    def step(self):
+        """One full layer step; returns the seconds it took."""
+        cfg, t = self.cfg, self.tabs
+        fp8 = cfg.w_dtype == self.wl.DT_E4M3
         t0 = time.perf_counter()
-        orc.moe_tokens(xb, tokens, idx, gate, tabs["gate"], tabs["up"], tabs["down"], cfg.E, cfg.S, cfg.routed_scale,
-                       tabs["gate_scale"] if fp8 else None, tabs["up_scale"] if fp8 else None,
-                       tabs["down_scale"] if fp8 else None)
-        t_all += time.perf_counter() - t0
-        reps += 1
-    t_ffn = t_all / reps
-    total = t_dec + t_ffn * T / len(tokens)
-    return T / total, t_dec + t_all, cores, len(tokens)
+        idx, gate, _ = self.decisions()
+        self.orc.moe_tokens(self.xb, list(range(self.T)), idx, gate, t["gate"], t["up"], t["down"], cfg.E, cfg.S, cfg.routed_scale,
+                            t["gate_scale"] if fp8 else None, t["up_scale"] if fp8 else None, t["down_scale"] if fp8 else None)
+        return time.perf_counter() - t0
 
 
-def run_reference(args, cfg, prune):
+def oracle_sample_text(o, reps):
+    return (f"the whole layer step on all {o.T} tokens ({o.n_experts} experts' weights touched), oracle as it stands "
+            f"(g++ -O2, OpenMP over the FFN rows), {reps} timed repetition(s), nothing extrapolated")
+
+
+def run_reference(args, cfg, prune, eps):
     """--impl reference: the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
     rank, world, _ = dist_env()
     if rank != 0:
         return
+    import torch
     T = args.tokens
-    n_sample = 1
-    vals, secs = [], []
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"      # inputs only: the experts' bits are drawn where it is fast
+    o = OracleLayer(cfg, T, prune, eps, 0, dev)
+    secs = []
     for i in range(args.warmup + args.steps):
-        v, sec, cores, ns = oracle_sample_run(cfg, T, prune, 0, n_sample, "cpu")
+        sec = o.step()
         if i >= args.warmup:
-            vals.append(v)
             secs.append(sec)
-    value = statistics.mean(vals)
-    sample = (f"per step: oracle decisions on all {T} tokens + FFN/combine on {n_sample} token(s), extrapolated linearly "
-              f"to {T} tokens; inputs drawn on the CPU generator")
+    ms = 1e3 * statistics.mean(secs)
+    value = T / (ms * 1e-3)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * T / value, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg, T, args.prune)},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_name(cfg, T, args.prune, eps)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": o.cores, "kind": "oracle", "sample": oracle_sample_text(o, len(secs))},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -193,7 +212,7 @@ def job_throughput(ms_local, tokens_local, world, device):
 
 
 # --------------------------------------------------------------------------- the CUDA arm
-def run_caee(args, cfg, prune):
+def run_caee(args, cfg, prune, eps):
     import torch
     from paper_2606_29982_b200 import binding as B
     from paper_2606_29982_b200 import workloads as wl
@@ -209,7 +228,7 @@ def run_caee(args, cfg, prune):
         dist.init_process_group("nccl", device_id=torch.device(dev))
     T, K, W = args.tokens, args.steps, max(args.warmup, 3)
     L = Layer(cfg, seed=rank, max_tokens=max(T, 128), device=dev)
-    params = None if prune is None else B.prune_params(prune[0], prune[1])
+    params = None if prune is None else B.prune_params(prune[0], prune[1], 0, eps)
     xs = [wl.hidden(cfg, T, rank * 1000 + 100 + i, dev) for i in range(4)]      # rotate a few batches
     y = torch.empty_like(xs[0])
     stats = B.stats_buffer(dev)
@@ -247,7 +266,9 @@ def run_caee(args, cfg, prune):
     # --- device-resident timing, with the expert kernel timed by its own event pair
     B.caee_profile(L.ctx, K)
     clocks = ClockSampler(local)
+    n0 = B.caee_launch_count(L.ctx)
     ms_total = timed(step, K)
+    gpu_launches = B.caee_launch_count(L.ctx) - n0       # counted by the library at its launch sites
     clk = clocks.stop()
     expert_ms = B.caee_profile_read(L.ctx, K)
     B.caee_profile(L.ctx, 0)
@@ -287,44 +308,47 @@ def run_caee(args, cfg, prune):
     launch_bytes = [batch_bytes[i % len(xs)] for i in range(len(expert_ms))]     # launch i ran batch i % 4
     bytes_per_launch = float(statistics.mean(launch_bytes)) if launch_bytes else None
     achieved = bytes_per_launch / (k_ms * 1e-3) / 1e9 if k_ms else None
-    # dram bytes per launch from the committed ncu --set full capture of this same command
-    # (profiles/traffic.json, written from the .ncu-rep by hand; null when not captured)
-    traffic = None
+    # DRAM bytes per launch of the dominant kernel: from the committed ncu --set full capture of this same
+    # command (profiles/traffic.json, written by paper_2606_29982_b200.profile_summary from the .ncu-rep at the
+    # commit it names); null when this workload was not captured
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(f"{cfg.name}/T{T}/{args.prune}", {}).get("dram_bytes_per_launch")
+            ent = json.load(f).get(f"{cfg.name}/T{T}/{args.prune}" + (f"/eps{args.eps_frac:g}T" if eps is not None else ""), {})
+        traffic = ent.get("dram_bytes_per_launch")
+        if traffic is not None:
+            traffic_src = f"committed ncu capture at commit {ent.get('commit', '?')} (profiles/traffic.json), {ent.get('launches', '?')} launches averaged"
     fp8 = cfg.w_dtype == wl.DT_E4M3
-    if T <= 256:
-        # k_router_logits, k_decide (S1-S6 + stats in one cooperative kernel), [k_act_split], expert kernel, k_combine
-        launches_per_step = 2 + (1 if fp8 else 0) + 1 + 1
-    else:
-        # stand-alone decision kernels: logits, top-k, [prune, compensate], count/scan/fill, [split], expert, combine, stats
-        n_prune = 0 if prune is None else (1 if T <= 512 else 2)      # k_prune, or k_prune_accum + k_prune_from_acc
-        launches_per_step = 2 + n_prune + (1 if prune is not None and prune[0] != 0 else 0) + 3 + (1 if fp8 else 0) + 1 + 1 + 1
-    if cfg.n_resident >= 0:
-        launches_per_step += 1 + st.n_fetch          # k_stats + one expert launch per fetched expert (C5)
+    dense_value = world * T / (dense_ms * 1e-3)
+    removed = 1.0 - st.weight_bytes / st_dense.weight_bytes if st_dense.weight_bytes else 0.0
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.w_dtype], "data": "synthetic",
-        "config": {"workload": workload_name(cfg, T, args.prune), "l2": "inputs larger than L2: each step streams "
+        "config": {"workload": workload_name(cfg, T, args.prune, eps) +
+                               f"; last batch: {100 * removed:.0f}% of the dense step's expert bytes removed, "
+                               f"F_imp = {st.F_imp / 2.0 ** 40:.2f} of {T} (gate units)",
+                   "l2": "inputs larger than L2: each step streams "
                    f"{st.weight_bytes / 1e9:.2f} GB of expert weights (L2 is 126 MB)", "parallelism": "replicas only",
                    "seed": 0},
+        "dense": {"value": dense_value, "unit": UNIT, "ms_per_step": dense_ms,
+                  "note": "the same batches without pruning (dense top-k), timed in the same run"},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                 "call": "caee_moe_forward_host: x from pinned host memory, y back to it, every step; copies double-buffered on two side streams",
                 "ms_per_step": ms_e2e},
-        "gpu_launches": launches_per_step * K,
+        "gpu_launches": gpu_launches,
         "roofline": {"bound": "hbm", "kernel": "k_expert_fp8" if fp8 else "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak if achieved else None, "traffic": traffic, "peak_source": peak_src,
+                     "frac": achieved / peak if achieved else None, "traffic": traffic, "traffic_source": traffic_src,
+                     "peak_source": peak_src,
                      "bytes_per_launch": bytes_per_launch, "kernel_ms": k_ms,
                      "bytes_by_batch": batch_bytes,
                      "frac_of_8TBps_nominal": achieved / 8000.0 if achieved else None},
         "latency_us": {"pruned": ms_step * 1e3, "dense": dense_ms * 1e3, "expert_kernel": k_ms * 1e3 if k_ms else None},
         "pruning": {"n_act": st.n_act, "n_keep": st.n_keep, "n_run": st.n_run, "F_cost_dense": st.F_cost_dense,
-                    "F_cost": st.F_cost, "bytes_pruned": st.weight_bytes, "bytes_dense": st_dense.weight_bytes,
-                    "n_run_dense": st_dense.n_run},
+                    "F_cost": st.F_cost, "F_imp": st.F_imp / 2.0 ** 40, "eps": eps, "bytes_pruned": st.weight_bytes,
+                    "bytes_dense": st_dense.weight_bytes, "bytes_removed_frac": removed, "n_run_dense": st_dense.n_run},
     }
     if fp8 and T > 256:
         # prefill-size e4m3 step: k_expert_fp8_wide (fp16 MMAs) is bound by the tensor pipe / its
@@ -337,18 +361,15 @@ def run_caee(args, cfg, prune):
                                 "flops_per_launch": flops, "hbm_gbs": achieved})
         out["roofline"].pop("frac_of_8TBps_nominal", None)
     if world == 1 and not args.no_cpu_baseline:
-        try:
-            import psutil
-            ram_gb = psutil.virtual_memory().available / 2 ** 30
-        except Exception:
-            ram_gb = 16.0
-        n_sample = max(1, min(16, int((ram_gb * 0.4) / (cfg.expert_bytes * cfg.k / 2 ** 30 + 1e-9))))
+        # the oracle as it stands on this box's host cores: the whole T-token layer step, a few repetitions
+        o = OracleLayer(cfg, T, prune, eps, 0, dev, layer=L)
         L.close()
         torch.cuda.empty_cache()
-        v, sec, cores, ns = oracle_sample_run(cfg, T, prune, 0, n_sample, dev, min_seconds=10.0)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                               "sample": f"oracle decisions on all {T} tokens + FFN/combine on {ns} of them, repeated "
-                                         f"for {sec:.1f} s of CPU work and averaged, extrapolated linearly to {T} tokens"}
+        secs = [o.step()]
+        while sum(secs) < 10.0 and len(secs) < 16:
+            secs.append(o.step())
+        out["cpu_baseline"] = {"value": T / statistics.mean(secs), "unit": UNIT, "cores": o.cores, "kind": "oracle",
+                               "sample": oracle_sample_text(o, len(secs))}
     else:
         L.close()
     print(json.dumps(out))
@@ -432,6 +453,8 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--tokens", type=int, default=128)
     ap.add_argument("--prune", default="thresh:0.6", help="dense | none | thresh:θ | cir:θ_imp | rank:b | frac:p")
+    ap.add_argument("--eps-frac", type=float, default=0.10,
+                    help="importance bound F_imp <= eps-frac * T (PAPER.md:150-152; CAEE_IMP_BOUND); negative = no bound")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cache-loop", action="store_true", help="SURVEY §8(f) NEXT-1: multi-layer decode loop over an LFU expert cache")
     ap.add_argument("--layers", type=int, default=2)
@@ -440,12 +463,13 @@ def main():
     from paper_2606_29982_b200 import workloads as wl
     cfg = wl.CONFIGS[args.workload.upper()]
     prune = parse_prune(args.prune)
+    eps = args.eps_frac * args.tokens if (prune is not None and args.eps_frac >= 0) else None
     if args.cache_loop:
         run_cache_loop(args, cfg)
     elif args.impl == "reference":
-        run_reference(args, cfg, prune)
+        run_reference(args, cfg, prune, eps)
     else:
-        run_caee(args, cfg, prune)
+        run_caee(args, cfg, prune, eps)
 
 
 if __name__ == "__main__":

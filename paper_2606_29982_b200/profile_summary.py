@@ -1,0 +1,160 @@
+"""Turns `ncu -i X.ncu-rep --page raw --csv` (stdin) into a text summary and, optionally, an entry of
+profiles/traffic.json — so that no number under profiles/ is typed by hand.
+
+    ncu -i gpurun_out/X.ncu-rep --page raw --csv | \
+        python -m paper_2606_29982_b200.profile_summary --title "..." --command "..." \
+            [--kernel k_expert_umma --traffic-key "C3-r1-bf16/T128/thresh:0.6" --traffic profiles/traffic.json] \
+            > profiles/rNN_name.md
+
+Only formatting and averaging live here; the measurements are Nsight Compute's.
+"""
+import argparse
+import csv
+import json
+import re
+import statistics
+import subprocess
+import sys
+
+COLS = [
+    ("gpu__time_duration.sum", "us", 1.0),
+    ("dram__bytes_read.sum", "MB read", None),
+    ("dram__bytes_write.sum", "MB written", None),
+    ("dram__bytes_read.sum.per_second", "read GB/s", None),
+    ("dram__throughput.avg.pct_of_peak_sustained_elapsed", "dram % peak", 1.0),
+    ("lts__t_sector_hit_rate.pct", "L2 hit %", 1.0),
+    ("sm__pipe_tensor_cycles_active_realtime.avg.pct_of_peak_sustained_elapsed", "tensor pipe %", 1.0),
+    ("sm__warps_active.avg.pct_of_peak_sustained_active", "occupancy %", 1.0),
+    ("launch__registers_per_thread", "regs", 1.0),
+    ("launch__shared_mem_per_block_dynamic", "dyn smem KB", None),
+]
+STALLS = re.compile(r"smsp__average_warps_issue_stalled_(\w+)_per_issue_active\.ratio$")
+
+
+def to_bytes(v, unit):
+    v = float(v.replace(",", "")) if v else 0.0
+    u = unit.lower()
+    for p, m in (("kbyte", 1e3), ("mbyte", 1e6), ("gbyte", 1e9), ("tbyte", 1e12), ("byte", 1.0)):
+        if u.startswith(p):
+            return v * m
+    return v
+
+
+def to_us(v, unit):
+    v = float(v.replace(",", "")) if v else 0.0
+    return v * {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}.get(unit.strip().lower(), 1.0)
+
+
+def short(name):
+    name = re.sub(r"^void\s+", "", name)
+    name = re.sub(r"<unnamed>::", "", name)
+    return name.split("(")[0]
+
+
+def git_head():
+    try:
+        return subprocess.run(["git", "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+    except OSError:
+        return ""
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--title", default="ncu summary")
+    ap.add_argument("--command", default="", help="the command that produced the .ncu-rep (printed in the summary)")
+    ap.add_argument("--note", default="")
+    ap.add_argument("--kernel", default="", help="kernel (substring) whose DRAM bytes go to --traffic")
+    ap.add_argument("--traffic", default="")
+    ap.add_argument("--traffic-key", default="")
+    ap.add_argument("--alg-bytes", default="", help="comma-separated algorithmic bytes of the captured launches of --kernel, in order")
+    args = ap.parse_args()
+    rows = list(csv.reader(sys.stdin))
+    hdr, units, data = rows[0], rows[1], rows[2:]
+
+    def col(suffix):
+        for i, h in enumerate(hdr):
+            if h == suffix or h.endswith("." + suffix):
+                return i
+        return None
+
+    ki = hdr.index("Kernel Name")
+    print(f"# {args.title}\n")
+    if args.command:
+        print(f"Command:\n\n```\n{args.command}\n```\n")
+    print(f"Summary written by `python -m paper_2606_29982_b200.profile_summary` from `ncu --page raw --csv` at commit "
+          f"`{git_head()}`; one line per captured launch.  Durations under the profiler are serialised and replayed: "
+          "they are evidence for traffic and pipe utilisation, not bench values.\n")
+    if args.note:
+        print(args.note + "\n")
+    head = ["#", "kernel", "grid", "block"] + [c[1] for c in COLS]
+    print("| " + " | ".join(head) + " |")
+    print("|" + "---|" * len(head))
+    gi, bi = col("launch__grid_size"), col("launch__block_size")
+    picked = []
+    for n, r in enumerate(data):
+        out = [str(n), short(r[ki]), r[gi] if gi is not None else "", r[bi] if bi is not None else ""]
+        vals = {}
+        for name, label, _ in COLS:
+            i = col(name)
+            if i is None or r[i] == "":
+                out.append("")
+                continue
+            if label == "us":
+                v = to_us(r[i], units[i]); out.append(f"{v:.1f}")
+            elif label.startswith("MB"):
+                v = to_bytes(r[i], units[i]); out.append(f"{v / 1e6:.2f}")
+            elif label == "read GB/s":
+                v = to_bytes(r[i], units[i]); out.append(f"{v / 1e9:.0f}")
+            elif label == "dyn smem KB":
+                v = to_bytes(r[i], units[i]); out.append(f"{v / 1e3:.1f}")
+            else:
+                v = float(r[i].replace(",", "")); out.append(f"{v:.1f}")
+            vals[name] = v
+        print("| " + " | ".join(out) + " |")
+        if args.kernel and args.kernel in r[ki]:
+            picked.append(vals)
+    # warp stall reasons, top five per kernel name
+    print("\nWarp stall reasons (cycles stalled per issued instruction, top five):\n")
+    seen = set()
+    for r in data:
+        k = short(r[ki])
+        if k in seen:
+            continue
+        seen.add(k)
+        st = []
+        for i, h in enumerate(hdr):
+            m = STALLS.search(h)
+            if m and r[i]:
+                st.append((float(r[i].replace(",", "")), m.group(1)))
+        st.sort(reverse=True)
+        print(f"- `{k}`: " + ", ".join(f"{n} {v:.2f}" for v, n in st[:5]))
+    if picked:
+        rd = [p.get("dram__bytes_read.sum", 0.0) for p in picked]
+        wr = [p.get("dram__bytes_write.sum", 0.0) for p in picked]
+        us = [p.get("gpu__time_duration.sum", 0.0) for p in picked]
+        tot = [a + b for a, b in zip(rd, wr)]
+        print(f"\n`{args.kernel}`: {len(picked)} launches; DRAM read+write per launch = "
+              + ", ".join(f"{t / 1e9:.3f}" for t in tot) + f" GB (mean {statistics.mean(tot) / 1e9:.3f} GB); "
+              f"read rate = " + ", ".join(f"{a / u / 1e3:.0f}" for a, u in zip(rd, us)) + " GB/s under the profiler.")
+        alg = [float(v) for v in args.alg_bytes.split(",") if v]
+        if alg and len(alg) == len(tot):
+            print("Traffic / algorithmic bytes per launch = " + ", ".join(f"{t / a:.3f}" for t, a in zip(tot, alg))
+                  + f" (mean {statistics.mean(tot) / statistics.mean(alg):.3f}).")
+        if args.traffic and args.traffic_key:
+            try:
+                with open(args.traffic) as f:
+                    tj = json.load(f)
+            except (OSError, ValueError):
+                tj = {}
+            tj[args.traffic_key] = {"kernel": args.kernel, "dram_bytes_per_launch": statistics.mean(tot),
+                                    "dram_bytes_by_launch": tot, "launches": len(tot), "commit": git_head(),
+                                    "source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum"}
+            if alg and len(alg) == len(tot):
+                tj[args.traffic_key]["algorithmic_bytes_by_launch"] = alg
+            with open(args.traffic, "w") as f:
+                json.dump(tj, f, indent=1, sort_keys=True)
+                f.write("\n")
+
+
+if __name__ == "__main__":
+    main()
