@@ -168,6 +168,13 @@ __global__ void __launch_bounds__(256) k_scale_norm(const float* __restrict__ ta
 // ------------------------------------------------------------------ the kernel, part 1: roles 0-3
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constant__ Fp8Params p);
 
+#ifdef CAEE_TILE_TRACE
+// tuning aid (not in the product build): per tile {sm, ticket, claim, first copy issued, last copy issued, epilogue done} in ns
+__device__ long long g_tile_trace[4096][6];
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ int smid() { int s; asm volatile("mov.u32 %0, %%smid;" : "=r"(s)); return s; }
+#endif
+
 // Per-tile epilogue body for CT token columns per warp (defined below).
 template <int CT>
 __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile& t, uint32_t tmem_base, uint32_t tfull0,
@@ -233,6 +240,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
         mbar_arrive(qfull0 + 8 * q);
         if (++q == kQueue) { q = 0; qph ^= 1; }
         if (!tm.at(i, t)) break;
+#ifdef CAEE_TILE_TRACE
+        if (i < 4096) { g_tile_trace[i][0] = smid(); g_tile_trace[i][1] = i; g_tile_trace[i][2] = gtime(); }
+#endif
         const int e = p.wl.run_expert[t.run];
         const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
         const uint8_t* src = p.packed[e] + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes;
@@ -240,6 +250,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
           mbar_wait(empty0 + 8 * stage, ph ^ 1);
           mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
           bulk_g2s_stream(smem_base + stage * p.stage_bytes, src + (size_t)kb * kAStageBytes, kAStageBytes, full0 + 8 * stage, pol);
+#ifdef CAEE_TILE_TRACE
+          if (i < 4096 && kb == 0) g_tile_trace[i][3] = gtime();
+          if (i < 4096 && kb == nkb - 1) g_tile_trace[i][4] = gtime();
+#endif
           if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
         }
       }
@@ -346,7 +360,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     // ===== epilogue (warps 4-11): warp -> TMEM lane quadrant q = warp % 4, column half hf
     const int q = warp & 3, hf = (warp - 4) >> 2;
     int acc_it = 0, p1_it = 0;
+#ifdef CAEE_TILE_TRACE
+    int cur = -1;
+    for (;;) {
+      if (cur >= 0 && cur < 4096 && threadIdx.x == 128) g_tile_trace[cur][5] = gtime();
+      cur = tq.pop();
+      if (!tm.at(cur, t)) break;
+#else
     while (tm.at(tq.pop(), t)) {
+#endif
       const int half_cols = ((p.wl.run_n[t.run] + 15) & ~15) >> 1;   // 8, 16, ..., 64
       if (half_cols <= 8) fp8_epilogue_tile<8>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
       else if (half_cols <= 16) fp8_epilogue_tile<16>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
@@ -498,6 +520,12 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     }
   }
 }
+
+#ifdef CAEE_TILE_TRACE
+}  // namespace
+extern "C" void caee_debug_tile_trace(long long* out, int n) { cudaMemcpyFromSymbol(out, g_tile_trace, sizeof(long long) * 6 * n); }
+namespace {
+#endif
 
 size_t table_floats(const caee_ctx* c) {
   const int P1 = c->d.I / kTileRows, P2 = c->d.H / (2 * kTileRows), KS1 = c->d.H / kKBlock, KS2 = c->d.I / kKBlock;

@@ -6,6 +6,11 @@ profiles/traffic.json — so that no number under profiles/ is typed by hand.
             [--kernel k_expert_umma --traffic-key "C3-r1-bf16/T128/thresh:0.6" --traffic profiles/traffic.json] \
             > profiles/rNN_name.md
 
+    cuobjdump -sass paper_2606_29982_b200/libcaee.so | c++filt | \
+        python -m paper_2606_29982_b200.profile_summary --sass --title "..." > profiles/rNN_sass.md
+
+(--sass: per kernel, counts of the SASS mnemonics that prove tcgen05 / TMEM / TMA use, plus the first line of each.)
+
 Only formatting and averaging live here; the measurements are Nsight Compute's.
 """
 import argparse
@@ -58,8 +63,60 @@ def git_head():
         return ""
 
 
+# SASS mnemonics of the Blackwell tensor / TMEM / bulk-copy paths (B200_PROFILING.md) and what they are
+SASS_OPS = [("UTCHMMA", "tcgen05.mma kind::f16"), ("UTCQMMA", "tcgen05.mma kind::f8f6f4"), ("UTCBAR", "tcgen05.commit"),
+            ("LDTM", "tcgen05.ld (TMEM -> registers)"), ("UTCATOMSWS", "tcgen05.alloc / dealloc"),
+            ("UBLKCP", "cp.async.bulk (bulk copy global -> shared)"), ("UTMALDG", "cp.async.bulk.tensor (TMA, incl. tile::gather4)"),
+            ("SYNCS", "mbarrier ops"), ("HMMA", "mma.sync (legacy tensor path)"), ("ACQBULK", "griddepcontrol.wait"),
+            ("ELECT", "elect.sync")]
+
+
+def sass_summary(title, want):
+    """stdin: `cuobjdump -sass lib.so`.  One table row per kernel whose name contains one of `want`."""
+    fn, counts, first, order = None, {}, {}, []
+    for line in sys.stdin:
+        m = re.search(r"Function : (.+)$", line)
+        if m:
+            fn = short(m.group(1).strip().replace("(anonymous namespace)::", ""))
+            continue
+        if fn is None or not any(w in fn for w in want):
+            continue
+        m = re.match(r"\s+/\*[0-9a-f]+\*/\s+(.*?);", line)
+        if not m:
+            continue
+        ins = m.group(1)
+        if fn not in counts:
+            counts[fn], first[fn] = {}, {}
+            order.append(fn)
+        counts[fn]["_total"] = counts[fn].get("_total", 0) + 1
+        for op, _ in SASS_OPS:
+            if re.search(r"(^|\s)" + op + r"[.\s]", " " + ins):
+                counts[fn][op] = counts[fn].get(op, 0) + 1
+                first[fn].setdefault(op, ins)
+    print(f"# {title}\n")
+    print("Written by `cuobjdump -sass paper_2606_29982_b200/libcaee.so | c++filt | python -m paper_2606_29982_b200.profile_summary --sass` "
+          f"at commit `{git_head()}` (the library as `paper_2606_29982_b200/build.py` builds it: "
+          "`nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3`).\n")
+    print("| mnemonic | PTX it comes from |\n|---|---|")
+    for op, what in SASS_OPS:
+        print(f"| `{op}` | {what} |")
+    print("\n| kernel | SASS instructions | " + " | ".join(op for op, _ in SASS_OPS) + " |")
+    print("|---|---|" + "---|" * len(SASS_OPS))
+    for fn in order:
+        name = fn
+        print(f"| `{name}` | {counts[fn]['_total']} | " + " | ".join(str(counts[fn].get(op, 0)) for op, _ in SASS_OPS) + " |")
+    print("\nFirst occurrence of each mnemonic:\n")
+    for fn in order:
+        print(f"- `{fn}`")
+        for op, _ in SASS_OPS:
+            if op in first[fn]:
+                print(f"  - `{first[fn][op]}`")
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--sass", action="store_true", help="stdin is `cuobjdump -sass`: count tensor / TMEM / TMA mnemonics per kernel")
+    ap.add_argument("--kernels", default="k_expert,k_router_mma", help="--sass: comma-separated substrings of the kernels to list")
     ap.add_argument("--title", default="ncu summary")
     ap.add_argument("--command", default="", help="the command that produced the .ncu-rep (printed in the summary)")
     ap.add_argument("--note", default="")
@@ -68,6 +125,9 @@ def main():
     ap.add_argument("--traffic-key", default="")
     ap.add_argument("--alg-bytes", default="", help="comma-separated algorithmic bytes of the captured launches of --kernel, in order")
     args = ap.parse_args()
+    if args.sass:
+        sass_summary(args.title, [w for w in args.kernels.split(",") if w])
+        return
     rows = list(csv.reader(sys.stdin))
     hdr, units, data = rows[0], rows[1], rows[2:]
 
