@@ -2,7 +2,7 @@
  * decode hot path on one NVIDIA B200 (sm_100a).
  *
  * Citations are to /root/reference/PAPER.md ("PAPER.md:<line>") and to the readings
- * R1..R37 listed in DESIGN.md §3.  The paper's "devices" are logical expert
+ * R1..R40 listed in DESIGN.md §3.  The paper's "devices" are logical expert
  * partitions on one GPU whose costs are aggregated by max.
  *
  * Conventions
@@ -306,6 +306,40 @@ caee_status caee_cache_read_stats(const caee_cache* cache, caee_cache_stats* out
 /* Contents per slot (host arrays of n_slots): layer and expert (-1: free slot) and the key's
  * frequency. */
 caee_status caee_cache_snapshot(const caee_cache* cache, int32_t* layer, int32_t* expert, int64_t* freq);
+
+/* ---- Expert parallelism over the GPUs of one NVLink / NVSwitch domain.
+ * PAPER.md:57 (II-B): "token dispatch -> expert activation -> computation -> result aggregation ...
+ * across devices"; Latency_total = max_d Latency_d; F_cost as a max over
+ * devices.  One process and one context per GPU ("rank"); every rank owns a subset of the routed experts
+ * (owner[e], normally the cost model's partition table) and holds the shared experts (R39).  A step:
+ *   1. every rank has the SAME x [T,H] (the ranks' own tokens, all-gathered by the caller's transport:
+ *      home tokens of rank r are the contiguous block [r ceil(T/world), (r+1) ceil(T/world)) ∩ [0,T));
+ *   2. caee_moe_forward*(x, T, p, y = NULL allowed) on every rank: each rank takes the same batch-global
+ *      decision from the same scores (R40: deterministic kernels on identical inputs), runs only the runs
+ *      of the experts it owns — its slice, in (expert, token) order, of the expert-major work list (R38) —
+ *      plus the shared experts of its home tokens, and its expert kernel's epilogue stores every
+ *      (token, slot) output row straight into the o buffer of the token's home rank through peer memory
+ *      (the aggregation all-to-all is fused into the expert kernel; no combine yet);
+ *   3. the caller synchronises the group (every rank's step-2 work complete: a barrier of its transport);
+ *   4. caee_ep_combine(T, y) on every rank: y rows of the rank's home tokens (other rows untouched) — the
+ *      same list-order sum as on one device, so the result is bit-identical to the single-device layer.
+ * caee_set_ep: rank, world <= 8, owner host [E] in 0..world-1, obuf_peers host [world] = every rank's
+ * caee_ep_obuf pointer as seen from THIS device (its own at [rank]; peers' through caee_ep_ipc_open of
+ * the handle their caee_ep_ipc_export wrote, 64 bytes, or plain pointers when the contexts share a
+ * process).  world <= 1 or owner == NULL switches expert parallelism off.  Synchronises.  Not combinable
+ * with non-resident experts or the expert cache (CAEE_ESTATE at the step).  The paper's per-device cost
+ * model is unchanged: set the partitions to the owner table and F_cost is the max over the physical devices.
+ * caee_ep_plan: the explicit dispatch plan of the LAST decision on this context — the valid
+ * (token, slot) entries in ascending (device, expert, token) order: counts dev [world], offs dev [world+1],
+ * tok / slot / expert dev [T k] (first offs[world] entries valid). */
+caee_status caee_set_ep(caee_ctx* ctx, int32_t rank, int32_t world, const int32_t* owner, void* const* obuf_peers);
+caee_status caee_ep_obuf(caee_ctx* ctx, void** out, int64_t* bytes);
+caee_status caee_ep_ipc_export(caee_ctx* ctx, void* handle64);
+caee_status caee_ep_ipc_open(caee_ctx* ctx, const void* handle64, void** out);
+caee_status caee_ep_ipc_close(caee_ctx* ctx, void* peer_ptr);
+caee_status caee_ep_combine(caee_ctx* ctx, int32_t T, void* y, void* stream);
+caee_status caee_ep_plan(caee_ctx* ctx, int32_t* counts, int32_t* offs, int32_t* tok, int32_t* slot, int32_t* expert,
+                         void* stream);
 
 /* Library / build identification, e.g. "caee-b200 0.1 sm_100a". */
 const char* caee_version(void);

@@ -7,7 +7,7 @@
 #include <cstring>
 #include <new>
 
-#include "caee_internal.cuh"
+#include "umma_common.cuh"
 
 static thread_local std::string g_create_err;
 
@@ -137,7 +137,7 @@ void free_all(caee_ctx* c) {
                   c->gate, c->act, c->must, c->keep, c->I_fix, c->load, c->scalars, c->wl.counts, c->wl.estart, c->wl.offs,
                   c->wl.expert_ids, c->wl.ent_tok, c->wl.ent_slot, c->wl.ent_wt, c->wl.ent_dst, c->wl.run_expert,
                   c->wl.run_start, c->wl.run_n, c->wl.run_hrow, c->wl.meta, c->wl.sched, c->hbuf_f32, c->hbuf_b16, c->obuf,
-                  c->packed.dev_ptrs, c->xq, c->xs, c->hq, c->hs, c->xg, c->wl_hist};
+                  c->packed.dev_ptrs, c->xq, c->xs, c->hq, c->hs, c->xg, c->wl_hist, c->wr_img, c->ks_part, c->ks_cnt, c->ep_owned, c->ep_owner};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (size_t e = 0; e < c->packed.base.size(); ++e) {
@@ -169,13 +169,17 @@ void free_all(caee_ctx* c) {
 caee_status create_impl(caee_ctx* c) {
   const caee_layer_desc& d = c->d;
   const size_t Tm = d.max_tokens, E = d.E, k = d.k, S = d.S;
+  caee_status rc;
+  if (const char* v = getenv("CAEE_ROUTER_MMA_MIN_TOKENS")) c->router_mma_min_tokens = std::max(1, atoi(v));   // tuning aid
+  if (caee_router_mma_supported(c) && d.max_tokens >= c->router_mma_min_tokens) {
+    if ((rc = dev_alloc(c, &c->wr_img, caee_router_mma_image_bytes(c))) != CAEE_OK) return rc;
+  }
   size_t prow = 1;
   for (int T = 1; T <= d.max_tokens; ++T) {
     int tt, ks;
     caee_router_shape(c, T, &tt, &ks, nullptr);
     prow = std::max(prow, (size_t)ks * T);
   }
-  caee_status rc;
 #define A(ptr, n) if ((rc = dev_alloc(c, &(ptr), (n))) != CAEE_OK) return rc
   A(c->part, E); A(c->pl_experts, E); A(c->pl_start, CAEE_MAX_D + 1); A(c->resident, E); A(c->w_eff, E);
   A(c->wg, E + S); A(c->wu, E + S); A(c->wd, E + S); A(c->sg, E + S); A(c->su, E + S); A(c->sd, E + S);
@@ -187,7 +191,7 @@ caee_status create_impl(caee_ctx* c) {
   A(c->wl.counts, E); A(c->wl.estart, E); A(c->wl.offs, E + 1); A(c->wl.expert_ids, E);
   A(c->wl.ent_tok, Tm * (k + S)); A(c->wl.ent_slot, Tm * k); A(c->wl.ent_wt, Tm * k); A(c->wl.ent_dst, Tm * (k + S));
   A(c->wl.run_expert, c->wl.max_runs); A(c->wl.run_start, c->wl.max_runs); A(c->wl.run_n, c->wl.max_runs);
-  c->wl.n_tickets = (int)E + 2;
+  c->wl.n_tickets = 2 * ((int)E + 2);    // per expert-kernel launch of a step: tile tickets, then (second half) reducer tickets (KSplit)
   A(c->wl.run_hrow, c->wl.max_runs); A(c->wl.meta, 16); A(c->wl.sched, c->wl.n_tickets + c->wl.max_runs);
   c->wl.ready = c->wl.sched + c->wl.n_tickets;
   if (caee_wl_hist_ints(c)) { A(c->wl_hist, caee_wl_hist_ints(c)); }
@@ -204,6 +208,13 @@ caee_status create_impl(caee_ctx* c) {
     if (d.max_tokens >= c->fp8_wide_min_tokens) { A(c->xg, caee_fp8_wide_xg_bytes(c)); }
   }
   A(c->obuf, Tm * (k + S) * d.H);
+  if (c->kernel == CAEE_KERNEL_UMMA && !(getenv("CAEE_NO_KSPLIT") && atoi(getenv("CAEE_NO_KSPLIT")) != 0)) {
+    // steps of one or two tokens: split phase-1 tiles while a step has at most 2 of them per SM (umma_common.cuh:
+    // KSplit; measured on C3 / C4: +3.5 / +5.6% at T = 1, +2.7 / 0% at T = 2, -1 / -3.6% at T = 4)
+    c->ks_tile_cap = 2 * c->num_sms;
+    A(c->ks_part, caee_umma::caee_ksplit_part_floats(c->ks_tile_cap)); A(c->ks_cnt, c->ks_tile_cap);
+    CAEE_CUDA(c, cudaMemset(c->ks_cnt, 0, sizeof(int32_t) * c->ks_tile_cap));
+  }
 #undef A
   if (const char* v = getenv("CAEE_NO_PDL")) c->pdl = atoi(v) == 0;   // tuning aid
   CAEE_CUDA(c, cudaMemset(c->wl.meta, 0, sizeof(int32_t) * 16));
@@ -223,13 +234,22 @@ caee_status create_impl(caee_ctx* c) {
   return CAEE_OK;
 }
 
+// expert parallelism: home tokens of this device in a T-token step (contiguous blocks of ceil(T / world))
+void ep_step_view(caee_ctx* c, int T) {
+  if (!c->wl.ep_owned) return;
+  c->wl.ep_per = std::max(1, caee_ceil_div(T, c->ep_world));
+  c->wl.ep_tlo = std::min(T, c->ep_rank * c->wl.ep_per);
+  c->wl.ep_thi = std::min(T, c->wl.ep_tlo + c->wl.ep_per);
+}
+
 // route -> [prune + compensate] -> work list.  scores_in == NULL: compute scores from x.
 caee_status enqueue_decisions(caee_ctx* c, const void* x, const float* scores_in, int T, const caee_prune_params* p,
                               int32_t* idx, float* gate, float* scores_out, bool do_route, cudaStream_t st) {
   const float* scores = scores_in;
   if (T > 0 && do_route) {
     if (!scores_in) {
-      caee_launch_router_logits(c, x, T, st);
+      caee_status rr = caee_launch_router_logits(c, x, T, st);
+      if (rr != CAEE_OK) return rr;
       caee_launch_route_topk(c, nullptr, T, scores_out ? scores_out : c->scores, idx, gate, st);
       scores = scores_out ? scores_out : c->scores;
     } else {
@@ -318,6 +338,11 @@ caee_status caee_set_router(caee_ctx* c, const float* W_r, const float* b_logit,
   DeviceGuard g(c->device);
   CAEE_CUDA(c, cudaDeviceSynchronize());
   c->Wr = W_r; c->b_logit = b_logit; c->corr_bias = corr_bias; c->have_router = true;
+  if (c->wr_img) {
+    // the tensor-core router's copy of W_r (three bf16 terms, router_mma.cu): made once, here
+    caee_launch_pack_router(c, nullptr);
+    CAEE_CUDA(c, cudaDeviceSynchronize());
+  }
   return CAEE_OK;
 }
 
@@ -499,7 +524,7 @@ caee_status caee_route(caee_ctx* c, const void* x, int32_t T, float* scores, int
   if (!x || !idx || !gate) return caee_fail(c, CAEE_EINVAL, "x, idx or gate is NULL");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  caee_launch_router_logits(c, x, T, st);
+  if ((rc = caee_launch_router_logits(c, x, T, st)) != CAEE_OK) return rc;
   caee_launch_route_topk(c, nullptr, T, scores, idx, gate, st);
   return after_launch(c, "caee_route");
 }
@@ -526,6 +551,7 @@ caee_status caee_prune(caee_ctx* c, const caee_prune_params* p, const float* sco
   cudaStream_t st = (cudaStream_t)stream;
   caee_prune_params none = {CAEE_PRUNE_NONE, 0, 0.0, 0.0};
   c->wl.run_cap = CAEE_RUN_TOKENS;
+  ep_step_view(c, T);
   rc = enqueue_decisions(c, nullptr, scores, T, p ? p : &none, idx, gate, nullptr, false, st);
   if (rc != CAEE_OK) return rc;
   caee_launch_export_worklist(c, T, out, st);
@@ -550,8 +576,10 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (!scores && !c->have_router) return caee_fail(c, CAEE_ESTATE, "caee_moe_forward before caee_set_router");
   if (p && p->mode != CAEE_PRUNE_NONE && !c->have_cost) return caee_fail(c, CAEE_ESTATE, "pruning requested before caee_set_cost_table / caee_calibrate_cost");
   if (T == 0) return CAEE_OK;
-  if (!x || !y) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
+  const bool ep = c->wl.ep_owned != nullptr;
+  if (!x || (!y && !ep)) return caee_fail(c, CAEE_EINVAL, "x or y is NULL");
   if (((uintptr_t)x | (uintptr_t)y) & 15) return caee_fail(c, CAEE_EINVAL, "x and y must be 16-byte aligned");
+  if (ep && (c->any_offload || c->cache)) return caee_fail(c, CAEE_ESTATE, "expert parallelism does not combine with offloaded experts or the expert cache");
   DeviceGuard g(c->device);
   cudaStream_t st = (cudaStream_t)stream;
   // decode steps (T <= 128) use 64-token runs: the smaller token operand leaves room for a deeper
@@ -574,6 +602,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     CAEE_CUDA(c, cudaMemcpyAsync(c->resident, rs, E, cudaMemcpyHostToDevice, st));
     CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs, dp, sizeof(void*) * n, cudaMemcpyHostToDevice, st));
   }
+  ep_step_view(c, T);
   const bool fused = caee_decide_fits(c, T);
   // e4m3 decode steps: the split of x into its two e4m3 terms depends on x alone, so it goes first and
   // the chain router GEMM -> decision kernel -> expert kernel stays free for programmatic dependent launches
@@ -581,7 +610,7 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   if (early_prep) caee_launch_umma_prepare(c, x, T, st);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
-    if (!scores) caee_launch_router_logits(c, x, T, st);
+    if (!scores && (rc = caee_launch_router_logits(c, x, T, st)) != CAEE_OK) return rc;
     CAEE_CUDA(c, caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st));
     if ((rc = after_launch(c, "decision kernel")) != CAEE_OK) return rc;
   } else {
@@ -646,7 +675,9 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
     }
   }
   if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);
-  caee_launch_combine(c, T, c->idx, c->gate, y, st);
+  // expert parallelism: the o rows of this device's home tokens are still arriving from its peers; the caller
+  // synchronises the group and then calls caee_ep_combine
+  if (!c->wl.ep_owned) caee_launch_combine(c, T, c->idx, c->gate, y, st);
   if (!fused || c->any_offload) caee_launch_stats(c, stats, p != nullptr, n_fetch, st);
   return after_launch(c, "caee_moe_forward");
 }
@@ -707,6 +738,94 @@ caee_status caee_host_flush(caee_ctx* c, void* stream) {
   DeviceGuard g(c->device);
   for (int b = 0; b < 2; ++b) CAEE_CUDA(c, cudaStreamWaitEvent((cudaStream_t)stream, c->ev_hout[b], 0));
   return CAEE_OK;
+}
+
+// ---------------------------------------------------------------- expert parallelism (include/caee.h)
+caee_status caee_set_ep(caee_ctx* c, int32_t rank, int32_t world, const int32_t* owner, void* const* obuf_peers) {
+  if (!c) return CAEE_EINVAL;
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaDeviceSynchronize());
+  if (world <= 1 || !owner) {                 // back to one device
+    c->ep_rank = 0; c->ep_world = 1; c->wl.ep_owned = nullptr; c->wl.ep_world = 1;
+    return CAEE_OK;
+  }
+  if (world > CAEE_EP_MAX) return caee_fail(c, CAEE_EINVAL, "world=%d exceeds CAEE_EP_MAX=%d", world, CAEE_EP_MAX);
+  if (rank < 0 || rank >= world) return caee_fail(c, CAEE_EINVAL, "rank=%d out of range for world=%d", rank, world);
+  if (!obuf_peers) return caee_fail(c, CAEE_EINVAL, "obuf_peers is NULL");
+  const int E = c->d.E;
+  std::vector<uint8_t> owned(E);
+  for (int e = 0; e < E; ++e) {
+    if (owner[e] < 0 || owner[e] >= world) return caee_fail(c, CAEE_EINVAL, "owner[%d]=%d out of range", e, owner[e]);
+    owned[e] = owner[e] == rank;
+  }
+  for (int r = 0; r < world; ++r)
+    if (!obuf_peers[r]) return caee_fail(c, CAEE_EINVAL, "obuf_peers[%d] is NULL", r);
+  if (obuf_peers[rank] != (void*)c->obuf) return caee_fail(c, CAEE_EINVAL, "obuf_peers[rank] must be this context's own buffer (caee_ep_obuf)");
+  caee_status rc;
+  if (!c->ep_owned && (rc = dev_alloc(c, &c->ep_owned, (size_t)E)) != CAEE_OK) return rc;
+  if (!c->ep_owner && (rc = dev_alloc(c, &c->ep_owner, (size_t)E)) != CAEE_OK) return rc;
+  CAEE_CUDA(c, cudaMemcpy(c->ep_owned, owned.data(), E, cudaMemcpyHostToDevice));
+  CAEE_CUDA(c, cudaMemcpy(c->ep_owner, owner, sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  c->ep_owner_h.assign(owner, owner + E);
+  c->ep_rank = rank; c->ep_world = world;
+  c->wl.ep_owned = c->ep_owned; c->wl.ep_world = world;
+  for (int r = 0; r < CAEE_EP_MAX; ++r) c->wl.ep_obuf[r] = r < world ? (float*)obuf_peers[r] : nullptr;
+  return CAEE_OK;
+}
+
+caee_status caee_ep_obuf(caee_ctx* c, void** out, int64_t* bytes) {
+  if (!c) return CAEE_EINVAL;
+  if (!out) return caee_fail(c, CAEE_EINVAL, "out is NULL");
+  *out = c->obuf;
+  if (bytes) *bytes = (int64_t)sizeof(float) * c->d.max_tokens * (c->d.k + c->d.S) * c->d.H;
+  return CAEE_OK;
+}
+
+caee_status caee_ep_ipc_export(caee_ctx* c, void* handle64) {
+  if (!c) return CAEE_EINVAL;
+  if (!handle64) return caee_fail(c, CAEE_EINVAL, "handle64 is NULL");
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+  DeviceGuard g(c->device);
+  CAEE_CUDA(c, cudaIpcGetMemHandle(reinterpret_cast<cudaIpcMemHandle_t*>(handle64), c->obuf));
+  return CAEE_OK;
+}
+
+caee_status caee_ep_ipc_open(caee_ctx* c, const void* handle64, void** out) {
+  if (!c) return CAEE_EINVAL;
+  if (!handle64 || !out) return caee_fail(c, CAEE_EINVAL, "handle64 or out is NULL");
+  DeviceGuard g(c->device);
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle64, sizeof(h));
+  CAEE_CUDA(c, cudaIpcOpenMemHandle(out, h, cudaIpcMemLazyEnablePeerAccess));
+  return CAEE_OK;
+}
+
+caee_status caee_ep_ipc_close(caee_ctx* c, void* peer_ptr) {
+  if (!c) return CAEE_EINVAL;
+  DeviceGuard g(c->device);
+  if (peer_ptr) CAEE_CUDA(c, cudaIpcCloseMemHandle(peer_ptr));
+  return CAEE_OK;
+}
+
+caee_status caee_ep_combine(caee_ctx* c, int32_t T, void* y, void* stream) {
+  caee_status rc = check_call(c, T);
+  if (rc != CAEE_OK) return rc;
+  if (!c->wl.ep_owned) return caee_fail(c, CAEE_ESTATE, "caee_ep_combine before caee_set_ep");
+  if (T == 0) return CAEE_OK;
+  if (!y) return caee_fail(c, CAEE_EINVAL, "y is NULL");
+  DeviceGuard g(c->device);
+  const int per = caee_ceil_div(T, c->ep_world), lo = std::min(T, c->ep_rank * per), hi = std::min(T, lo + per);
+  caee_launch_combine(c, T, c->idx, c->gate, y, (cudaStream_t)stream, lo, hi);
+  return after_launch(c, "caee_ep_combine");
+}
+
+caee_status caee_ep_plan(caee_ctx* c, int32_t* counts, int32_t* offs, int32_t* tok, int32_t* slot, int32_t* expert, void* stream) {
+  if (!c) return CAEE_EINVAL;
+  if (!c->wl.ep_owned) return caee_fail(c, CAEE_ESTATE, "caee_ep_plan before caee_set_ep");
+  if (!counts || !offs || !tok || !slot || !expert) return caee_fail(c, CAEE_EINVAL, "an output pointer is NULL");
+  DeviceGuard g(c->device);
+  caee_launch_ep_plan(c, c->ep_owner, c->ep_world, counts, offs, tok, slot, expert, (cudaStream_t)stream);
+  return after_launch(c, "caee_ep_plan");
 }
 
 caee_status caee_profile(caee_ctx* c, int32_t n_slots) {

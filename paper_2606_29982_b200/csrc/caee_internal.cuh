@@ -19,6 +19,7 @@
 #define CAEE_RUN_TOKENS_MIN 64
 #define CAEE_RUN_TOKENS_WIDE 256 /* e4m3 prefill kernel (expert_fp8_wide.cu): one N = 256 UMMA tile */
 #define CAEE_FP8_WIDE_MIN_TOKENS 257 /* steps of at least this many tokens take the e4m3 prefill kernel */
+#define CAEE_EP_MAX 8 /* most devices of an expert-parallel group (one NVSwitch domain) */
 #define CAEE_DECIDE_MAX_TOKENS 256 /* largest step the one-kernel decision path takes (decide.cu) */
 
 // One unit of expert work: <= CAEE_RUN_TOKENS tokens of one expert.
@@ -44,7 +45,19 @@ struct caee_worklist {
   int32_t max_runs, n_tickets;
   int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, 64 (UMMA decode steps, T <= 128) or
                         // CAEE_RUN_TOKENS_WIDE (e4m3 prefill steps)
+  // Expert parallelism (caee_set_ep): this device runs only the experts it
+  // owns (runs are built for them alone; the lists still hold every entry) and the shared experts of its home
+  // tokens [ep_tlo, ep_thi); an o row goes to the o buffer of the token's home device, ep_obuf[t / ep_per]
+  const uint8_t* ep_owned;   // [E] 1: this device owns the expert; NULL: no expert parallelism
+  int32_t ep_world, ep_per;  // devices; home tokens per device this step = ceil(T / world)
+  int32_t ep_tlo, ep_thi;
+  float* ep_obuf[CAEE_EP_MAX];
 };
+
+// the o buffer a (token, slot) output row goes to
+__device__ __forceinline__ float* caee_o_base(const caee_worklist& wl, float* local, int tok) {
+  return wl.ep_owned ? wl.ep_obuf[tok / wl.ep_per] : local;
+}
 
 struct caee_packed {
   // per expert (E+S) device pointer to the packed tile image, or NULL if not packed / not resident
@@ -104,6 +117,9 @@ struct caee_ctx {
   std::vector<const float*> sg_h, su_h, sd_h;
   caee_packed packed;
 
+  uint8_t* wr_img = nullptr;        // three bf16 terms of W_r as MMA stage images (router_mma.cu); NULL: shape not supported
+  int router_mma_min_tokens = 257;  // steps of at least this many tokens take the tensor-core router (env CAEE_ROUTER_MMA_MIN_TOKENS)
+
   // scratch
   float* partial = nullptr;  // [ksplit, T, E] split-K partial logits of x W_r^T (sized for the worst T)
   uint8_t* decide_scratch = nullptr;  // k_decide's self-cleaning accumulators, membership matrix, barriers
@@ -132,8 +148,18 @@ struct caee_ctx {
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
   bool pdl = true;                   // programmatic dependent launches on the decode path (env CAEE_NO_PDL=1 switches them off)
   bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
+  float* ks_part = nullptr;          // UMMA decode kernels: partial sums of split phase-1 tiles (KSplit, umma_common.cuh)
+  int32_t* ks_cnt = nullptr;         //   and their per-tile counters (zero between steps)
+  int ks_tile_cap = 0;               //   steps with at most this many phase-1 tiles split them (0: never; env CAEE_NO_KSPLIT=1)
   float* obuf = nullptr;             // [Tmax*(k+S), H] fp32 expert outputs, token-major slots
   size_t h_rows_cap = 0;
+
+  // expert parallelism (caee_set_ep)
+  int ep_rank = 0, ep_world = 1;
+  uint8_t* ep_owned = nullptr;       // dev [E]
+  std::vector<int32_t> ep_owner_h;   // [E] owner device of every routed expert
+  float* ep_obuf_h[CAEE_EP_MAX] = {nullptr};
+  int32_t* ep_owner = nullptr;       // dev [E]
 
   long long n_launches = 0;          // kernels of this library enqueued by the per-step calls (caee_launch_count)
   // the timed points of the last caee_calibrate_cost (caee_calibrate_points): [tier] -> sizes in bytes, medians in ns
@@ -180,7 +206,14 @@ static inline int caee_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 // router.cu
 void caee_router_shape(const caee_ctx* c, int T, int* token_tile, int* ksplit, int* k_chunk);
-void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t s);
+caee_status caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t s);
+// router_mma.cu
+bool caee_router_mma_supported(const caee_ctx* c);
+size_t caee_router_mma_image_bytes(const caee_ctx* c);
+bool caee_router_uses_mma(const caee_ctx* c, int T);
+void caee_router_mma_shape(const caee_ctx* c, int T, int* ksplit, int* stages_per_split);
+void caee_launch_pack_router(caee_ctx* c, cudaStream_t s);
+caee_status caee_launch_router_mma(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate,
                             cudaStream_t s);
 // decide.cu
@@ -225,8 +258,11 @@ caee_status caee_cache_prepare_layer(caee_ctx* c, size_t slot_bytes);
 void caee_cache_detach(caee_ctx* c);
 caee_status caee_cache_step(caee_ctx* c, const int32_t* executed, int n_executed, std::vector<uint8_t*>* miss_slots);
 // combine.cu
-void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s);
+void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t s, int t_lo = 0, int t_hi = -1);
 void caee_launch_stats(caee_ctx* c, caee_fwd_stats* stats, int pruned, int n_fetch, cudaStream_t s);
 long long caee_expert_bytes(const caee_ctx* c);
+// ep.cu
+void caee_launch_ep_plan(caee_ctx* c, const int32_t* owner_dev, int world, int32_t* counts, int32_t* offs, int32_t* tok,
+                         int32_t* slot, int32_t* expert, cudaStream_t s);
 // calibrate.cu
 caee_status caee_calibrate_impl(caee_ctx* c, const caee_calib_opts* o, caee_cost_fit fit[2]);

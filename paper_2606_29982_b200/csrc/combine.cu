@@ -18,11 +18,11 @@ template <> __device__ __forceinline__ void st4<__nv_bfloat16>(__nv_bfloat16* p,
 template <typename YT>
 __global__ void __launch_bounds__(256) k_combine(const float* __restrict__ obuf, const int32_t* __restrict__ idx,
                                                  const float* __restrict__ gate, YT* __restrict__ y, int H, int k, int S,
-                                                 float routed_scale) {
+                                                 float routed_scale, int t_lo) {
   // K_final and the gates were complete before the expert kernel started: fetch them while it still runs
   __shared__ int s_idx[32];
   __shared__ float s_gate[32];
-  const int t = blockIdx.y, c = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  const int t = t_lo + blockIdx.y, c = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
   if (threadIdx.x < k) {
     const int e = idx[(size_t)t * k + threadIdx.x];
     s_idx[threadIdx.x] = e;
@@ -56,11 +56,13 @@ __global__ void k_stats(caee_fwd_stats* st, const int64_t* scalars, const int64_
 
 }  // namespace
 
-void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t st) {
+// tokens [t_lo, t_hi) of the step (t_hi < 0: all T): an expert-parallel device combines its home tokens only
+void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* gate, void* y, cudaStream_t st, int t_lo, int t_hi) {
   const caee_layer_desc& d = c->d;
-  if (T <= 0) return;
+  if (t_hi < 0) t_hi = T;
+  if (T <= 0 || t_hi <= t_lo) return;
   ++c->n_launches;
-  dim3 grid(caee_ceil_div(d.H, 1024), T);
+  dim3 grid(caee_ceil_div(d.H, 1024), t_hi - t_lo);
   if (c->pdl && !c->any_offload && d.act_dtype != CAEE_F32) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -71,13 +73,13 @@ void caee_launch_combine(caee_ctx* c, int T, const int32_t* idx, const float* ga
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, k_combine<__nv_bfloat16>, (const float*)c->obuf, idx, gate, (__nv_bfloat16*)y, (int)d.H, (int)d.k, (int)d.S,
-                       (float)d.routed_scale);
+                       (float)d.routed_scale, t_lo);
     return;
   }
   if (d.act_dtype == CAEE_F32)
-    k_combine<float><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (float*)y, d.H, d.k, d.S, d.routed_scale);
+    k_combine<float><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (float*)y, d.H, d.k, d.S, d.routed_scale, t_lo);
   else
-    k_combine<__nv_bfloat16><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (__nv_bfloat16*)y, d.H, d.k, d.S, d.routed_scale);
+    k_combine<__nv_bfloat16><<<grid, 256, 0, st>>>(c->obuf, idx, gate, (__nv_bfloat16*)y, d.H, d.k, d.S, d.routed_scale, t_lo);
 }
 
 long long caee_expert_bytes(const caee_ctx* c) {

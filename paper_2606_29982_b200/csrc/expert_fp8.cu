@@ -59,6 +59,7 @@ struct Fp8Params {
   // [hi rows | lo rows] x k byte arrays of x and of h; lo row = hi row + lo_row_*
   CUtensorMap tm_x, tm_h;
   int lo_row_x, lo_row_h;
+  KSplit ksp;               // split k range of phase-1 tiles in steps of a few tokens (umma_common.cuh)
 };
 
 // two floats -> two e4m3 codes (low byte = a), round to nearest even, saturating
@@ -179,7 +180,7 @@ __device__ __forceinline__ int smid() { int s; asm volatile("mov.u32 %0, %%smid;
 template <int CT>
 __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile& t, uint32_t tmem_base, uint32_t tfull0,
                                                   uint32_t tempty0, int& acc_it, int& p1_it, float (*amax_s)[kTileRows], int q,
-                                                  int hf, int lane);
+                                                  int hf, int lane, int KS);
 
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constant__ Fp8Params p) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -224,7 +225,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
   // overlaps the decision kernel's tail; the work list exists from here on
   griddep_wait();
   griddep_launch();
-  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
+  const int n_runs = p.run_count >= 0 ? p.run_count : p.wl.meta[1];
+  const int KS = (p.ksp.ks > 1 && n_runs * p.P1 <= p.ksp.tile_cap) ? p.ksp.ks : 1;
+  const TileMap tm{n_runs, p.run_begin, p.P1, p.P2, KS};
+  const int KB1s = p.KB1 / KS;             // 128-k stages of one phase-1 (sub-)tile
   TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
   Tile t;
 
@@ -233,19 +237,34 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     if (lane == 0) {
       int stage = 0, ph = 0, q = 0, qph = 0;
       const uint64_t pol = l2_evict_first_policy();
+      // where a tile's stages start in its expert's packed image, and how many there are
+      auto resolve = [&](const Tile& tt, const uint8_t*& src, int& nkb) {
+        const int e = p.wl.run_expert[tt.run];
+        nkb = tt.phase == 1 ? KB1s : p.KB2;
+        src = p.packed[e] + (tt.phase == 1 ? (size_t)tt.sub * p.KB1 + (size_t)tt.kq * KB1s : (size_t)p.P1 * p.KB1 + (size_t)tt.sub * p.KB2) * kAStageBytes;
+      };
+      // The next tile's ticket (an atomic round trip) and its image pointer (two dependent loads) are
+      // fetched while the current tile's copies are being issued: claimed and resolved at the tile
+      // boundary they left the copy engine idle for ~1.2 us per tile.  (Tickets still come in
+      // increasing order per CTA; every CTA ends on a ticket beyond the last tile.)
+      int nxt = atomicAdd(p.wl.sched + p.ticket, 1);
+      Tile tn;
+      const uint8_t* srcn = nullptr;
+      int nkbn = 0;
+      bool vn = tm.at(nxt, tn);
+      if (vn) resolve(tn, srcn, nkbn);
       for (;;) {
+        const int i = nxt, nkb = nkbn;
+        const uint8_t* src = srcn;
         mbar_wait(qempty0 + 8 * q, qph ^ 1);
-        const int i = atomicAdd(p.wl.sched + p.ticket, 1);
         tq_slots[q] = i;
         mbar_arrive(qfull0 + 8 * q);
         if (++q == kQueue) { q = 0; qph ^= 1; }
-        if (!tm.at(i, t)) break;
+        if (!vn) break;
 #ifdef CAEE_TILE_TRACE
         if (i < 4096) { g_tile_trace[i][0] = smid(); g_tile_trace[i][1] = i; g_tile_trace[i][2] = gtime(); }
 #endif
-        const int e = p.wl.run_expert[t.run];
-        const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-        const uint8_t* src = p.packed[e] + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes;
+        nxt = atomicAdd(p.wl.sched + p.ticket, 1);
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, ph ^ 1);
           mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
@@ -255,6 +274,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
           if (i < 4096 && kb == nkb - 1) g_tile_trace[i][4] = gtime();
 #endif
           if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+          if (kb == (nkb >> 1)) {
+            vn = tm.at(nxt, tn);
+            if (vn) resolve(tn, srcn, nkbn);
+          }
         }
       }
     }
@@ -263,7 +286,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     // The whole warp runs the loop (uniform control flow); one elected lane issues.
     int stage = 0, ph = 0, acc_it = 0;
     while (tm.at(tq.pop(), t)) {
-      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const int nkb = t.phase == 1 ? KB1s : p.KB2;
       const int npad = (__shfl_sync(0xffffffffu, p.wl.run_n[t.run], 0) + 15) & ~15;
       // up to 64 tokens the lo rows follow the hi rows and ONE MMA of N = 2 npad takes both terms
       // (hi and lo partial sums in separate columns, added by the epilogue): the weight tile is
@@ -317,7 +340,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     while (tm.at(tq.pop(), t)) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       const int npad = (n + 15) & ~15;
-      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const int nkb = t.phase == 1 ? KB1s : p.KB2, kb0 = t.kq * KB1s;     // kq = 0 in phase 2
       const uint32_t lo_smem = npad <= 64 ? (uint32_t)npad * kKBlock : (uint32_t)p.b_term_bytes;   // see the MMA warp
       const CUtensorMap* tmap = t.phase == 1 ? &p.tm_x : &p.tm_h;
       const int lo_row = t.phase == 1 ? p.lo_row_x : p.lo_row_h;
@@ -348,14 +371,61 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
         if (lane == 0) mbar_arrive_expect_tx(full0 + 8 * stage, 2u * npad * kKBlock);
         __syncwarp();
         if (mine) {
-          tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, kb * kKBlock, rh[0], rh[1], rh[2], rh[3]);
-          tma_gather4(b_addr + lo_smem + lane * 512, tmap, full0 + 8 * stage, kb * kKBlock, rl[0], rl[1], rl[2], rl[3]);
+          tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, (kb0 + kb) * kKBlock, rh[0], rh[1], rh[2], rh[3]);
+          tma_gather4(b_addr + lo_smem + lane * 512, tmap, full0 + 8 * stage, (kb0 + kb) * kKBlock, rl[0], rl[1], rl[2], rl[3]);
         }
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
       }
     }
   } else if (warp == 3) {
-    // spare warp
+    // ===== reducer (only in steps that split their phase-1 tiles, KSplit): finishes tiles whose ks
+    // partial sums are complete: h = silu(gate) * up, its (token, 128-feature block) scale and two e4m3
+    // terms — the arithmetic of the unsplit epilogue below; lane l holds features 4 l .. 4 l + 3
+    if (KS > 1) {
+      const int n_tiles = n_runs * p.P1;
+      for (;;) {
+        int j = 0;
+        if (lane == 0) j = atomicAdd(p.wl.sched + p.ksp.rticket, 1);
+        j = __shfl_sync(0xffffffffu, j, 0);
+        if (j >= n_tiles) break;
+        const int run = p.run_begin + j / p.P1, ft = j % p.P1;
+        const int n = p.wl.run_n[run], hrow = p.wl.run_hrow[run];
+        if (lane == 0) {
+          while (ld_acquire(p.ksp.cnt + j) < KS) __nanosleep(100);
+          p.ksp.cnt[j] = 0;                     // every sub-tile has arrived: ready for the next step
+        }
+        __syncwarp();
+        const float* part = p.ksp.part + (size_t)j * KS * (2 * kKSplitCols * kTileRows) + 4 * lane;
+        for (int c = 0; c < n; ++c) {
+          float4 g = make_float4(0.f, 0.f, 0.f, 0.f), u = g;
+          for (int kq = 0; kq < KS; ++kq) {
+            const float4 a = __ldcg(reinterpret_cast<const float4*>(part + (kq * 2 * kKSplitCols + c) * kTileRows));
+            const float4 b = __ldcg(reinterpret_cast<const float4*>(part + (kq * 2 * kKSplitCols + kKSplitCols + c) * kTileRows));
+            g.x += a.x; g.y += a.y; g.z += a.z; g.w += a.w;
+            u.x += b.x; u.y += b.y; u.z += b.z; u.w += b.w;
+          }
+          const float h0 = g.x / (1.0f + __expf(-g.x)) * u.x, h1 = g.y / (1.0f + __expf(-g.y)) * u.y;
+          const float h2 = g.z / (1.0f + __expf(-g.z)) * u.z, h3 = g.w / (1.0f + __expf(-g.w)) * u.w;
+          float m = fmaxf(fmaxf(fabsf(h0), fabsf(h1)), fmaxf(fabsf(h2), fabsf(h3)));
+#pragma unroll
+          for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+          const float sc = m > 0.f ? m * (1.0f / 448.0f) : 1.0f;
+          const float v0 = h0 / sc, v1 = h1 / sc, v2 = h2 / sc, v3 = h3 / sc;
+          const uint16_t hi01 = cvt_e4m3x2(v0, v1), hi23 = cvt_e4m3x2(v2, v3);
+          const float2 f01 = e4m3x2_to_float2(hi01), f23 = e4m3x2_to_float2(hi23);
+          const uint16_t lo01 = cvt_e4m3x2(v0 - f01.x, v1 - f01.y), lo23 = cvt_e4m3x2(v2 - f23.x, v3 - f23.y);
+          const size_t off = (size_t)(hrow + c) * p.I + ft * kTileRows + 4 * lane;
+          *reinterpret_cast<uint32_t*>(p.hq_hi + off) = (uint32_t)hi01 | ((uint32_t)hi23 << 16);
+          *reinterpret_cast<uint32_t*>(p.hq_lo + off) = (uint32_t)lo01 | ((uint32_t)lo23 << 16);
+          if (lane == 0) p.hs[(size_t)(hrow + c) * p.KB2 + ft] = sc;
+        }
+        // publish the tile's slice of h (read through the async proxy by other SMs' TMA gathers)
+        asm volatile("fence.proxy.async;" ::: "memory");
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) atomicAdd(p.wl.ready + run, 1);
+      }
+    }
   } else {
     // ===== epilogue (warps 4-11): warp -> TMEM lane quadrant q = warp % 4, column half hf
     const int q = warp & 3, hf = (warp - 4) >> 2;
@@ -370,10 +440,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
     while (tm.at(tq.pop(), t)) {
 #endif
       const int half_cols = ((p.wl.run_n[t.run] + 15) & ~15) >> 1;   // 8, 16, ..., 64
-      if (half_cols <= 8) fp8_epilogue_tile<8>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
-      else if (half_cols <= 16) fp8_epilogue_tile<16>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
-      else if (half_cols <= 32) fp8_epilogue_tile<32>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
-      else fp8_epilogue_tile<64>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane);
+      if (half_cols <= 8) fp8_epilogue_tile<8>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane, KS);
+      else if (half_cols <= 16) fp8_epilogue_tile<16>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane, KS);
+      else if (half_cols <= 32) fp8_epilogue_tile<32>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane, KS);
+      else fp8_epilogue_tile<64>(p, t, tmem_base, tfull0, tempty0, acc_it, p1_it, amax_s, q, hf, lane, KS);
     }
   }
 
@@ -392,14 +462,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
 template <int CT>
 __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile& t, uint32_t tmem_base, uint32_t tfull0,
                                                   uint32_t tempty0, int& acc_it, int& p1_it, float (*amax_s)[kTileRows], int q,
-                                                  int hf, int lane) {
+                                                  int hf, int lane, int KS) {
   constexpr int NJ = CT > 32 ? 2 : 1;
   const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run], hrow = p.wl.run_hrow[t.run];
-  const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+  const int nkb = t.phase == 1 ? p.KB1 / KS : p.KB2, kb0 = t.kq * nkb;      // kq = 0 unless a phase-1 tile's k range is split
   const int npad = (n + 15) & ~15;
   const int col0 = hf * CT, row = q * 32 + lane;
   const float* tab = reinterpret_cast<const float*>(p.packed[p.wl.run_expert[t.run]] + p.sc_off);
-  const float* wsc = t.phase == 1 ? tab + (size_t)t.sub * p.KB1 * 2 : tab + p.t2_off + (size_t)t.sub * p.KB2 * 2;
+  const float* wsc = t.phase == 1 ? tab + ((size_t)t.sub * p.KB1 + kb0) * 2 : tab + p.t2_off + (size_t)t.sub * p.KB2 * 2;
   // activation scales: lane l fetches those of column col0 + l (+ 32), broadcast by shuffle below
   const float* abase[NJ];
 #pragma unroll
@@ -407,7 +477,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     const int cl = lane + 32 * j, col = col0 + cl;
     abase[j] = nullptr;
     if (cl < CT && col < n)
-      abase[j] = t.phase == 1 ? p.xs + (size_t)p.wl.ent_tok[start + col] * p.KB1 : p.hs + (size_t)(hrow + col) * p.KB2;
+      abase[j] = t.phase == 1 ? p.xs + (size_t)p.wl.ent_tok[start + col] * p.KB1 + kb0 : p.hs + (size_t)(hrow + col) * p.KB2;
   }
   float acc0[CT], acc1[CT];
 #pragma unroll
@@ -461,6 +531,27 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     if (lane == 0) mbar_arrive(tempty0 + 8 * as);
   }
 
+  if (t.phase == 1 && KS > 1) {
+    // split k range (KSplit, umma_common.cuh): leave this sub-tile's partial sums and count it; a reducer
+    // warp finishes the tile (n <= kKSplitCols: CT == 8 and the hf == 0 warps hold every column)
+    const int tile = (t.run - p.run_begin) * p.P1 + t.sub;
+    float* mine = p.ksp.part + ((size_t)tile * KS + t.kq) * (2 * kKSplitCols * kTileRows);
+    if (hf == 0) {
+#pragma unroll
+      for (int c = 0; c < kKSplitCols; ++c) {
+        if (c < n) {
+          __stcg(mine + c * kTileRows + row, acc0[c]);
+          __stcg(mine + (kKSplitCols + c) * kTileRows + row, acc1[c]);
+        }
+      }
+    }
+    asm volatile("bar.sync 3, 256;" ::: "memory");
+    if (threadIdx.x == 128) {
+      __threadfence();                        // cumulative: the CTA's partial stores, ordered by the barrier
+      atomicAdd(p.ksp.cnt + tile, 1);
+    }
+    return;
+  }
   if (t.phase == 1) {
     // h = silu(gate) * up; per-token maximum over the tile's 128 features -> the (token, k block)
     // scale of phase 2's activation operand; then the two e4m3 terms
@@ -513,7 +604,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     for (int c = 0; c < CT; ++c) {
       const int col = col0 + c;
       if (col < n) {
-        float* o = ocol + (size_t)p.wl.ent_dst[start + col] * p.H;
+        float* o = caee_o_base(p.wl, p.obuf, p.wl.ent_tok[start + col]) + (ocol - p.obuf) + (size_t)p.wl.ent_dst[start + col] * p.H;
         o[0] = acc0[c];
         o[kTileRows] = acc1[c];
       }
@@ -611,6 +702,7 @@ void caee_launch_expert_fp8(caee_ctx* c, int T, int run_begin, int run_count, in
   const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers / amax buffers
   p.n_stages = std::min(kMaxStages, (max_dyn - 1024) / p.stage_bytes);
   const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
+  p.ksp = caee_ksplit_for(c, T, p.KB1, ticket);
   if (!(c->attr_done & 2u)) {
     cudaFuncSetAttribute(k_expert_fp8, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
     c->attr_done |= 2u;

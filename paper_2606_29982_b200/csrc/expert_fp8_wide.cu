@@ -80,6 +80,7 @@ struct WideParams {
   int sc_off;               // byte offset of the scale table in a packed image
   int t2_off;               // float offset of its phase-2 part
   int norm_off;             // byte offset of the expert's {2^J, 2^-J} pair (expert_fp8.cu: k_scale_norm)
+  int slots;                // k + S: an o row d belongs to token d / slots
 };
 
 // 16 e4m3 codes (one core-matrix row of the image) x scale -> 16 fp16, as two 8-element rows.
@@ -374,7 +375,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
           for (int j = 0; j < 16; ++j) {
             const int d = __shfl_sync(0xffffffffu, dsel, (rel & 31) + j);
             if (c + j < c_hi) {
-              float* o = ocol + (size_t)d * p.H;
+              float* o = caee_o_base(p.wl, p.obuf, d / p.slots) + (ocol - p.obuf) + (size_t)d * p.H;
               o[0] = __uint_as_float(v0[j]) * inv;
               o[kTileRows] = __uint_as_float(v1[j]) * inv;
             }
@@ -548,6 +549,7 @@ void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_coun
   p.sc_off = (int)((size_t)3 * d.H * d.I);
   p.t2_off = p.P1 * p.KB1 * 2;
   p.norm_off = (int)caee_fp8_norm_offset(c);
+  p.slots = d.k + d.S;
   if (!(c->attr_done & 4u)) {
     cudaFuncSetAttribute(k_expert_fp8_wide<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
     cudaFuncSetAttribute(k_expert_fp8_wide<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);

@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_simt_down(caee_worklist wl, cons
 #pragma unroll
     for (int q = 0; q < TCH; ++q) {
       float v = warp_sum(acc[q]);
-      if (lane == 0 && n0 + q < n) obuf[(size_t)wl.ent_dst[start + n0 + q] * H + ro] = v;
+      if (lane == 0 && n0 + q < n) caee_o_base(wl, obuf, wl.ent_tok[start + n0 + q])[(size_t)wl.ent_dst[start + n0 + q] * H + ro] = v;
     }
   }
 }

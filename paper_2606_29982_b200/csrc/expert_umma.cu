@@ -55,6 +55,7 @@ struct UmmaParams {
   int run_begin, run_count;   // runs [run_begin, run_begin + run_count) of the work list; run_count < 0: all
   int ticket;                 // which tile-ticket counter of wl.sched this launch uses
   CUtensorMap tm_x, tm_h;     // byte maps over x [T, 2H] and hbuf [rows, 2I] for the TMA row gathers
+  KSplit ksp;                 // split k range of phase-1 tiles in steps of a few tokens (umma_common.cuh)
 };
 
 // ------------------------------------------------------------------ the kernel
@@ -99,7 +100,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
   // overlaps the decision kernel's tail; the work list exists from here on
   griddep_wait();
   griddep_launch();
-  const TileMap tm{p.run_count >= 0 ? p.run_count : p.wl.meta[1], p.run_begin, p.P1, p.P2};
+  const int n_runs = p.run_count >= 0 ? p.run_count : p.wl.meta[1];
+  const int KS = (p.ksp.ks > 1 && n_runs * p.P1 <= p.ksp.tile_cap) ? p.ksp.ks : 1;
+  const TileMap tm{n_runs, p.run_begin, p.P1, p.P2, KS};
+  const int KB1s = p.KB1 / KS;             // 64-k stages of one phase-1 (sub-)tile
   TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
   Tile t;
 
@@ -108,21 +112,40 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
     if (lane == 0) {
       int stage = 0, ph = 0, q = 0, qph = 0;
       const uint64_t pol = l2_evict_first_policy();
+      // where a tile's stages start in its expert's packed image, and how many there are
+      auto resolve = [&](const Tile& tt, const uint8_t*& src, int& nkb) {
+        const int e = p.wl.run_expert[tt.run];
+        nkb = tt.phase == 1 ? KB1s : p.KB2;
+        src = p.packed[e] + (tt.phase == 1 ? (size_t)tt.sub * p.KB1 + (size_t)tt.kq * KB1s : (size_t)p.P1 * p.KB1 + (size_t)tt.sub * p.KB2) * kAStageBytes;
+      };
+      // The next tile's ticket (an atomic round trip) and its image pointer (two dependent loads) are
+      // fetched while the current tile's copies are being issued: claimed and resolved at the tile
+      // boundary they left the copy engine idle for ~1.2 us per tile.  (Tickets still come in
+      // increasing order per CTA; every CTA ends on a ticket beyond the last tile.)
+      int nxt = atomicAdd(p.wl.sched + p.ticket, 1);
+      Tile tn;
+      const uint8_t* srcn = nullptr;
+      int nkbn = 0;
+      bool vn = tm.at(nxt, tn);
+      if (vn) resolve(tn, srcn, nkbn);
       for (;;) {
+        const int i = nxt, nkb = nkbn;
+        const uint8_t* src = srcn;
         mbar_wait(qempty0 + 8 * q, qph ^ 1);
-        const int i = atomicAdd(p.wl.sched + p.ticket, 1);
         tq_slots[q] = i;
         mbar_arrive(qfull0 + 8 * q);
         if (++q == kQueue) { q = 0; qph ^= 1; }
-        if (!tm.at(i, t)) break;
-        const int e = p.wl.run_expert[t.run];
-        const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
-        const uint8_t* src = p.packed[e] + (t.phase == 1 ? (size_t)t.sub * p.KB1 : (size_t)p.P1 * p.KB1 + (size_t)t.sub * p.KB2) * kAStageBytes;
+        if (!vn) break;
+        nxt = atomicAdd(p.wl.sched + p.ticket, 1);
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, ph ^ 1);
           mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
           bulk_g2s_stream(smem_base + stage * p.stage_bytes, src + (size_t)kb * kAStageBytes, kAStageBytes, full0 + 8 * stage, pol);
           if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
+          if (kb == (nkb >> 1)) {
+            vn = tm.at(nxt, tn);
+            if (vn) resolve(tn, srcn, nkbn);
+          }
         }
       }
     }
@@ -134,7 +157,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
       const int as = it & 1;
       const int npad = (__shfl_sync(0xffffffffu, p.wl.run_n[t.run], 0) + 15) & ~15;
       const uint32_t idesc = make_idesc(npad, true);
-      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const int nkb = t.phase == 1 ? KB1s : p.KB2;
       mbar_wait(tempty0 + 8 * as, ((it >> 1) & 1) ^ 1);
       const uint32_t d0 = tmem_base + as * 256, d1 = d0 + 128;
       for (int kb = 0; kb < nkb; ++kb) {
@@ -170,7 +193,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
     while (tm.at(tq.pop(), t)) {
       const int n = p.wl.run_n[t.run], start = p.wl.run_start[t.run];
       const int npad = (n + 15) & ~15;
-      const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
+      const int nkb = t.phase == 1 ? KB1s : p.KB2, kb0 = t.kq * KB1s;     // kq = 0 in phase 2
       const CUtensorMap* tmap = t.phase == 1 ? &p.tm_x : &p.tm_h;
       int r[4];
 #pragma unroll
@@ -195,12 +218,49 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
         const uint32_t b_addr = smem_base + stage * p.stage_bytes + kAStageBytes;
         if (lane == 0) mbar_arrive_expect_tx(full0 + 8 * stage, (uint32_t)npad * 128u);
         __syncwarp();
-        if (mine) tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, kb * 128, r[0], r[1], r[2], r[3]);
+        if (mine) tma_gather4(b_addr + lane * 512, tmap, full0 + 8 * stage, (kb0 + kb) * 128, r[0], r[1], r[2], r[3]);
         if (++stage == p.n_stages) { stage = 0; ph ^= 1; }
       }
     }
   } else if (warp == 3) {
-    // spare warp
+    // ===== reducer (only in steps that split their phase-1 tiles, KSplit): finishes tiles whose ks
+    // partial sums are complete; lane l holds features 4 l .. 4 l + 3
+    if (KS > 1) {
+      const int n_tiles = n_runs * p.P1;
+      for (;;) {
+        int j = 0;
+        if (lane == 0) j = atomicAdd(p.wl.sched + p.ksp.rticket, 1);
+        j = __shfl_sync(0xffffffffu, j, 0);
+        if (j >= n_tiles) break;
+        const int run = p.run_begin + j / p.P1, ft = j % p.P1;
+        const int n = p.wl.run_n[run], hrow = p.wl.run_hrow[run];
+        if (lane == 0) {
+          while (ld_acquire(p.ksp.cnt + j) < KS) __nanosleep(100);
+          p.ksp.cnt[j] = 0;                     // every sub-tile has arrived: ready for the next step
+        }
+        __syncwarp();
+        const float* part = p.ksp.part + (size_t)j * KS * (2 * kKSplitCols * kTileRows) + 4 * lane;
+        for (int c = 0; c < n; ++c) {
+          float4 g = make_float4(0.f, 0.f, 0.f, 0.f), u = g;
+          for (int kq = 0; kq < KS; ++kq) {
+            const float4 a = __ldcg(reinterpret_cast<const float4*>(part + (kq * 2 * kKSplitCols + c) * kTileRows));
+            const float4 b = __ldcg(reinterpret_cast<const float4*>(part + (kq * 2 * kKSplitCols + kKSplitCols + c) * kTileRows));
+            g.x += a.x; g.y += a.y; g.z += a.z; g.w += a.w;
+            u.x += b.x; u.y += b.y; u.z += b.z; u.w += b.w;
+          }
+          const float h0 = g.x / (1.0f + __expf(-g.x)) * u.x, h1 = g.y / (1.0f + __expf(-g.y)) * u.y;
+          const float h2 = g.z / (1.0f + __expf(-g.z)) * u.z, h3 = g.w / (1.0f + __expf(-g.w)) * u.w;
+          const uint32_t w0 = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(h0)) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(h1)) << 16);
+          const uint32_t w1 = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(h2)) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(h3)) << 16);
+          *reinterpret_cast<uint2*>(p.hbuf + (size_t)(hrow + c) * p.I + ft * kTileRows + 4 * lane) = make_uint2(w0, w1);
+        }
+        // publish the tile's slice of h (read through the async proxy by other SMs' TMA gathers)
+        asm volatile("fence.proxy.async;" ::: "memory");
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) atomicAdd(p.wl.ready + run, 1);
+      }
+    }
   } else if (warp < 8) {
     // ===== epilogue: TMEM -> registers -> SwiGLU -> h (phase 1) or -> o rows (phase 2)
     const int q = warp - 4;  // TMEM lane quadrant of this warp (warp % 4)
@@ -211,6 +271,32 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
       tc_fence_after();
       const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + as * 256;
       const int row = q * 32 + lane;
+      if (t.phase == 1 && KS > 1) {
+        // split k range (KSplit, umma_common.cuh): leave this sub-tile's partial sums and count it; a
+        // reducer warp finishes the tile (n <= kKSplitCols)
+        uint32_t g[8], u[8];
+        tmem_ld8(tbase, g);
+        tmem_ld8(tbase + 128, u);
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty0 + 8 * as);
+        const int tile = (t.run - p.run_begin) * p.P1 + t.sub;
+        float* mine = p.ksp.part + ((size_t)tile * KS + t.kq) * (2 * kKSplitCols * kTileRows);
+#pragma unroll
+        for (int c = 0; c < kKSplitCols; ++c) {
+          if (c < n) {
+            __stcg(mine + c * kTileRows + row, __uint_as_float(g[c]));
+            __stcg(mine + (kKSplitCols + c) * kTileRows + row, __uint_as_float(u[c]));
+          }
+        }
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        if (threadIdx.x == 128) {
+          __threadfence();                      // cumulative: the CTA's partial stores, ordered by the barrier
+          atomicAdd(p.ksp.cnt + tile, 1);
+        }
+        continue;
+      }
       if (t.phase == 1) {
         uint16_t* hcol = p.hbuf + (size_t)p.wl.run_hrow[t.run] * p.I + t.sub * kTileRows + row;
         for (int c = 0; c < n; c += 16) {
@@ -237,7 +323,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             if (c + j < n) {
-              float* o = ocol + (size_t)p.wl.ent_dst[start + c + j] * p.H;
+              float* o = caee_o_base(p.wl, p.obuf, p.wl.ent_tok[start + c + j]) + (ocol - p.obuf) + (size_t)p.wl.ent_dst[start + c + j] * p.H;
               o[0] = __uint_as_float(d0[j]);
               o[kTileRows] = __uint_as_float(d1[j]);
             }
@@ -367,6 +453,7 @@ caee_status caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_b
   const int max_dyn = 227 * 1024 - 4096;            // leave room for the static barriers
   p.n_stages = std::min(kMaxStages, (max_dyn - 1024) / p.stage_bytes);
   const size_t dyn = (size_t)p.n_stages * p.stage_bytes + 1024;
+  p.ksp = caee_ksplit_for(c, T, p.KB1, ticket);
   if (!(c->attr_done & 1u)) {
     cudaFuncSetAttribute(k_expert_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn);
     c->attr_done |= 1u;

@@ -258,6 +258,13 @@ void launch_logits(caee_ctx* c, const XT* x, int T, cudaStream_t st) {
 // stage depth.  Steps of at most 4 tokens take the GEMV-shaped kernel (token tile 1, 2 or 4).
 void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit, int* hs) {
   const caee_layer_desc& d = c->d;
+  if (caee_router_uses_mma(c, T)) {   // prefill-size steps: tensor-core router (router_mma.cu), 128-token tiles
+    int sps;
+    caee_router_mma_shape(c, T, ksplit, &sps);
+    *tt = 128;
+    if (hs) *hs = sps * 64;
+    return;
+  }
   const bool small = T <= 4;
   *tt = small ? (T <= 1 ? 1 : (T <= 2 ? 2 : 4)) : (T <= 16 ? 16 : (T >= 1024 ? 64 : 32));   // prefill-size steps: 4 x 4 outputs per thread
   const int tiles = small ? caee_ceil_div(d.E, SE) : caee_ceil_div(d.E, TE) * caee_ceil_div(T, *tt);
@@ -270,9 +277,11 @@ void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit, int* hs) 
   if (hs) *hs = Hs;
 }
 
-void caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t st) {
+caee_status caee_launch_router_logits(caee_ctx* c, const void* x, int T, cudaStream_t st) {
+  if (caee_router_uses_mma(c, T)) return caee_launch_router_mma(c, x, T, st);
   if (c->d.act_dtype == CAEE_F32) launch_logits<float>(c, (const float*)x, T, st);
   else launch_logits<__nv_bfloat16>(c, (const __nv_bfloat16*)x, T, st);
+  return CAEE_OK;
 }
 
 void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* scores_out, int32_t* idx, float* gate,

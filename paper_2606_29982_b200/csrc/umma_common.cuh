@@ -207,12 +207,43 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
 }
 struct Tile {
   int phase, run, sub;  // sub = ft (phase 1) or op (phase 2)
+  int kq;               // phase 1 with a split k range (see KSplit): which quarter of k this sub-tile contracts
 };
+// Steps of a few tokens have fewer phase-1 tiles than it takes to balance 148 SMs whose shares of the
+// HBM bandwidth differ by +-25% (a C4 step of one token: 144 tiles of 1.8 MB, one per SM, the slowest
+// SM 48 us against the fastest's 27).  Such steps split every phase-1 tile's k range into `ks` sub-tiles
+// (tickets (run, ft, kq), kq fastest).  A sub-tile's epilogue only leaves its partial gate / up sums in
+// `part` and counts itself in `cnt`; the tile is FINISHED by a reducer warp (the CTAs' otherwise idle
+// warp 3; tiles handed out by a second ticket counter): it waits for the tile's ks partials, adds them
+// in ascending kq — a fixed order —, applies SwiGLU, writes h and counts the tile in the run's "h
+// complete" counter.  Sub-tiles never wait and all of them hold lower tickets than any phase-2 tile,
+// so a reducer's wait and the phase-2 wait on a run's h always end.
+struct KSplit {
+  float* part;     // [tile_cap][ks][2][kKSplitCols][128] partial sums, tile = (run - run_begin) * P1 + ft
+  int32_t* cnt;    // [tile_cap] finished sub-tiles of a tile; reset by the tile's reducer
+  int ks;          // 1: never split
+  int tile_cap;    // split only while n_runs * P1 <= tile_cap
+  int rticket;     // index in wl.sched of the reducers' ticket counter of this launch
+};
+constexpr int kKSplit = 4;           // sub-tiles per phase-1 tile when a step is split
+constexpr int kKSplitCols = 8;       // most tokens of a run in a split step (host: T <= kKSplitCols)
+// Host: the split a T-token step may use (kb1 = k stages of a whole phase-1 tile)
+inline KSplit caee_ksplit_for(const caee_ctx* c, int T, int kb1, int ticket) {
+  const bool on = c->ks_part && c->ks_tile_cap > 0 && T <= kKSplitCols && kb1 % kKSplit == 0;
+  return KSplit{c->ks_part, c->ks_cnt, on ? kKSplit : 1, c->ks_tile_cap, c->wl.n_tickets / 2 + ticket};
+}
+inline size_t caee_ksplit_part_floats(int tile_cap) { return (size_t)tile_cap * kKSplit * 2 * kKSplitCols * kTileRows; }
 struct TileMap {
   int n_runs, run_begin, P1, P2;
+  int KS = 1;
   __device__ __forceinline__ bool at(int i, Tile& t) const {
-    const int t1 = n_runs * P1;
-    if (i < t1) { const int r = i / P1; t.phase = 1; t.sub = i - r * P1; t.run = run_begin + r; return true; }
+    const int t1 = n_runs * P1 * KS;
+    t.kq = 0;
+    if (i < t1) {
+      const int per = P1 * KS, r = i / per, rem = i - r * per;
+      t.phase = 1; t.sub = rem / KS; t.kq = rem - t.sub * KS; t.run = run_begin + r;
+      return true;
+    }
     i -= t1;
     if (i < n_runs * P2) { const int r = i / P2; t.phase = 2; t.sub = i - r * P2; t.run = run_begin + r; return true; }
     return false;
@@ -268,6 +299,33 @@ inline bool encode_row_gather_map(void* tm_out, const void* base, size_t row_byt
   return enc(reinterpret_cast<CUtensorMap*>(tm_out), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), gd, gs, box, es,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+
+// Host: 2D tensor map over a row-major [rows, cols] bf16 array for plain tiled loads of box_rows x 64
+// elements (128 bytes per row) with the 128-byte swizzle — the SWIZZLE_128B K-major operand layout
+// (8-row atoms of 1024 B).  Rows or columns beyond the array come back as zeros.
+inline bool encode_tile_map_bf16(void* tm_out, const void* base, size_t rows, size_t cols, unsigned box_rows) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn enc = nullptr;
+  if (!enc) {
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &q) != cudaSuccess) enc = nullptr;
+    if (!enc) return false;
+  }
+  const cuuint64_t gd[2] = {(cuuint64_t)cols, (cuuint64_t)rows}, gs[1] = {(cuuint64_t)cols * 2};
+  const cuuint32_t box[2] = {64, box_rows}, es[2] = {1, 1};
+  return enc(reinterpret_cast<CUtensorMap*>(tm_out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gd, gs, box, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// box (c0 = first column, c1 = first row) of a tiled tensor map -> shared memory
+__device__ __forceinline__ void tma_tile_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1)
+               : "memory");
 }
 
 }  // namespace caee_umma

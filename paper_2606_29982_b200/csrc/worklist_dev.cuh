@@ -87,16 +87,19 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
   const int e = threadIdx.x, cap = wl.run_cap;   // tokens per run (a multiple of 16)
   const int c = e < E ? count_e : 0;
   const bool res = e < E && resident[e] != 0;
-  const int nch = (c + cap - 1) / cap, rows = (c + 15) & ~15;
+  // expert parallelism: the lists hold every entry, runs exist only for the experts this device owns
+  const int cr = (e < E && wl.ep_owned && !wl.ep_owned[e]) ? 0 : c;
+  const int t_lo = wl.ep_owned ? min(wl.ep_tlo, T) : 0, Th = (wl.ep_owned ? min(wl.ep_thi, T) : T) - t_lo;   // home tokens
+  const int nch = (cr + cap - 1) / cap, rows = (cr + 15) & ~15;
   const int v[6] = {c > 0, c, res ? nch : 0, res ? rows : 0, res ? 0 : nch, res ? 0 : rows};
   int ex[6], tot[6];
   caee_block_excl_scan<6>(v, ex, tot, scratch);
   if (e < E) estart[e] = ex[1];
   if (!write) return;
-  const int sh_chunks = T > 0 ? (T + cap - 1) / cap : 0;
+  const int sh_chunks = Th > 0 ? (Th + cap - 1) / cap : 0;
   const int sh_runs = S * sh_chunks;
   int sh_rows_each = 0;   // h rows of one shared expert: every chunk padded to 16
-  for (int t0 = 0; t0 < T; t0 += cap) sh_rows_each += (min(cap, T - t0) + 15) & ~15;
+  for (int t0 = 0; t0 < Th; t0 += cap) sh_rows_each += (min(cap, Th - t0) + 15) & ~15;
   if (c > 0) {
     wl.expert_ids[ex[0]] = e;
     wl.offs[ex[0]] = ex[1];
@@ -105,16 +108,16 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
     for (int j = 0; j < nch; ++j) {
       wl.run_expert[r0 + j] = e;
       wl.run_start[r0 + j] = ex[1] + j * cap;
-      wl.run_n[r0 + j] = min(cap, c - j * cap);
+      wl.run_n[r0 + j] = min(cap, cr - j * cap);
       wl.run_hrow[r0 + j] = h0 + j * cap;
     }
   }
-  for (int i = e; i < sh_runs; i += blockDim.x) {   // shared-expert runs over all tokens
+  for (int i = e; i < sh_runs; i += blockDim.x) {   // shared-expert runs over all (home) tokens
     const int s = i / sh_chunks, j = i - s * sh_chunks, t0 = j * cap;
     const int r = tot[2] + i;
     wl.run_expert[r] = E + s;
-    wl.run_start[r] = T * k + s * T + t0;
-    wl.run_n[r] = min(cap, T - t0);
+    wl.run_start[r] = T * k + s * T + t_lo + t0;
+    wl.run_n[r] = min(cap, Th - t0);
     wl.run_hrow[r] = tot[3] + s * sh_rows_each + j * cap;
   }
   if (e == 0) {

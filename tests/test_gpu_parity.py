@@ -63,6 +63,34 @@ def test_route_scores_and_selection(H, cfg):
         L.close()
 
 
+@pytest.mark.parametrize("cfg,min_tokens", [(C2S, None), (R1S, None), (wl.C2, None), (R1S, 1),
+                                            (wl.scaled(wl.C3, name="R1-router-full", I=128), None)], ids=lambda c: getattr(c, "name", str(c)))
+def test_route_scores_tensor_core_router(H, cfg, min_tokens, monkeypatch):
+    """S0 on the tensor cores (router_mma.cu; steps of >= 257 tokens, or every step when the tuning variable
+    lowers the bound): W_r as three bf16 terms keeps the scores within the same 1e-5 relative bound as the
+    fp32 FMA path, ragged last token tile and ragged k split included; selection on the GPU's own scores
+    differs from the oracle's on at most 1% of the picks (near-ties)."""
+    from paper_2606_29982_b200 import binding as B
+    if min_tokens is not None:
+        monkeypatch.setenv("CAEE_ROUTER_MMA_MIN_TOKENS", str(min_tokens))
+    L = _layer(H, cfg, max_tokens=1000)
+    try:
+        for T in ((1, 7, 130) if min_tokens else (257, 300, 1000)):
+            x = wl.hidden(cfg, T, 5, L.device)
+            s_gpu = torch.empty(T, cfg.E, dtype=torch.float32, device=L.device)
+            idx = torch.empty(T, cfg.k, dtype=torch.int32, device=L.device)
+            gate = torch.empty(T, cfg.k, dtype=torch.float32, device=L.device)
+            B.caee_route(L.ctx, x, T, s_gpu, idx, gate)
+            torch.cuda.synchronize()
+            s_ref = L.oracle_scores(x)
+            np.testing.assert_allclose(s_gpu.cpu().numpy(), s_ref, rtol=1e-5, atol=1e-10)
+            d = L.oracle_decisions(s_ref)
+            flips = int((np.sort(idx.cpu().numpy(), axis=1) != np.sort(d["idx0"], axis=1)).sum())
+            assert flips <= 0.01 * T * cfg.k + 1, f"T={T}: {flips} picks differ"
+    finally:
+        L.close()
+
+
 R1B = wl.scaled(R1S, name="R1-small-bias", corr_bias_std=0.3)    # the route's list order != gate order on most tokens (R36)
 # one partition of 64 experts: partitions of more than 32 experts take the block-wide decision code, the others one warp per partition
 C2W = wl.scaled(wl.C2, name="C2-one-partition", H=256, I=128, S=0, D=1)
