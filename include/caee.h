@@ -273,6 +273,13 @@ caee_status caee_last_routing(caee_ctx* ctx, int32_t T, int32_t* idx, float* gat
  * expert_ms (host, [n_slots]) and their number to n_out (host), then rewinds to slot 0. */
 caee_status caee_profile(caee_ctx* ctx, int32_t n_slots);
 caee_status caee_profile_read(caee_ctx* ctx, float* expert_ms, int32_t* n_out);
+/* Offloading steps recorded by caee_profile (static residency; call BEFORE caee_profile_read, which rewinds):
+ * per recorded step, copy_ms = duration of the step's H2D copy train on the side stream (first copy
+ * starts .. last copy ends), resident_ms = duration of the resident experts' launch on the caller's stream,
+ * lead_ms = from the start of the copy train to the end of the resident launch: resident compute is hidden
+ * behind the copies when lead_ms <= copy_ms (north_star (4)).  Host arrays of `cap`. */
+caee_status caee_profile_read_offload(caee_ctx* ctx, int32_t cap, float* copy_ms, float* resident_ms, float* lead_ms,
+                                      int32_t* n_out);
 
 /* ---- LFU expert cache (Fig. 8: "each HBM caches only a subset of 1024 experts,
  * managed by a Least Frequently Used (LFU) eviction policy").  Turns the

@@ -28,8 +28,10 @@ EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", 
            "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_calibrate_points",
            "caee_get_cost_table", "caee_launch_count", "caee_route",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
-           "caee_moe_forward_host", "caee_host_flush", "caee_last_routing", "caee_profile", "caee_profile_read", "caee_version",
-           "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot"]
+           "caee_moe_forward_host", "caee_host_flush", "caee_last_routing", "caee_profile", "caee_profile_read", "caee_profile_read_offload", "caee_version",
+           "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot",
+           "caee_set_ep", "caee_ep_obuf", "caee_ep_ipc_export", "caee_ep_ipc_open", "caee_ep_ipc_close", "caee_ep_combine",
+           "caee_ep_plan"]
 
 
 class caee_layer_desc(C.Structure):
@@ -107,6 +109,14 @@ _lib.caee_host_flush.argtypes = [_ctx_p, C.c_void_p]
 _lib.caee_last_routing.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_profile.argtypes = [_ctx_p, C.c_int32]
 _lib.caee_profile_read.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
+_lib.caee_profile_read_offload.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.caee_set_ep.argtypes = [_ctx_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+_lib.caee_ep_obuf.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
+_lib.caee_ep_ipc_export.argtypes = [_ctx_p, C.c_void_p]
+_lib.caee_ep_ipc_open.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
+_lib.caee_ep_ipc_close.argtypes = [_ctx_p, C.c_void_p]
+_lib.caee_ep_combine.argtypes = [_ctx_p, C.c_int32, C.c_void_p, C.c_void_p]
+_lib.caee_ep_plan.argtypes = [_ctx_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 for _n in EXPORTS:
     if _n not in ("caee_last_error", "caee_version", "caee_cache_destroy"):
         getattr(_lib, _n).restype = C.c_int32
@@ -268,6 +278,15 @@ def caee_profile_read(ctx, n_slots):
     return ms[:n.value].copy()
 
 
+def caee_profile_read_offload(ctx, n_slots):
+    """(copy_ms, resident_ms, lead_ms) per recorded offloading step; call before caee_profile_read."""
+    cap = max(int(n_slots), 1)
+    a, b, c_ = (np.zeros(cap, np.float32) for _ in range(3))
+    n = C.c_int32(0)
+    _check(_lib.caee_profile_read_offload(ctx, cap, _ptr(a), _ptr(b), _ptr(c_), C.addressof(n)), ctx)
+    return a[:n.value].copy(), b[:n.value].copy(), c_[:n.value].copy()
+
+
 def caee_cache_create(n_slots):
     cache = C.c_void_p()
     _check(_lib.caee_cache_create(int(n_slots), C.byref(cache)))
@@ -294,6 +313,47 @@ def caee_cache_snapshot(cache, n_slots):
     freq = np.zeros(n_slots, np.int64)
     _check(_lib.caee_cache_snapshot(cache, _ptr(layer), _ptr(expert), _ptr(freq)))
     return [None if layer[s] < 0 else (int(layer[s]), int(expert[s]), int(freq[s])) for s in range(n_slots)]
+
+
+def caee_set_ep(ctx, rank, world, owner=None, obuf_peers=None):
+    """owner: int32 [E] (None: expert parallelism off); obuf_peers: one device address per rank."""
+    o = None if owner is None else np.ascontiguousarray(owner, dtype=np.int32)
+    peers = None
+    if obuf_peers is not None:
+        peers = (C.c_void_p * len(obuf_peers))(*[int(p) for p in obuf_peers])
+    _check(_lib.caee_set_ep(ctx, int(rank), int(world), _ptr(o), C.cast(peers, C.c_void_p) if peers is not None else None), ctx)
+
+
+def caee_ep_obuf(ctx):
+    """(device address, bytes) of this context's o buffer (the target of its peers' stores)."""
+    p, n = C.c_void_p(), C.c_int64(0)
+    _check(_lib.caee_ep_obuf(ctx, C.addressof(p), C.addressof(n)), ctx)
+    return p.value, n.value
+
+
+def caee_ep_ipc_export(ctx):
+    h = (C.c_ubyte * 64)()
+    _check(_lib.caee_ep_ipc_export(ctx, C.addressof(h)), ctx)
+    return bytes(h)
+
+
+def caee_ep_ipc_open(ctx, handle):
+    h = (C.c_ubyte * 64)(*handle)
+    p = C.c_void_p()
+    _check(_lib.caee_ep_ipc_open(ctx, C.addressof(h), C.addressof(p)), ctx)
+    return p.value
+
+
+def caee_ep_ipc_close(ctx, peer_ptr):
+    _check(_lib.caee_ep_ipc_close(ctx, int(peer_ptr)), ctx)
+
+
+def caee_ep_combine(ctx, T, y, stream=None):
+    _check(_lib.caee_ep_combine(ctx, int(T), _ptr(y), _stream(stream)), ctx)
+
+
+def caee_ep_plan(ctx, counts, offs, tok, slot, expert, stream=None):
+    _check(_lib.caee_ep_plan(ctx, _ptr(counts), _ptr(offs), _ptr(tok), _ptr(slot), _ptr(expert), _stream(stream)), ctx)
 
 
 # ---- small conveniences for tests / bench (marshalling only) -----------------------------

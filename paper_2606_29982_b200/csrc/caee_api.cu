@@ -145,8 +145,12 @@ void free_all(caee_ctx* c) {
     if (c->packed.on_host[e]) cudaFreeHost(c->packed.base[e]);
     else cudaFree(c->packed.base[e]);
   }
-  for (uint8_t* p : c->stage_slot)
+  for (uint8_t* p : c->stage_ring)
     if (p) cudaFree(p);
+  for (cudaEvent_t e : c->ring_free_ev) cudaEventDestroy(e);
+  if (c->ring_ptr_pin) cudaFreeHost(c->ring_ptr_pin);
+  for (cudaEvent_t e : c->prof_off_ev) cudaEventDestroy(e);
+  c->prof_off_ev.clear();
   for (cudaEvent_t e : c->fetch_ev) cudaEventDestroy(e);
   if (c->host_meta) cudaFreeHost(c->host_meta);
   if (c->cache_up) cudaFreeHost(c->cache_up);
@@ -420,10 +424,12 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     P.base.assign(n, nullptr); P.on_host.assign(n, 0);
     P.bytes_per_expert = caee_umma_packed_bytes(c);
     if (!P.dev_ptrs) CAEE_CUDA(c, cudaMalloc((void**)&P.dev_ptrs, pb));
-    for (uint8_t* q : c->stage_slot)
+    for (uint8_t* q : c->stage_ring)
       if (q) cudaFree(q);
+    for (cudaEvent_t ev : c->ring_free_ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : c->fetch_ev) cudaEventDestroy(ev);
-    c->stage_slot.assign(n, nullptr);
+    c->stage_ring.clear(); c->ring_free_ev.clear();
+    c->ring_next = 0;
     c->fetch_ev.clear();
     c->any_offload = false;
     if (c->cache) {
@@ -447,10 +453,7 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
         CAEE_CUDA(c, cudaMallocHost((void**)&P.base[e], P.bytes_per_expert));
         P.on_host[e] = 1;
         CAEE_CUDA(c, cudaMemcpy(P.base[e], tmp, P.bytes_per_expert, cudaMemcpyDeviceToHost));
-        if (!c->cache) {   // static offload: a staging slot per expert; cache mode: the cache's slots
-          CAEE_CUDA(c, cudaMalloc((void**)&c->stage_slot[e], P.bytes_per_expert));
-          dptr[e] = c->stage_slot[e];
-        }
+        // static offload: the image pointer is set per step to the ring slot the copy goes to; cache mode: the cache's slots
         cudaEvent_t ev;
         CAEE_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         c->fetch_ev.push_back(ev);
@@ -459,6 +462,21 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     }
     CAEE_CUDA(c, cudaDeviceSynchronize());
     if (tmp) cudaFree(tmp);
+    if (c->any_offload && !c->cache) {
+      // the staging ring (caee_internal.cuh): a few slots, reused by the misses of every step
+      const int n_ring = std::min<int>(CAEE_STAGE_RING, (int)c->fetch_ev.size());
+      if (!c->ring_ptr_pin) CAEE_CUDA(c, cudaMallocHost((void**)&c->ring_ptr_pin, sizeof(uint8_t*) * CAEE_STAGE_RING));
+      for (int i = 0; i < n_ring; ++i) {
+        uint8_t* q = nullptr;
+        CAEE_CUDA(c, cudaMalloc((void**)&q, P.bytes_per_expert));
+        c->stage_ring.push_back(q);
+        c->ring_ptr_pin[i] = q;
+        cudaEvent_t ev;
+        CAEE_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        CAEE_CUDA(c, cudaEventRecord(ev, nullptr));       // nothing to wait for yet
+        c->ring_free_ev.push_back(ev);
+      }
+    }
     CAEE_CUDA(c, cudaMemcpy(P.dev_ptrs, dptr.data(), pb, cudaMemcpyHostToDevice));
     CAEE_CUDA(c, cudaDeviceSynchronize());
     c->dptr_h = dptr;
@@ -660,19 +678,45 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
       for (size_t i = 0; i < segs.size(); ++i)
         CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs + segs[i].e, &c->dptr_h[segs[i].e], sizeof(void*), cudaMemcpyHostToDevice, st));
     }
-    for (size_t i = 0; i < segs.size(); ++i) {
-      const int e = segs[i].e;
-      uint8_t* dst = c->cache ? miss_slots[i] : c->stage_slot[e];
-      CAEE_CUDA(c, cudaMemcpyAsync(dst, c->packed.base[e], c->packed.bytes_per_expert, cudaMemcpyHostToDevice, c->side_stream));
-      CAEE_CUDA(c, cudaEventRecord(c->fetch_ev[i], c->side_stream));
-    }
+    const int n_ring = (int)c->stage_ring.size();
+    cudaEvent_t* pev = (prof && (size_t)c->prof_used * 4 + 3 < c->prof_off_ev.size()) ? &c->prof_off_ev[(size_t)c->prof_used * 4] : nullptr;
     n_fetch = (int)segs.size();
     if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used], st);
+    if (pev) { cudaEventRecord(pev[0], c->side_stream); cudaEventRecord(pev[2], st); }
     if (n_res > 0 && (rc = caee_launch_expert_umma(c, x, T, 0, n_res, 0, st)) != CAEE_OK) return rc;
-    for (size_t i = 0; i < segs.size(); ++i) {
-      CAEE_CUDA(c, cudaStreamWaitEvent(st, c->fetch_ev[i], 0));
-      if ((rc = caee_launch_expert_umma(c, x, T, segs[i].begin, segs[i].count, 1 + (int)i, st)) != CAEE_OK) return rc;
+    if (pev) cudaEventRecord(pev[3], st);
+    // Fetched experts run in groups of consecutive misses: the group's copies (side stream, back to back with the
+    // previous group's), then ONE expert-kernel launch behind the group's last copy.  Static offload stages the
+    // images in the ring: a slot is free again once the launch that last read it is done, so the copy train runs at
+    // most one ring ahead of the launches — enqueued in this order, which is what makes the slot events valid.
+    const size_t G = c->cache ? 1 : (size_t)std::max(1, std::min<int>(CAEE_FETCH_GROUP, n_ring / 2));
+    int ticket = 1;
+    std::vector<int> slot_of(G, -1);
+    for (size_t i = 0; i < segs.size(); i += G) {
+      const size_t j = std::min(segs.size(), i + G) - 1;          // last miss of the group
+      for (size_t q = i; q <= j; ++q) {
+        const int e = segs[q].e;
+        uint8_t* dst;
+        if (c->cache) {
+          dst = miss_slots[q];
+        } else {
+          const int sl = (int)(c->ring_next++ % (unsigned)n_ring);
+          slot_of[q - i] = sl;
+          dst = c->stage_ring[sl];
+          CAEE_CUDA(c, cudaStreamWaitEvent(c->side_stream, c->ring_free_ev[sl], 0));
+          // the expert's image pointer follows the slot (pinned source: nothing here waits for the stream)
+          CAEE_CUDA(c, cudaMemcpyAsync(c->packed.dev_ptrs + e, &c->ring_ptr_pin[sl], sizeof(void*), cudaMemcpyHostToDevice, st));
+        }
+        CAEE_CUDA(c, cudaMemcpyAsync(dst, c->packed.base[e], c->packed.bytes_per_expert, cudaMemcpyHostToDevice, c->side_stream));
+      }
+      CAEE_CUDA(c, cudaEventRecord(c->fetch_ev[j], c->side_stream));
+      CAEE_CUDA(c, cudaStreamWaitEvent(st, c->fetch_ev[j], 0));
+      const int begin = segs[i].begin, count = segs[j].begin + segs[j].count - begin;
+      if ((rc = caee_launch_expert_umma(c, x, T, begin, count, ticket++, st)) != CAEE_OK) return rc;
+      if (!c->cache)
+        for (size_t q = i; q <= j; ++q) CAEE_CUDA(c, cudaEventRecord(c->ring_free_ev[slot_of[q - i]], st));
     }
+    if (pev) cudaEventRecord(pev[1], c->side_stream);
   }
   if (prof) cudaEventRecord(c->prof_ev[2 * c->prof_used++ + 1], st);
   // expert parallelism: the o rows of this device's home tokens are still arriving from its peers; the caller
@@ -837,6 +881,26 @@ caee_status caee_profile(caee_ctx* c, int32_t n_slots) {
   c->prof_ev.assign((size_t)n_slots * 2, nullptr);
   c->prof_used = 0;
   for (auto& e : c->prof_ev) CAEE_CUDA(c, cudaEventCreate(&e));
+  for (cudaEvent_t e : c->prof_off_ev) cudaEventDestroy(e);
+  c->prof_off_ev.assign(c->any_offload ? (size_t)n_slots * 4 : 0, nullptr);
+  for (auto& e : c->prof_off_ev) CAEE_CUDA(c, cudaEventCreate(&e));
+  return CAEE_OK;
+}
+
+caee_status caee_profile_read_offload(caee_ctx* c, int32_t cap, float* copy_ms, float* resident_ms, float* lead_ms, int32_t* n_out) {
+  if (!c) return CAEE_EINVAL;
+  if (!copy_ms || !resident_ms || !lead_ms || !n_out) return caee_fail(c, CAEE_EINVAL, "an output pointer is NULL");
+  DeviceGuard g(c->device);
+  const int n = std::min<int>({c->prof_used, cap, (int)(c->prof_off_ev.size() / 4)});
+  for (int i = 0; i < n; ++i) {
+    cudaEvent_t* ev = &c->prof_off_ev[(size_t)i * 4];
+    CAEE_CUDA(c, cudaEventSynchronize(ev[1]));
+    CAEE_CUDA(c, cudaEventSynchronize(ev[3]));
+    CAEE_CUDA(c, cudaEventElapsedTime(&copy_ms[i], ev[0], ev[1]));       // the step's copy train, first copy .. last copy
+    CAEE_CUDA(c, cudaEventElapsedTime(&resident_ms[i], ev[2], ev[3]));   // the resident experts' launch
+    CAEE_CUDA(c, cudaEventElapsedTime(&lead_ms[i], ev[0], ev[3]));       // copy train start .. resident launch done
+  }
+  *n_out = n;
   return CAEE_OK;
 }
 

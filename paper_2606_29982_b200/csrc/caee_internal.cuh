@@ -19,6 +19,8 @@
 #define CAEE_RUN_TOKENS_MIN 64
 #define CAEE_RUN_TOKENS_WIDE 256 /* e4m3 prefill kernel (expert_fp8_wide.cu): one N = 256 UMMA tile */
 #define CAEE_FP8_WIDE_MIN_TOKENS 257 /* steps of at least this many tokens take the e4m3 prefill kernel */
+#define CAEE_STAGE_RING 8  /* staging slots of the static offload path */
+#define CAEE_FETCH_GROUP 4 /* fetched experts per expert-kernel launch */
 #define CAEE_EP_MAX 8 /* most devices of an expert-parallel group (one NVSwitch domain) */
 #define CAEE_DECIDE_MAX_TOKENS 256 /* largest step the one-kernel decision path takes (decide.cu) */
 
@@ -174,8 +176,18 @@ struct caee_ctx {
   // on the side stream, only when they survive pruning
   cudaStream_t side_stream = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-  std::vector<uint8_t*> stage_slot;      // [E+S] device staging slot of a non-resident expert, else NULL
+  // Static offload stages the fetched images in a small RING of device slots (not one slot per non-resident
+  // expert: 192 x 88 MB would pin 16.9 GB of HBM): miss i of a step goes to slot (ring_next + i) % n, after the
+  // expert-kernel launch that last read that slot (ring_free_ev).  Fetched experts run in groups of
+  // CAEE_FETCH_GROUP per expert-kernel launch, each launch behind the last copy of its group.
+  std::vector<uint8_t*> stage_ring;      // device slots of one packed expert each
+  std::vector<cudaEvent_t> ring_free_ev; // per slot: the last launch that read it has been enqueued up to here
+  uint8_t** ring_ptr_pin = nullptr;      // pinned copy of stage_ring (source of the per-miss image-pointer updates)
+  unsigned ring_next = 0;
   std::vector<cudaEvent_t> fetch_ev;     // one per non-resident expert
+  // copy-train timing of profiled offloading steps (caee_profile / caee_profile_read_offload): per slot
+  // {first copy starts, last copy ends} on the side stream, {resident launch starts, ends} on the caller's
+  std::vector<cudaEvent_t> prof_off_ev;  // 4 per slot
   int32_t* host_meta = nullptr;          // pinned: meta[16] then run_expert[max_runs]
   bool any_offload = false;
 

@@ -113,8 +113,37 @@ def sass_summary(title, want):
                 print(f"  - `{first[fn][op]}`")
 
 
+def launches_summary(title, command, note):
+    """stdin: the --csv log of `ncu --metrics gpu__time_duration.sum` (one row per launch)."""
+    rows = list(csv.reader(l for l in sys.stdin if l.startswith('"')))
+    hdr = rows[0]
+    ki, vi, ui = hdr.index("Kernel Name"), hdr.index("Metric Value"), hdr.index("Metric Unit")
+    agg, order = {}, []
+    for r in rows[1:]:
+        n = short(r[ki])
+        if n not in agg:
+            agg[n] = []
+            order.append(n)
+        agg[n].append(to_us(r[vi], r[ui]))
+    total = sum(sum(v) for v in agg.values())
+    print(f"# {title}\n")
+    if command:
+        print(f"Command:\n\n```\n{command}\n```\n")
+    print(f"Table written by `python -m paper_2606_29982_b200.profile_summary --launches` from the launch list (the `.csv` beside "
+          f"this file = ncu's log without its `==PROF==` lines) at commit `{git_head()}`.  Times under the profiler are cold-cache and "
+          "serialised (short kernels also run at reduced clocks between replays): only SHARES are comparable with the live "
+          "CUDA-event timing of bench.py.\n")
+    if note:
+        print(note + "\n")
+    print("| kernel | launches | mean us | min us | max us | share of listed time |\n|---|---|---|---|---|---|")
+    for n in order:
+        v = agg[n]
+        print(f"| `{n}` | {len(v)} | {statistics.mean(v):.1f} | {min(v):.1f} | {max(v):.1f} | {100 * sum(v) / total:.1f}% |")
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--launches", action="store_true", help="stdin is the --csv launch list of `ncu --metrics gpu__time_duration.sum`")
     ap.add_argument("--sass", action="store_true", help="stdin is `cuobjdump -sass`: count tensor / TMEM / TMA mnemonics per kernel")
     ap.add_argument("--kernels", default="k_expert,k_router_mma", help="--sass: comma-separated substrings of the kernels to list")
     ap.add_argument("--title", default="ncu summary")
@@ -127,6 +156,9 @@ def main():
     args = ap.parse_args()
     if args.sass:
         sass_summary(args.title, [w for w in args.kernels.split(",") if w])
+        return
+    if args.launches:
+        launches_summary(args.title, args.command, args.note)
         return
     rows = list(csv.reader(sys.stdin))
     hdr, units, data = rows[0], rows[1], rows[2:]

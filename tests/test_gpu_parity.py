@@ -747,3 +747,88 @@ def test_forward_is_cuda_graph_capturable(H):
             assert n_run_graph == B.read_stats(stats).n_run
     finally:
         L.close()
+
+
+# ---------------------------------------------------------------- NEXT-2: expert parallelism
+@pytest.mark.parametrize("cfg_name,world,mode,scattered", [("C1", 2, "rank", False), ("R1S", 2, "dense", False), ("R1S", 4, "thresh", True),
+                                                           ("C2S", 4, "cir", False), ("C4S", 2, "frac", True), ("R1S", 8, "cir", False)])
+def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered):
+    """`world` contexts in one process stand for the ranks of an expert-parallel group: each owns a
+    subset of the experts and runs ITS slice of the step (the runs of its experts, the shared experts of its
+    home tokens), storing every o row into the home rank's o buffer (here: plain pointers instead of IPC
+    handles); the slices run one after the other on one stream — nobody waits for anybody — and then every
+    rank combines its home tokens.  Result: bit-identical to the single-device step, within tolerance of the
+    oracle; the explicit dispatch plan equals oracle/ep_oracle.py's (R38)."""
+    from oracle import ep_oracle
+    from paper_2606_29982_b200 import binding as B
+    from paper_2606_29982_b200 import ep
+    cfg = {"C1": wl.C1, "R1S": R1S, "C2S": C2S, "C4S": C4S}[cfg_name]
+    T = 29 if cfg_name != "C1" else 16
+    single = _layer(H, cfg, max_tokens=32)
+    ranks = [_layer(H, cfg, max_tokens=32) for _ in range(world)]
+    try:
+        rng = np.random.default_rng(5)
+        owner = rng.integers(0, world, size=cfg.E).astype(np.int32) if scattered else ep.owner_table(cfg.E, world)
+        peers = [B.caee_ep_obuf(L.ctx)[0] for L in ranks]
+        for r, L in enumerate(ranks):
+            B.caee_set_ep(L.ctx, r, world, owner, peers)
+        m, theta = MODES.get(mode, (0, 0.0))
+        th = _thresh_theta(cfg, T) if theta is None else theta
+        params = None if mode == "dense" else B.prune_params(m, th)
+        x = wl.hidden(cfg, T, 31, single.device)
+        s = single.oracle_scores(x)
+        s_dev = torch.from_numpy(s).to(single.device)
+        d = single.oracle_decisions(s, None if mode == "dense" else m, th)
+        y1 = single.forward(x, params, s_dev)
+        # step 2 of the protocol on every rank, then (after all of them) step 4
+        y = torch.full_like(x, float("nan"))
+        for L in ranks:
+            B.caee_moe_forward_from_scores(L.ctx, x, s_dev, T, params, None)
+        torch.cuda.synchronize()
+        for L in ranks:
+            B.caee_ep_combine(L.ctx, T, y)
+        torch.cuda.synchronize()
+        assert torch.equal(y.view(torch.int16) if y.dtype == torch.bfloat16 else y.view(torch.int32),
+                           y1.view(torch.int16) if y1.dtype == torch.bfloat16 else y1.view(torch.int32))
+        H.check_y(y, single.oracle_y(x, d["idx"], d["gate"], range(T)), range(T), H.TOL[cfg.w_dtype])
+        for L in ranks:                                           # every rank took the same decision
+            idx_g, gate_g = L.last_routing(T)
+            assert np.array_equal(idx_g, d["idx"]) and np.array_equal(gate_g.view(np.uint32), d["gate"].view(np.uint32))
+        # the explicit dispatch plan of the step (any rank; they are identical)
+        dev = single.device
+        counts, offs = torch.zeros(world, dtype=torch.int32, device=dev), torch.zeros(world + 1, dtype=torch.int32, device=dev)
+        tok, slot, expert = (torch.full((T * cfg.k,), -1, dtype=torch.int32, device=dev) for _ in range(3))
+        B.caee_ep_plan(ranks[-1].ctx, counts, offs, tok, slot, expert)
+        torch.cuda.synchronize()
+        p = ep_oracle.ep_plan(d["idx"], owner, world)
+        n = int(p["offs"][-1])
+        assert np.array_equal(counts.cpu().numpy(), p["counts"]) and np.array_equal(offs.cpu().numpy(), p["offs"])
+        assert np.array_equal(tok.cpu().numpy()[:n], p["tok"]) and np.array_equal(slot.cpu().numpy()[:n], p["slot"])
+        assert np.array_equal(expert.cpu().numpy()[:n], p["expert"])
+        # switching expert parallelism off restores the single-device step
+        B.caee_set_ep(ranks[0].ctx, 0, 1, None, None)
+        y0 = ranks[0].forward(x, params, s_dev)
+        assert torch.equal(y0.view(torch.int16) if y0.dtype == torch.bfloat16 else y0.view(torch.int32),
+                           y1.view(torch.int16) if y1.dtype == torch.bfloat16 else y1.view(torch.int32))
+    finally:
+        single.close()
+        for L in ranks:
+            L.close()
+
+
+def test_expert_parallel_argument_errors(H):
+    from paper_2606_29982_b200 import binding as B
+    L = _layer(H, C2S, max_tokens=8)
+    try:
+        mine = B.caee_ep_obuf(L.ctx)[0]
+        owner = np.zeros(C2S.E, np.int32)
+        for args, code in (((0, 9, owner, [mine] * 9), B.CAEE_EINVAL), ((2, 2, owner, [mine, mine]), B.CAEE_EINVAL),
+                           ((0, 2, owner + 5, [mine, mine]), B.CAEE_EINVAL), ((1, 2, owner, [mine, mine + 256]), B.CAEE_EINVAL)):
+            with pytest.raises(B.CaeeError) as ei:
+                B.caee_set_ep(L.ctx, *args)
+            assert ei.value.code == code
+        with pytest.raises(B.CaeeError) as ei:                    # no group set
+            B.caee_ep_combine(L.ctx, 4, torch.zeros(4, C2S.H, dtype=torch.bfloat16, device=L.device))
+        assert ei.value.code == B.CAEE_ESTATE
+    finally:
+        L.close()
