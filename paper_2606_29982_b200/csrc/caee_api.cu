@@ -200,6 +200,7 @@ caee_status create_impl(caee_ctx* c) {
   c->wl.ready = c->wl.sched + c->wl.n_tickets;
   if (caee_wl_hist_ints(c)) { A(c->wl_hist, caee_wl_hist_ints(c)); }
   c->h_rows_cap = Tm * k + 15 * std::min(E, Tm * k) + S * (Tm + 15) + 16;
+  c->wl.ent_cap = (int32_t)(Tm * (k + S)); c->wl.hrow_cap = (int32_t)c->h_rows_cap;
   if (c->kernel == CAEE_KERNEL_SIMT) { A(c->hbuf_f32, c->h_rows_cap * d.I); }
   else { A(c->hbuf_b16, c->h_rows_cap * d.I); }
   if (c->kernel == CAEE_KERNEL_UMMA && d.w_dtype == CAEE_E4M3) {

@@ -12,6 +12,16 @@
 
 #include "../../include/caee.h"
 
+// Bounds checks of our own (compute-sanitizer is closed on this pool): a build with -DCAEE_ASSERTS
+// (CAEE_NVCC_EXTRA) traps the kernel when an index computed on the device leaves its array; the small parity
+// tests are run under such a build (profiles/r02_asserts.md).  Compiled out of the product build.
+#ifdef CAEE_ASSERTS
+#include <cassert>
+#define CAEE_DEV_ASSERT(cond) assert(cond)
+#else
+#define CAEE_DEV_ASSERT(cond) ((void)0)
+#endif
+
 #define CAEE_FIX_ONE_F 1099511627776.0f /* 2^40: fixed-point unit of I(e) */
 #define CAEE_MAX_E 512
 #define CAEE_MAX_D 64
@@ -45,6 +55,7 @@ struct caee_worklist {
   int32_t* sched;       // [n_tickets + max_runs]: tile-ticket counters (one per expert-kernel launch of a step),
   int32_t* ready;       //   then (= sched + n_tickets) per-run "h complete" counters; zeroed every step
   int32_t max_runs, n_tickets;
+  int32_t ent_cap, hrow_cap;   // entries of ent_tok / ent_dst, rows of the h scratch (bounds, CAEE_ASSERTS builds)
   int32_t run_cap;      // tokens per run this step: CAEE_RUN_TOKENS, 64 (UMMA decode steps, T <= 128) or
                         // CAEE_RUN_TOKENS_WIDE (e4m3 prefill steps)
   // Expert parallelism (caee_set_ep): this device runs only the experts it
@@ -120,7 +131,8 @@ struct caee_ctx {
   caee_packed packed;
 
   uint8_t* wr_img = nullptr;        // three bf16 terms of W_r as MMA stage images (router_mma.cu); NULL: shape not supported
-  int router_mma_min_tokens = 257;  // steps of at least this many tokens take the tensor-core router (env CAEE_ROUTER_MMA_MIN_TOKENS)
+  int router_mma_min_tokens = 64;   // steps of at least this many tokens take the tensor-core router (env CAEE_ROUTER_MMA_MIN_TOKENS;
+                                    // measured on C3: T=32 +-0, T=64 -4 us, T=128 -17 us, T=256 -42 us, T=4096 -440 us per step)
 
   // scratch
   float* partial = nullptr;  // [ksplit, T, E] split-K partial logits of x W_r^T (sized for the worst T)

@@ -364,6 +364,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8(const __grid_constan
         __syncwarp();
         asm volatile("fence.proxy.async;" ::: "memory");
       }
+      CAEE_DEV_ASSERT(n >= 1 && n <= p.wl.run_cap && start >= 0 && start + n <= p.wl.ent_cap && p.wl.run_hrow[t.run] + npad <= p.wl.hrow_cap);
       const bool mine = lane * 4 < npad;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty0 + 8 * stage, ph ^ 1);
@@ -535,6 +536,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     // split k range (KSplit, umma_common.cuh): leave this sub-tile's partial sums and count it; a reducer
     // warp finishes the tile (n <= kKSplitCols: CT == 8 and the hf == 0 warps hold every column)
     const int tile = (t.run - p.run_begin) * p.P1 + t.sub;
+    CAEE_DEV_ASSERT(tile >= 0 && tile < p.ksp.tile_cap && n <= kKSplitCols);
     float* mine = p.ksp.part + ((size_t)tile * KS + t.kq) * (2 * kKSplitCols * kTileRows);
     if (hf == 0) {
 #pragma unroll
@@ -604,6 +606,7 @@ __device__ __forceinline__ void fp8_epilogue_tile(const Fp8Params& p, const Tile
     for (int c = 0; c < CT; ++c) {
       const int col = col0 + c;
       if (col < n) {
+        CAEE_DEV_ASSERT(p.wl.ent_dst[start + col] >= 0 && p.wl.ent_dst[start + col] < p.wl.ent_cap);
         float* o = caee_o_base(p.wl, p.obuf, p.wl.ent_tok[start + col]) + (ocol - p.obuf) + (size_t)p.wl.ent_dst[start + col] * p.H;
         o[0] = acc0[c];
         o[kTileRows] = acc1[c];

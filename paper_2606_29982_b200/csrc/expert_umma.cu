@@ -212,6 +212,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
         __syncwarp();
         asm volatile("fence.proxy.async;" ::: "memory");
       }
+      CAEE_DEV_ASSERT(n >= 1 && n <= p.wl.run_cap && start >= 0 && start + n <= p.wl.ent_cap && p.wl.run_hrow[t.run] + npad <= p.wl.hrow_cap);
       const bool mine = lane * 4 < npad;
       for (int kb = 0; kb < nkb; ++kb) {
         mbar_wait(empty0 + 8 * stage, ph ^ 1);
@@ -282,6 +283,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty0 + 8 * as);
         const int tile = (t.run - p.run_begin) * p.P1 + t.sub;
+        CAEE_DEV_ASSERT(tile >= 0 && tile < p.ksp.tile_cap && n <= kKSplitCols);
         float* mine = p.ksp.part + ((size_t)tile * KS + t.kq) * (2 * kKSplitCols * kTileRows);
 #pragma unroll
         for (int c = 0; c < kKSplitCols; ++c) {
@@ -323,6 +325,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             if (c + j < n) {
+              CAEE_DEV_ASSERT(p.wl.ent_dst[start + c + j] >= 0 && p.wl.ent_dst[start + c + j] < p.wl.ent_cap);
               float* o = caee_o_base(p.wl, p.obuf, p.wl.ent_tok[start + c + j]) + (ocol - p.obuf) + (size_t)p.wl.ent_dst[start + c + j] * p.H;
               o[0] = __uint_as_float(d0[j]);
               o[kTileRows] = __uint_as_float(d1[j]);

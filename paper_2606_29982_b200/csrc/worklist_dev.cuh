@@ -105,6 +105,7 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
     wl.offs[ex[0]] = ex[1];
     const int r0 = res ? ex[2] : tot[2] + sh_runs + ex[4];
     const int h0 = res ? ex[3] : tot[3] + S * sh_rows_each + ex[5];
+    CAEE_DEV_ASSERT(r0 + nch <= wl.max_runs && h0 + rows <= wl.hrow_cap && ex[1] + c <= wl.ent_cap);
     for (int j = 0; j < nch; ++j) {
       wl.run_expert[r0 + j] = e;
       wl.run_start[r0 + j] = ex[1] + j * cap;
@@ -115,6 +116,7 @@ __device__ __forceinline__ void caee_wl_scan_block(const caee_worklist& wl, int 
   for (int i = e; i < sh_runs; i += blockDim.x) {   // shared-expert runs over all (home) tokens
     const int s = i / sh_chunks, j = i - s * sh_chunks, t0 = j * cap;
     const int r = tot[2] + i;
+    CAEE_DEV_ASSERT(r < wl.max_runs && tot[3] + s * sh_rows_each + j * cap + ((min(cap, Th - t0) + 15) & ~15) <= wl.hrow_cap);
     wl.run_expert[r] = E + s;
     wl.run_start[r] = T * k + s * T + t_lo + t0;
     wl.run_n[r] = min(cap, Th - t0);
@@ -146,6 +148,7 @@ __device__ __forceinline__ void caee_wl_fill_token(const caee_worklist& wl, cons
       int pos = estart[e];
       for (int w = 0; w < (t >> 5); ++w) pos += __popc(kShared ? row[w] : __ldcg(row + w));
       pos += __popc((kShared ? row[t >> 5] : __ldcg(row + (t >> 5))) & ((1u << (t & 31)) - 1u));
+      CAEE_DEV_ASSERT(pos >= 0 && pos < TK && e < E);
       wl.ent_tok[pos] = t;
       wl.ent_slot[pos] = lane;
       wl.ent_wt[pos] = gr[lane];
