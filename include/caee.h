@@ -179,11 +179,15 @@ caee_status caee_destroy(caee_ctx* ctx);
 const char* caee_last_error(const caee_ctx* ctx);
 
 /* Router parameters (dev, fp32).  W_r [E,H]; b_logit [E] or NULL (added to the logit);
- * corr_bias [E] or NULL (added to the score for SELECTION only, R1). */
+ * corr_bias [E] or NULL (added to the score for SELECTION only, R1).  Steps of fewer than 64 tokens
+ * read W_r in place (fp32 FMAs); for larger steps (bf16 activations, E a multiple of 16 up to 256,
+ * H a multiple of 64) this call also makes the library's own copy of W_r as three bf16 terms
+ * (hi + mid + lo = W_r exactly) for the tensor-core router GEMM: fp32 accumulation of exact products,
+ * scores within the same 1e-5 relative bound.  Call it again after changing W_r. */
 caee_status caee_set_router(caee_ctx* ctx, const float* W_r, const float* b_logit, const float* corr_bias);
 /* Expert weights.  pack != 0: the library repacks each expert once into its own tile-major
- * copy (device memory for resident experts; pinned host memory plus a device staging slot of
- * the same size for non-resident ones) and no longer refers to the caller's buffers
+ * copy (device memory for resident experts; pinned host memory for non-resident ones, which share
+ * a ring of 8 device staging slots) and no longer refers to the caller's buffers
  * afterwards.  The UMMA kernel (bf16 or e4m3 weights with bf16 activations) requires
  * pack != 0; the SIMT kernel reads the caller's buffers in place and needs every expert in
  * device memory.  The e4m3 UMMA kernel feeds the e4m3 codes to the tensor cores as they are and
@@ -334,7 +338,10 @@ caee_status caee_cache_snapshot(const caee_cache* cache, int32_t* layer, int32_t
  * caee_ep_obuf pointer as seen from THIS device (its own at [rank]; peers' through caee_ep_ipc_open of
  * the handle their caee_ep_ipc_export wrote, 64 bytes, or plain pointers when the contexts share a
  * process).  world <= 1 or owner == NULL switches expert parallelism off.  Synchronises.  Not combinable
- * with non-resident experts or the expert cache (CAEE_ESTATE at the step).  The paper's per-device cost
+ * with non-resident experts or the expert cache (CAEE_ESTATE at the step).  When caee_set_ep precedes
+ * caee_set_weights, the weight pointers of experts the rank does not own may be NULL: they are neither
+ * read nor packed (a rank holds E/world routed experts + the shared ones); switching expert parallelism
+ * off, or handing the rank an expert it never loaded, then invalidates the weights (set them again).  The paper's per-device cost
  * model is unchanged: set the partitions to the owner table and F_cost is the max over the physical devices.
  * caee_ep_plan: the explicit dispatch plan of the LAST decision on this context — the valid
  * (token, slot) entries in ascending (device, expert, token) order: counts dev [world], offs dev [world+1],

@@ -400,7 +400,12 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
   const int n = c->d.E + c->d.S;
   const bool fp8 = c->d.w_dtype == CAEE_E4M3;
   if (fp8 && (!w->gate_scale || !w->up_scale || !w->down_scale)) return caee_fail(c, CAEE_EINVAL, "e4m3 weights need block scales");
+  // expert parallelism set up first (caee_set_ep): a rank needs only the experts it owns (and the shared ones);
+  // the others may be NULL and are skipped
+  auto needed = [&](int e) { return e >= c->d.E || c->ep_owner_h.empty() || c->ep_owner_h[e] == c->ep_rank; };
+  c->weights_partial = false;
   for (int e = 0; e < n; ++e) {
+    if (!needed(e) && !w->gate[e] && !w->up[e] && !w->down[e]) { c->weights_partial = true; continue; }
     if (!w->gate[e] || !w->up[e] || !w->down[e]) return caee_fail(c, CAEE_EINVAL, "expert %d has a NULL weight pointer", e);
     if (fp8 && (!w->gate_scale[e] || !w->up_scale[e] || !w->down_scale[e])) return caee_fail(c, CAEE_EINVAL, "expert %d has a NULL scale pointer", e);
   }
@@ -441,6 +446,7 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     std::vector<uint8_t*> dptr(n, nullptr);
     uint8_t* tmp = nullptr;  // device scratch for packing a host-resident expert
     for (int e = 0; e < n; ++e) {
+      if (!c->wg_h[e]) continue;    // an expert this rank does not own (expert parallelism): no image
       const bool res = e >= c->d.E || (!c->cache && c->resident_h[e]);
       if (res) {
         CAEE_CUDA(c, cudaMalloc((void**)&P.base[e], P.bytes_per_expert));
@@ -486,6 +492,7 @@ caee_status caee_set_weights(caee_ctx* c, const caee_expert_weights* w, int32_t 
     for (int e = 0; e < c->d.E; ++e)
       if (!c->resident_h[e]) return caee_fail(c, CAEE_EUNSUPPORTED, "the SIMT expert kernel needs every expert in device memory");
   }
+  if (c->weights_partial && (c->any_offload || c->cache)) return caee_fail(c, CAEE_ESTATE, "expert parallelism does not combine with offloaded experts or the expert cache");
   c->have_weights = true;
   return CAEE_OK;
 }
@@ -792,6 +799,8 @@ caee_status caee_set_ep(caee_ctx* c, int32_t rank, int32_t world, const int32_t*
   CAEE_CUDA(c, cudaDeviceSynchronize());
   if (world <= 1 || !owner) {                 // back to one device
     c->ep_rank = 0; c->ep_world = 1; c->wl.ep_owned = nullptr; c->wl.ep_world = 1;
+    c->ep_owner_h.clear();
+    if (c->weights_partial) c->have_weights = false;    // only this rank's experts were loaded: set the weights again
     return CAEE_OK;
   }
   if (world > CAEE_EP_MAX) return caee_fail(c, CAEE_EINVAL, "world=%d exceeds CAEE_EP_MAX=%d", world, CAEE_EP_MAX);
@@ -811,6 +820,9 @@ caee_status caee_set_ep(caee_ctx* c, int32_t rank, int32_t world, const int32_t*
   if (!c->ep_owner && (rc = dev_alloc(c, &c->ep_owner, (size_t)E)) != CAEE_OK) return rc;
   CAEE_CUDA(c, cudaMemcpy(c->ep_owned, owned.data(), E, cudaMemcpyHostToDevice));
   CAEE_CUDA(c, cudaMemcpy(c->ep_owner, owner, sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  if (c->weights_partial && c->have_weights)
+    for (int e = 0; e < E; ++e)
+      if (owner[e] == rank && !c->wg_h[e]) { c->have_weights = false; break; }   // a newly owned expert was never loaded
   c->ep_owner_h.assign(owner, owner + E);
   c->ep_rank = rank; c->ep_world = world;
   c->wl.ep_owned = c->ep_owned; c->wl.ep_world = world;

@@ -173,6 +173,7 @@ struct caee_ctx {
   uint8_t* ep_owned = nullptr;       // dev [E]
   std::vector<int32_t> ep_owner_h;   // [E] owner device of every routed expert
   float* ep_obuf_h[CAEE_EP_MAX] = {nullptr};
+  bool weights_partial = false;      // caee_set_weights skipped experts this rank does not own
   int32_t* ep_owner = nullptr;       // dev [E]
 
   long long n_launches = 0;          // kernels of this library enqueued by the per-step calls (caee_launch_count)

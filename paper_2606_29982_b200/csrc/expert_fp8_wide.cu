@@ -25,7 +25,11 @@
 // version of this kernel.  So both token operands are kept as per-run STAGE IMAGES: for run r
 // (rows padded to 16) stage s = the 64 k of every row, 128 bytes each, in 128-byte-swizzled
 // 8-row atoms — ONE contiguous bulk copy per stage.  x's images are written once per step by
-// k_gather_x (0.17 ms at 4096 tokens); h's images are written in place by the phase-1 epilogue.
+// k_gather_x (0.19 ms at 4096 tokens, bound by HBM writes: 0.59 GB); h's images are written in place by
+// the phase-1 epilogue.  (Round 2 tried to drop k_gather_x by gathering the x rows inside this kernel with
+// 16-byte cp.async copies from an fp16 copy of x — two loader warps, 2048 copies per stage, swizzled on the
+// way in, cp.async.mbarrier.arrive on the stage barrier: correct, but the expert kernel went from 4.15 to
+// 5.8 ms at 4096 tokens, so the images stay.)
 //
 // What bounds it.  Shared-memory bandwidth (128 B/clk): per 64 k the two MMAs read 32 KB of
 // weights and 2 x 32 KB of tokens, the bulk copy writes 32 KB of tokens and the converters write

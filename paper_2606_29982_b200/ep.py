@@ -68,7 +68,9 @@ def exchange_bytes(payload: bytes, group=None):
 
 
 class EpGroup:
-    """One rank of an expert-parallel group around a layer context (binding handle `ctx`)."""
+    """One rank of an expert-parallel group around a layer context (binding handle `ctx`).  Construct it BEFORE
+    caee_set_weights and the rank may pass NULL for the experts it does not own (it then holds E / world routed
+    experts + the shared ones)."""
 
     def __init__(self, ctx, E, owner=None, group=None):
         from . import binding as B

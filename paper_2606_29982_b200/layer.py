@@ -10,10 +10,13 @@ from . import workloads as wl
 
 class Layer:
     def __init__(self, cfg, seed=0, max_tokens=128, kernel=B.CAEE_KERNEL_AUTO, keep_raw=False, device="cuda:0",
-                 cache=None, layer_id=0, weight_seed=None):
+                 cache=None, layer_id=0, weight_seed=None, ep=None):
         """cache: a caee_cache handle — the layer's routed experts then live in pinned host memory and
         are served through the LFU cache (layer_id = its key there).  weight_seed: seed of the expert
-        weights when it should differ from the router's seed (layers of a synthetic multi-layer model)."""
+        weights when it should differ from the router's seed (layers of a synthetic multi-layer model).
+        ep: (rank, world, owner, obuf_peers_fn) — expert parallelism is set up BEFORE the weights and only the
+        experts the rank owns (and the shared ones) are drawn and loaded; obuf_peers_fn(ctx) returns the peers'
+        o-buffer addresses (the rank's own at [rank])."""
         self.cfg, self.seed, self.device, self.max_tokens = cfg, seed, device, max_tokens
         self.weight_seed = seed if weight_seed is None else weight_seed
         torch.cuda.set_device(device)
@@ -31,7 +34,13 @@ class Layer:
         self.ticks_res, self.ticks_miss = wl.cost_tables(cfg)
         B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
         n = cfg.E + cfg.S
-        raw = [wl.expert_weights(cfg, self.weight_seed, e, device) for e in range(n)]
+        mine = lambda e: True
+        if ep is not None:
+            rank, world, owner, peers_fn = ep
+            B.caee_set_ep(self.ctx, rank, world, owner, peers_fn(self.ctx))
+            mine = lambda e: e >= cfg.E or owner[e] == rank
+        none = dict.fromkeys(("gate", "up", "down", "gate_scale", "up_scale", "down_scale"))
+        raw = [wl.expert_weights(cfg, self.weight_seed, e, device) if mine(e) else none for e in range(n)]
         fp8 = cfg.w_dtype == wl.DT_E4M3
         B.caee_set_weights(self.ctx, [r["gate"] for r in raw], [r["up"] for r in raw], [r["down"] for r in raw],
                            [r["gate_scale"] for r in raw] if fp8 else None, [r["up_scale"] for r in raw] if fp8 else None,

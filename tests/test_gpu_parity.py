@@ -750,25 +750,30 @@ def test_forward_is_cuda_graph_capturable(H):
 
 
 # ---------------------------------------------------------------- NEXT-2: expert parallelism
-@pytest.mark.parametrize("cfg_name,world,mode,scattered", [("C1", 2, "rank", False), ("R1S", 2, "dense", False), ("R1S", 4, "thresh", True),
-                                                           ("C2S", 4, "cir", False), ("C4S", 2, "frac", True), ("R1S", 8, "cir", False)])
-def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered):
+@pytest.mark.parametrize("cfg_name,world,mode,scattered,partial", [
+    ("C1", 2, "rank", False, False), ("R1S", 2, "dense", False, True), ("R1S", 4, "thresh", True, True),
+    ("C2S", 4, "cir", False, False), ("C4S", 2, "frac", True, True), ("R1S", 8, "cir", False, True)])
+def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered, partial):
     """`world` contexts in one process stand for the ranks of an expert-parallel group: each owns a
     subset of the experts and runs ITS slice of the step (the runs of its experts, the shared experts of its
     home tokens), storing every o row into the home rank's o buffer (here: plain pointers instead of IPC
     handles); the slices run one after the other on one stream — nobody waits for anybody — and then every
     rank combines its home tokens.  Result: bit-identical to the single-device step, within tolerance of the
-    oracle; the explicit dispatch plan equals oracle/ep_oracle.py's (R38)."""
+    oracle; the explicit dispatch plan equals oracle/ep_oracle.py's (R38).  partial: the group is set up before
+    the weights and every rank loads ONLY the experts it owns (the other weight pointers are NULL)."""
     from oracle import ep_oracle
     from paper_2606_29982_b200 import binding as B
     from paper_2606_29982_b200 import ep
     cfg = {"C1": wl.C1, "R1S": R1S, "C2S": C2S, "C4S": C4S}[cfg_name]
     T = 29 if cfg_name != "C1" else 16
+    rng = np.random.default_rng(5)
+    owner = rng.integers(0, world, size=cfg.E).astype(np.int32) if scattered else ep.owner_table(cfg.E, world)
     single = _layer(H, cfg, max_tokens=32)
-    ranks = [_layer(H, cfg, max_tokens=32) for _ in range(world)]
+    if partial:      # the peers' buffers do not exist yet: the rank's own buffer stands in until they do
+        ranks = [_layer(H, cfg, max_tokens=32, ep=(r, world, owner, lambda ctx: [B.caee_ep_obuf(ctx)[0]] * world)) for r in range(world)]
+    else:
+        ranks = [_layer(H, cfg, max_tokens=32) for _ in range(world)]
     try:
-        rng = np.random.default_rng(5)
-        owner = rng.integers(0, world, size=cfg.E).astype(np.int32) if scattered else ep.owner_table(cfg.E, world)
         peers = [B.caee_ep_obuf(L.ctx)[0] for L in ranks]
         for r, L in enumerate(ranks):
             B.caee_set_ep(L.ctx, r, world, owner, peers)
@@ -805,11 +810,17 @@ def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered):
         assert np.array_equal(counts.cpu().numpy(), p["counts"]) and np.array_equal(offs.cpu().numpy(), p["offs"])
         assert np.array_equal(tok.cpu().numpy()[:n], p["tok"]) and np.array_equal(slot.cpu().numpy()[:n], p["slot"])
         assert np.array_equal(expert.cpu().numpy()[:n], p["expert"])
-        # switching expert parallelism off restores the single-device step
+        # switching expert parallelism off restores the single-device step — or, for a rank that loaded only its
+        # own experts, leaves it without weights until they are set again
         B.caee_set_ep(ranks[0].ctx, 0, 1, None, None)
-        y0 = ranks[0].forward(x, params, s_dev)
-        assert torch.equal(y0.view(torch.int16) if y0.dtype == torch.bfloat16 else y0.view(torch.int32),
-                           y1.view(torch.int16) if y1.dtype == torch.bfloat16 else y1.view(torch.int32))
+        if partial:
+            with pytest.raises(B.CaeeError) as ei:
+                ranks[0].forward(x, params, s_dev)
+            assert ei.value.code == B.CAEE_ESTATE
+        else:
+            y0 = ranks[0].forward(x, params, s_dev)
+            assert torch.equal(y0.view(torch.int16) if y0.dtype == torch.bfloat16 else y0.view(torch.int32),
+                               y1.view(torch.int16) if y1.dtype == torch.bfloat16 else y1.view(torch.int32))
     finally:
         single.close()
         for L in ranks:
