@@ -141,8 +141,47 @@ def launches_summary(title, command, note):
         print(f"| `{n}` | {len(v)} | {statistics.mean(v):.1f} | {min(v):.1f} | {max(v):.1f} | {100 * sum(v) / total:.1f}% |")
 
 
+def bench_table(title, command, note):
+    """stdin: bench.py result lines (one JSON object per line), e.g. the rows of a latency table."""
+    print(f"# {title}\n")
+    if command:
+        print(f"Command:\n\n```\n{command}\n```\n")
+    print(f"Table written by `python -m paper_2606_29982_b200.profile_summary --bench-table` from bench.py's JSON lines at commit "
+          f"`{git_head()}`.  step = `ms_per_step` (K steps between one event pair, with the expert kernel's own event pair inside); "
+          "w/o events = the same steps without the kernel events (programmatic dependent launches overlap); dense = the same batches "
+          "without pruning; kernel = the expert kernel's event-pair duration; rate = algorithmic bytes (or useful flops) / kernel time.\n")
+    if note:
+        print(note + "\n")
+    lines = [json.loads(l) for l in sys.stdin if l.strip().startswith("{")]
+    if lines and "rows" in lines[0]:
+        # bench.py --cache-loop lines: one table row per (tokens per step, setting)
+        print("| T | setting | ms / step | misses / step | hits / step | H2D GB / step | H2D GB/s | vs dense |\n|---|---|---|---|---|---|---|---|")
+        for d in lines:
+            T = d["config"]["workload"].split("T=")[1].split(" ")[0]
+            for r in d["rows"]:
+                print(f"| {T} | {r['setting']} | {r['ms_per_step']:.2f} | {r['misses_per_step']:.1f} | {r['hits_per_step']:.1f} | "
+                      f"{r['h2d_gb_per_step']:.2f} | {r['h2d_gbs']:.1f} | {r['vs_dense']:.3f} |")
+        return
+    print("| workload | T | mode | step us | w/o events us | dense us | kernel us | rate | frac of measured peak | experts run | launches / K steps | clocks MHz, reasons |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for d in lines:
+        w = d["config"]["workload"]
+        name = w.split(":")[0]
+        T = w.split("T=")[1].split(",")[0]
+        mode = "dense" if ", dense top-k" in w else w.split("CAEE prune ")[1].split(";")[0]
+        r, lat = d["roofline"], d["latency_us"]
+        rate = f"{r['achieved']:.0f} {r['unit']}" if r.get("achieved") else ""
+        frac = f"{r['frac']:.3f}" if r.get("frac") else ""
+        ker = f"{lat['expert_kernel']:.1f}" if lat.get("expert_kernel") else ""
+        plain = f"{lat['pruned_without_kernel_events']:.1f}" if lat.get("pruned_without_kernel_events") else ""
+        clk = d.get("clocks", {})
+        print(f"| {name} | {T} | {mode} | {lat['pruned']:.1f} | {plain} | {lat['dense']:.1f} | {ker} | {rate} | {frac} | "
+              f"{d['pruning']['n_run']} | {d['gpu_launches']} / {d['steps']} | {clk.get('sm_mhz')} {','.join(clk.get('reasons', [])) or '-'} |")
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--bench-table", action="store_true", help="stdin is bench.py JSON lines: format them as a latency table")
     ap.add_argument("--launches", action="store_true", help="stdin is the --csv launch list of `ncu --metrics gpu__time_duration.sum`")
     ap.add_argument("--sass", action="store_true", help="stdin is `cuobjdump -sass`: count tensor / TMEM / TMA mnemonics per kernel")
     ap.add_argument("--kernels", default="k_expert,k_router_mma", help="--sass: comma-separated substrings of the kernels to list")
@@ -159,6 +198,9 @@ def main():
         return
     if args.launches:
         launches_summary(args.title, args.command, args.note)
+        return
+    if args.bench_table:
+        bench_table(args.title, args.command, args.note)
         return
     rows = list(csv.reader(sys.stdin))
     hdr, units, data = rows[0], rows[1], rows[2:]

@@ -6,9 +6,12 @@ expert cost per device before and after pruning).
     python -m paper_2606_29982_b200.sweep --workload c3 --tokens 8,32,64,128 > sweep.md
 
 Everything is measured through the C ABI (caee_moe_forward + caee_fwd_stats); this module only
-marshals arguments and formats the table.  Latency = CUDA events around `--steps` calls after
-`--warmup` calls, rotating over 4 seeded token batches; the per-partition columns are the summed
-C~ ticks of the experts each partition keeps (stats.load) on the first batch.
+marshals arguments and formats the table.  Latency = median of `--steps` steps, each between its own
+CUDA-event pair, after `--warmup` steps, rotating over 4 seeded token batches; a pruned setting is
+measured INTERLEAVED with the dense step (dense, pruned, dense, pruned, ... on the same batches) so that
+"vs dense" compares steps taken in the same thermal / power state.  "experts run" and "GB read" are means
+over the 4 batches; kept / activated, F_cost and the per-partition columns (summed C~ ticks of the
+experts each partition keeps, stats.load) are the first batch's.
 """
 import argparse
 import statistics
@@ -20,24 +23,37 @@ from . import workloads as wl
 from .layer import Layer
 
 
-def measure(L, xs, params, steps, warmup):
+def measure(L, xs, params, steps, warmup, against_dense=False):
+    """(median step us, first batch's stats, mean experts run, mean GB read[, median us of the interleaved dense steps])."""
     dev = L.device
     y = torch.empty_like(xs[0])
     stats = B.stats_buffer(dev)
     for i in range(warmup):
         L.forward(xs[i % len(xs)], params, y=y, stats=stats)
-    L.forward(xs[0], params, y=y, stats=stats)
-    torch.cuda.synchronize()
-    st0 = B.read_stats(stats)
-    ms = []
-    for i in range(steps):
+    per_batch = []
+    for x in xs:
+        L.forward(x, params, y=y, stats=stats)
+        torch.cuda.synchronize()
+        per_batch.append(B.read_stats(stats))
+    st0 = per_batch[0]
+    n_run = statistics.mean(s.n_run for s in per_batch)
+    gb = statistics.mean(s.weight_bytes for s in per_batch) / 1e9
+
+    def one(x, p):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        L.forward(xs[i % len(xs)], params, y=y, stats=stats)
+        L.forward(x, p, y=y, stats=stats)
         e1.record()
         torch.cuda.synchronize()
-        ms.append(e0.elapsed_time(e1))
-    return statistics.median(ms) * 1e3, st0
+        return e0.elapsed_time(e1)
+
+    ms, ms_dense = [], []
+    for i in range(steps):
+        if against_dense:
+            ms_dense.append(one(xs[i % len(xs)], None))
+        ms.append(one(xs[i % len(xs)], params))
+    out = (statistics.median(ms) * 1e3, st0, n_run, gb)
+    return out + (statistics.median(ms_dense) * 1e3,) if against_dense else out
 
 
 def ablation(L, cfg, Ts, args):
@@ -91,25 +107,25 @@ def main():
         return
     print(f"# Knob sweep, {cfg.name} (H={cfg.H} I={cfg.I} E={cfg.E}+{cfg.S} top-{cfg.k}, D={D} partitions, "
           f"partition {cfg.straggler_part} costs 2x)\n")
-    print("| T | setting | step µs | vs dense | experts run | GB read | F_cost ticks (dense → kept) | per-partition load after pruning, % of the dense max |")
-    print("|---|---|---|---|---|---|---|---|")
+    print("| T | setting | step µs | dense step µs (interleaved) | vs dense | experts run (mean of 4 batches) | kept / activated (batch 0) | GB read (mean) | F_cost ticks (dense → kept) | per-partition load after pruning, % of the dense max |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
     try:
         for T in Ts:
             xs = [wl.hidden(cfg, T, 100 + i, dev) for i in range(4)]
-            base_us, st = measure(L, xs, None, args.steps, args.warmup)
+            base_us, st, n_run, gb = measure(L, xs, None, args.steps, args.warmup)
             # dense loads: THRESH θ = 0 keeps every activated expert and reports the loads
-            _, st_d = measure(L, xs, B.prune_params(B.CAEE_PRUNE_THRESH, 0.0), 1, 1)
+            st_d = measure(L, xs, B.prune_params(B.CAEE_PRUNE_THRESH, 0.0), 1, 1)[1]
             fmax = max(1, st_d.F_cost_dense)
             loads = " ".join(f"{100 * st_d.load[d] / fmax:.0f}" for d in range(D))
-            print(f"| {T} | dense | {base_us:.0f} | 1.000 | {st.n_run} | {st.weight_bytes / 1e9:.2f} | {st_d.F_cost_dense} | {loads} |")
+            print(f"| {T} | dense | {base_us:.0f} | | 1.000 | {n_run:.1f} | | {gb:.2f} | {st_d.F_cost_dense} | {loads} |")
             grid = [("thresh", B.CAEE_PRUNE_THRESH, float(v)) for v in args.thresh.split(",") if v] + \
                    [("cir", B.CAEE_PRUNE_CIR, float(v)) for v in args.cir.split(",") if v] + \
                    [("frac", B.CAEE_PRUNE_FRAC, float(v)) for v in args.frac.split(",") if v]
             for name, mode, theta in grid:
-                us, s = measure(L, xs, B.prune_params(mode, theta), args.steps, args.warmup)
+                us, s, n_run, gb, dense_us = measure(L, xs, B.prune_params(mode, theta), args.steps, args.warmup, against_dense=True)
                 loads = " ".join(f"{100 * s.load[d] / fmax:.0f}" for d in range(D))
-                print(f"| {T} | {name} {theta:g} | {us:.0f} | {us / base_us:.3f} | {s.n_run} (kept {s.n_keep}/{s.n_act}) | "
-                      f"{s.weight_bytes / 1e9:.2f} | {s.F_cost_dense} → {s.F_cost} | {loads} |")
+                print(f"| {T} | {name} {theta:g} | {us:.0f} | {dense_us:.0f} | {us / dense_us:.3f} | {n_run:.1f} | {s.n_keep}/{s.n_act} | "
+                      f"{gb:.2f} | {s.F_cost_dense} → {s.F_cost} | {loads} |")
     finally:
         L.close()
 
