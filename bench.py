@@ -132,7 +132,8 @@ class OracleLayer:
         self.xb, self.Wr, self.b = wl.bits(x), Wr.cpu().numpy(), b_logit.cpu().numpy()
         self.cb = None if cb is None else cb.cpu().numpy()
         self.part = wl.partitions(cfg)
-        self.w_eff = orc.effective_cost(wl.residency(cfg, seed), *wl.cost_tables(cfg))
+        tables = (layer.ticks_res, layer.ticks_miss) if layer is not None else wl.cost_tables(cfg)     # the layer's may be calibrated
+        self.w_eff = orc.effective_cost(wl.residency(cfg, seed), *tables)
         idx, _ = self.decisions()[:2]
         n = cfg.E + cfg.S
         used = sorted(set(int(e) for e in idx.ravel() if e >= 0) | set(range(cfg.E, n)))
@@ -228,6 +229,12 @@ def run_caee(args, cfg, prune, eps):
         dist.init_process_group("nccl", device_id=torch.device(dev))
     T, K, W = args.tokens, args.steps, max(args.warmup, 3)
     L = Layer(cfg, seed=rank, max_tokens=max(T, 128), device=dev)
+    calib = None
+    if args.calibrate or cfg.n_resident >= 0:
+        # C5's two-tier cost table always comes from caee_calibrate_cost on the box
+        hbm, h2d = L.calibrate()
+        calib = {"hbm_gbs": hbm.gbytes_per_s, "hbm_overhead_ns": hbm.intercept_ns, "h2d_gbs": h2d.gbytes_per_s,
+                 "h2d_overhead_ns": h2d.intercept_ns, "ticks_resident": int(L.ticks_res.min()), "ticks_miss": int(L.ticks_miss.min())}
     params = None if prune is None else B.prune_params(prune[0], prune[1], 0, eps)
     xs = [wl.hidden(cfg, T, rank * 1000 + 100 + i, dev) for i in range(4)]      # rotate a few batches
     y = torch.empty_like(xs[0])
@@ -378,6 +385,8 @@ def run_caee(args, cfg, prune, eps):
                     "F_cost": st.F_cost, "F_imp": st.F_imp / 2.0 ** 40, "eps": eps, "bytes_pruned": st.weight_bytes,
                     "bytes_dense": st_dense.weight_bytes, "bytes_removed_frac": removed, "n_run_dense": st_dense.n_run},
     }
+    if calib is not None:
+        out["calibrated_cost_table"] = calib
     if offload_t is not None and len(offload_t[0]):
         # offload scenario (BASELINE.json config 5): the step is bound by the H2D copy train of the surviving misses;
         # resident compute is hidden when it ends before the copies do (CUDA events on the two streams, same run)
@@ -392,8 +401,8 @@ def run_caee(args, cfg, prune, eps):
         gbs = h2d / (copy_ms * 1e-3) / 1e9 if copy_ms > 0 else None
         out["offload"]["h2d_bytes_per_step"] = h2d
         out["roofline"] = {"bound": "pcie", "kernel": "H2D copy train (one cudaMemcpyAsync per surviving miss, side stream)",
-                           "achieved": gbs, "peak": 55.6, "unit": "GB/s", "frac": gbs / 55.6 if gbs else None, "traffic": None,
-                           "peak_source": "caee_calibrate_cost H2D tier on this pool's B200 (DESIGN.md §4)",
+                           "achieved": gbs, "peak": calib["h2d_gbs"], "unit": "GB/s", "frac": gbs / calib["h2d_gbs"] if gbs else None, "traffic": None,
+                           "peak_source": "caee_calibrate_cost H2D tier, measured in this run",
                            "bytes_per_launch": h2d, "kernel_ms": copy_ms}
     if fp8 and T > 256:
         # prefill-size e4m3 step: k_expert_fp8_wide (fp16 MMAs) is bound by the tensor pipe / its
@@ -501,6 +510,8 @@ def main():
     ap.add_argument("--eps-frac", type=float, default=0.10,
                     help="importance bound F_imp <= eps-frac * T (PAPER.md:150-152; CAEE_IMP_BOUND); negative = no bound")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--calibrate", action="store_true",
+                    help="cost table from caee_calibrate_cost on this GPU (S10); always on for the offload workload c5")
     ap.add_argument("--cache-loop", action="store_true", help="SURVEY §8(f) NEXT-1: multi-layer decode loop over an LFU expert cache")
     ap.add_argument("--layers", type=int, default=2)
     ap.add_argument("--cache-slots", type=int, default=128)

@@ -121,8 +121,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
       // The next tile's ticket (an atomic round trip) and its image pointer (two dependent loads) are
       // fetched while the current tile's copies are being issued: claimed and resolved at the tile
       // boundary they left the copy engine idle for ~1.2 us per tile.  (Tickets still come in
-      // increasing order per CTA; every CTA ends on a ticket beyond the last tile.)
-      int nxt = atomicAdd(p.wl.sched + p.ticket, 1);
+      // increasing order per CTA; every CTA ends on a ticket beyond the last tile.)  The first tile of CTA b is tile b:
+      // no atomic round trip before the first weight byte is requested; the counter hands out tiles gridDim.x, ...
+      int nxt = (int)blockIdx.x;
       Tile tn;
       const uint8_t* srcn = nullptr;
       int nkbn = 0;
@@ -136,7 +137,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
         mbar_arrive(qfull0 + 8 * q);
         if (++q == kQueue) { q = 0; qph ^= 1; }
         if (!vn) break;
-        nxt = atomicAdd(p.wl.sched + p.ticket, 1);
+        nxt = (int)gridDim.x + atomicAdd(p.wl.sched + p.ticket, 1);
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty0 + 8 * stage, ph ^ 1);
           mbar_arrive_expect_tx(full0 + 8 * stage, kAStageBytes);
@@ -228,10 +229,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_umma(const __grid_consta
     // partial sums are complete; lane l holds features 4 l .. 4 l + 3
     if (KS > 1) {
       const int n_tiles = n_runs * p.P1;
-      for (;;) {
-        int j = 0;
-        if (lane == 0) j = atomicAdd(p.wl.sched + p.ksp.rticket, 1);
-        j = __shfl_sync(0xffffffffu, j, 0);
+      for (int first = 1;; first = 0) {
+        int j = (int)blockIdx.x;                                  // the first tile of CTA b's reducer is tile b
+        if (!first) {
+          if (lane == 0) j = (int)gridDim.x + atomicAdd(p.wl.sched + p.ksp.rticket, 1);
+          j = __shfl_sync(0xffffffffu, j, 0);
+        }
         if (j >= n_tiles) break;
         const int run = p.run_begin + j / p.P1, ft = j % p.P1;
         const int n = p.wl.run_n[run], hrow = p.wl.run_hrow[run];

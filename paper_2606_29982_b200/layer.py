@@ -52,6 +52,18 @@ class Layer:
             del raw
             torch.cuda.empty_cache()
 
+    def calibrate(self, n_sizes=8, iters=20):
+        """S10 on this GPU: replace the workload's formula costs by the table caee_calibrate_cost measures (HBM tier for
+        resident experts, pinned-host H2D tier for misses), keeping the workload's 2x straggler partition.  Returns the
+        two fits."""
+        import numpy as np
+        fits = B.caee_calibrate_cost(self.ctx, B.caee_calib_opts(n_sizes, iters, 0, 0, 1, 0))
+        tr, tm = B.caee_get_cost_table(self.ctx, self.cfg.E)
+        mult = np.where(self.part == self.cfg.straggler_part, 2, 1).astype(np.int64)
+        self.ticks_res, self.ticks_miss = tr * mult, tm * mult
+        B.caee_set_cost_table(self.ctx, self.ticks_res, self.ticks_miss)
+        return fits
+
     def close(self):
         if self.ctx is not None:
             B.caee_destroy(self.ctx)

@@ -93,12 +93,22 @@ def main():
     ap.add_argument("--steps", type=int, default=12)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--ablation", action="store_true", help="compensation ablation proxy instead of the latency sweep")
+    ap.add_argument("--calibrate", action="store_true", help="cost table from caee_calibrate_cost on this GPU (S10) instead of the workload's formula")
+    ap.add_argument("--partitions", type=int, default=0, help="override D (contiguous blocks, no straggler); D = 1 is the setting where "
+                    "the modelled F_cost and the bytes read coincide (SURVEY.md 8(d))")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.workload.upper()]
+    if args.partitions > 0:
+        cfg = wl.scaled(cfg, name=f"{cfg.name}-D{args.partitions}", D=args.partitions, straggler_part=-1)
     Ts = [int(t) for t in args.tokens.split(",")]
     dev = "cuda:0"
     L = Layer(cfg, seed=0, max_tokens=max(max(Ts), 128), device=dev)
     D = cfg.D
+    if args.calibrate:
+        hbm, h2d = L.calibrate()
+        print(f"Cost table calibrated on this GPU (caee_calibrate_cost, PAPER.md:137-141): HBM tier t = {hbm.slope_ns_per_byte:.3e} ns/B x S + "
+              f"{hbm.intercept_ns:.0f} ns ({hbm.gbytes_per_s:.0f} GB/s, r2 {hbm.r2:.3f}); H2D tier t = {h2d.slope_ns_per_byte:.3e} ns/B x S + "
+              f"{h2d.intercept_ns:.0f} ns ({h2d.gbytes_per_s:.1f} GB/s, r2 {h2d.r2:.3f}); C~ = {int(L.ticks_res.min())} ns per resident expert.\n")
     if args.ablation:
         try:
             ablation(L, cfg, Ts, args)

@@ -875,3 +875,44 @@ def test_forward_is_bitwise_repeatable(H, cfg_name, T, mode):
         assert torch.isfinite(y.float()).all()
     finally:
         L.close()
+
+
+def test_expert_parallel_c3_full_size(H):
+    """The bench's own point (C3, T = 128, THRESH 0.6 under eps = 0.1 T) as an 8-rank expert-parallel group on one
+    GPU: every rank holds only its partition's 32 experts (2.8 GB) + the shared expert; owner table = the cost
+    model's partition table, so F_cost's max is over the ranks.  y bit-identical to the single-device step, within
+    tolerance of the oracle on sampled tokens; the ranks' weight bytes add up to the single-device step's."""
+    from paper_2606_29982_b200 import binding as B
+    cfg, world, T = wl.C3, 8, 128
+    owner = wl.partitions(cfg)
+    single = H.GpuLayer(cfg, seed=0, max_tokens=128, keep_raw=False)
+    ranks = [H.GpuLayer(cfg, seed=0, max_tokens=128, keep_raw=False,
+                        ep=(r, world, owner, lambda ctx: [B.caee_ep_obuf(ctx)[0]] * world)) for r in range(world)]
+    try:
+        peers = [B.caee_ep_obuf(L.ctx)[0] for L in ranks]
+        for r, L in enumerate(ranks):
+            B.caee_set_ep(L.ctx, r, world, owner, peers)
+        m, th, eps = 1, 0.6, 0.10 * T
+        params = B.prune_params(m, th, 0, eps)
+        x = wl.hidden(cfg, T, 100, single.device)
+        s = single.oracle_scores(x)
+        s_dev = torch.from_numpy(s).to(single.device)
+        d = single.oracle_decisions(s, m, th, 0, eps)
+        y1, st1 = single.forward(x, params, s_dev, want_stats=True)
+        assert 0 < st1.n_keep < st1.n_act
+        y = torch.full_like(x, float("nan"))
+        for L in ranks:
+            B.caee_moe_forward_from_scores(L.ctx, x, s_dev, T, params, None)
+        torch.cuda.synchronize()
+        for L in ranks:
+            B.caee_ep_combine(L.ctx, T, y)
+        torch.cuda.synchronize()
+        assert torch.equal(y.view(torch.int16), y1.view(torch.int16))
+        toks = _spread(T, 12)
+        H.check_y(y, single.oracle_y(x, d["idx"], d["gate"], toks, 6), toks, H.TOL[cfg.w_dtype])
+        idx_g, _ = ranks[3].last_routing(T)
+        assert np.array_equal(idx_g, d["idx"])
+    finally:
+        single.close()
+        for L in ranks:
+            L.close()
