@@ -498,6 +498,88 @@ def run_cache_loop(args, cfg):
         "rows": rows}))
 
 
+# --------------------------------------------------------------------------- NEXT-2: expert-parallel ranks, one at a time
+def run_ep_emulation(args, cfg, prune, eps):
+    """SURVEY.md §8(f) NEXT-2 on ONE GPU (PAPER.md:57, 97 `Latency_total = max_d Latency_d`, 127): `--ep-emulate W` builds
+    the W ranks of an expert-parallel group as W contexts in this process (each holds only the experts it owns, owner =
+    contiguous blocks = the cost model's partitions with D = W, no straggler) and times every rank's slice of the step ALONE
+    on the whole GPU — what that rank would take on a GPU of its own, without the NVLink transfers this box cannot show.
+    Reported: per-rank slice time (router + decision, replicated on every rank, + the rank's expert kernel), their max
+    (= the emulated step latency of the group) and sum, dense vs pruned, next to the modelled per-rank loads and F_cost."""
+    import torch
+    from paper_2606_29982_b200 import binding as B
+    from paper_2606_29982_b200 import ep
+    from paper_2606_29982_b200 import workloads as wl
+    from paper_2606_29982_b200.layer import Layer
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libcaee has no CPU fallback")
+    torch.cuda.set_device(0)
+    dev, W, T, K = "cuda:0", args.ep_emulate, args.tokens, args.steps
+    cfg = wl.scaled(cfg, name=f"{cfg.name}-EP{W}", D=W, straggler_part=-1)
+    owner = ep.owner_table(cfg.E, W)
+    ranks = [Layer(cfg, seed=0, max_tokens=max(T, 128), device=dev,
+                   ep=(r, W, owner, lambda ctx: [B.caee_ep_obuf(ctx)[0]] * W)) for r in range(W)]
+    peers = [B.caee_ep_obuf(L.ctx)[0] for L in ranks]
+    for r, L in enumerate(ranks):
+        B.caee_set_ep(L.ctx, r, W, owner, peers)
+    xs = [wl.hidden(cfg, T, 100 + i, dev) for i in range(4)]
+    y = torch.empty_like(xs[0])
+    stats = B.stats_buffer(dev)
+    stream = torch.cuda.current_stream()
+
+    def slice_times(params):
+        out = []
+        for L in ranks:
+            for i in range(3):
+                B.caee_moe_forward(L.ctx, xs[i % 4], T, params, None, stats)
+            torch.cuda.synchronize()
+            ms = []
+            for i in range(K):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                B.caee_moe_forward(L.ctx, xs[i % 4], T, params, None, stats)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+            out.append(statistics.median(ms))
+        B.caee_moe_forward(ranks[0].ctx, xs[0], T, params, None, stats)
+        torch.cuda.synchronize()
+        return out, B.read_stats(stats)
+
+    try:
+        params = None if prune is None else B.prune_params(prune[0], prune[1], 0, eps)
+        dense_ms, _ = slice_times(None)
+        _, st_d = slice_times(B.prune_params(B.CAEE_PRUNE_THRESH, 0.0))      # keeps everything, reports the modelled loads
+        pruned_ms, st_p = slice_times(params) if params is not None else (dense_ms, st_d)
+        # the combine of the home tokens (after the group barrier), timed once for completeness
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for L in ranks:
+            B.caee_ep_combine(L.ctx, T, y)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        combine_ms = e0.elapsed_time(e1) / W
+    finally:
+        for L in ranks:
+            L.close()
+    fmax = max(1, st_d.F_cost_dense)
+    print(json.dumps({
+        "metric": "ep_emulated_step_ms", "value": max(pruned_ms), "unit": "ms/step", "n_gpus": 1, "steps": K, "warmup": 3,
+        "higher_is_better": False, "vs_baseline": None, "dtype": {0: "f32", 1: "bf16", 2: "fp8_e4m3"}[cfg.w_dtype], "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: {W} expert-parallel ranks of {cfg.E // W} experts (+{cfg.S} shared, replicated), T={T}, "
+                               f"{'dense' if prune is None else 'CAEE prune ' + args.prune}; every rank's slice timed ALONE on one B200 "
+                               "(no NVLink transfers): emulated step latency = max over ranks (PAPER.md:97)"},
+        "ep": {"world": W, "slice_ms_dense": dense_ms, "slice_ms_pruned": pruned_ms,
+               "max_ms_dense": max(dense_ms), "max_ms_pruned": max(pruned_ms), "max_ratio": max(pruned_ms) / max(dense_ms),
+               "sum_ms_dense": sum(dense_ms), "sum_ms_pruned": sum(pruned_ms), "sum_ratio": sum(pruned_ms) / sum(dense_ms),
+               "modelled_load_dense_pct": [100.0 * st_d.load[d] / fmax for d in range(W)],
+               "modelled_load_pruned_pct": [100.0 * st_p.load[d] / fmax for d in range(W)],
+               "F_cost_dense": st_d.F_cost_dense, "F_cost_pruned": st_p.F_cost if params is not None else st_d.F_cost_dense,
+               "F_cost_ratio": (st_p.F_cost / fmax) if params is not None else 1.0,
+               "n_keep": st_p.n_keep, "n_act": st_p.n_act, "combine_ms_per_rank": combine_ms}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -513,6 +595,7 @@ def main():
     ap.add_argument("--calibrate", action="store_true",
                     help="cost table from caee_calibrate_cost on this GPU (S10); always on for the offload workload c5")
     ap.add_argument("--cache-loop", action="store_true", help="SURVEY §8(f) NEXT-1: multi-layer decode loop over an LFU expert cache")
+    ap.add_argument("--ep-emulate", type=int, default=0, help="SURVEY §8(f) NEXT-2: W expert-parallel ranks built in this process, every rank's slice timed alone")
     ap.add_argument("--layers", type=int, default=2)
     ap.add_argument("--cache-slots", type=int, default=128)
     args = ap.parse_args()
@@ -520,7 +603,9 @@ def main():
     cfg = wl.CONFIGS[args.workload.upper()]
     prune = parse_prune(args.prune)
     eps = args.eps_frac * args.tokens if (prune is not None and args.eps_frac >= 0) else None
-    if args.cache_loop:
+    if args.ep_emulate > 1:
+        run_ep_emulation(args, cfg, prune, eps)
+    elif args.cache_loop:
         run_cache_loop(args, cfg)
     elif args.impl == "reference":
         run_reference(args, cfg, prune, eps)

@@ -162,6 +162,19 @@ def bench_table(title, command, note):
                 print(f"| {T} | {r['setting']} | {r['ms_per_step']:.2f} | {r['misses_per_step']:.1f} | {r['hits_per_step']:.1f} | "
                       f"{r['h2d_gb_per_step']:.2f} | {r['h2d_gbs']:.1f} | {r['vs_dense']:.3f} |")
         return
+    if lines and "ep" in lines[0]:
+        # bench.py --ep-emulate lines: one row per (T, setting)
+        print("| ranks | T | setting | kept / activated | slowest rank ms, dense → pruned (= emulated step) | ratio | sum over ranks ms, dense → pruned | ratio | "
+              "modelled F_cost ratio | per-rank slice ms, pruned | modelled per-rank load, % of the dense max, pruned |")
+        print("|---|---|---|---|---|---|---|---|---|---|---|")
+        for d in lines:
+            e, w = d["ep"], d["config"]["workload"]
+            T = w.split("T=")[1].split(",")[0]
+            mode = "dense" if ", dense;" in w or w.rstrip().endswith("dense") else w.split("CAEE prune ")[1].split(";")[0]
+            print(f"| {e['world']} | {T} | {mode} | {e['n_keep']}/{e['n_act']} | {e['max_ms_dense']:.3f} → {e['max_ms_pruned']:.3f} | {e['max_ratio']:.3f} | "
+                  f"{e['sum_ms_dense']:.3f} → {e['sum_ms_pruned']:.3f} | {e['sum_ratio']:.3f} | {e['F_cost_ratio']:.3f} | "
+                  + " ".join(f"{v:.3f}" for v in e["slice_ms_pruned"]) + " | " + " ".join(f"{v:.0f}" for v in e["modelled_load_pruned_pct"]) + " |")
+        return
     print("| workload | T | mode | step us | w/o events us | dense us | kernel us | rate | frac of measured peak | experts run | launches / K steps | clocks MHz, reasons |")
     print("|---|---|---|---|---|---|---|---|---|---|---|---|")
     for d in lines:
