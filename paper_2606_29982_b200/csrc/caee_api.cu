@@ -174,6 +174,7 @@ caee_status create_impl(caee_ctx* c) {
   const caee_layer_desc& d = c->d;
   const size_t Tm = d.max_tokens, E = d.E, k = d.k, S = d.S;
   caee_status rc;
+  if (const char* v = getenv("CAEE_ROUTER_SMALL_WAVES")) c->router_small_waves = std::max(1, std::min(4, atoi(v)));   // tuning aid
   if (const char* v = getenv("CAEE_ROUTER_MMA_MIN_TOKENS")) c->router_mma_min_tokens = std::max(1, atoi(v));   // tuning aid
   if (caee_router_mma_supported(c) && d.max_tokens >= c->router_mma_min_tokens) {
     if ((rc = dev_alloc(c, &c->wr_img, caee_router_mma_image_bytes(c))) != CAEE_OK) return rc;
@@ -633,11 +634,13 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   // e4m3 decode steps: the split of x into its two e4m3 terms depends on x alone, so it goes first and
   // the chain router GEMM -> decision kernel -> expert kernel stays free for programmatic dependent launches
   const bool early_prep = c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && c->wl.run_cap != CAEE_RUN_TOKENS_WIDE;
-  if (early_prep) caee_launch_umma_prepare(c, x, T, st);
+  // ... and in steps of <= 16 tokens the one-CTA decision kernel does the split itself, ahead of its wait for the router
+  const bool split_in_decide = early_prep && fused && caee_decide_splits_x(c, T);
+  if (early_prep && !split_in_decide) caee_launch_umma_prepare(c, x, T, st);
   if (fused) {
     // decode-size step: router GEMM, then ONE kernel for S1-S6 + stats (decide.cu)
     if (!scores && (rc = caee_launch_router_logits(c, x, T, st)) != CAEE_OK) return rc;
-    CAEE_CUDA(c, caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st));
+    CAEE_CUDA(c, caee_launch_decide(c, scores, T, p, c->any_offload ? nullptr : stats, st, split_in_decide ? x : nullptr));
     if ((rc = after_launch(c, "decision kernel")) != CAEE_OK) return rc;
   } else {
     rc = enqueue_decisions(c, x, scores, T, p, c->idx, c->gate, nullptr, true, st);

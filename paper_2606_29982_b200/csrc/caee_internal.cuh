@@ -130,6 +130,7 @@ struct caee_ctx {
   std::vector<const float*> sg_h, su_h, sd_h;
   caee_packed packed;
 
+  int router_small_waves = 1;       // CTAs per SM of the GEMV-shaped router (steps of <= 4 tokens); env CAEE_ROUTER_SMALL_WAVES
   uint8_t* wr_img = nullptr;        // three bf16 terms of W_r as MMA stage images (router_mma.cu); NULL: shape not supported
   int router_mma_min_tokens = 64;   // steps of at least this many tokens take the tensor-core router (env CAEE_ROUTER_MMA_MIN_TOKENS;
                                     // measured on C3: T=32 +-0, T=64 -4 us, T=128 -17 us, T=256 -42 us, T=4096 -440 us per step)
@@ -244,8 +245,9 @@ void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* s
 // decide.cu
 bool caee_decide_fits(const caee_ctx* c, int T);
 size_t caee_decide_scratch_bytes(const caee_ctx* c);
+bool caee_decide_splits_x(const caee_ctx* c, int T);   // the one-CTA decision kernel also does the e4m3 decode kernel's x split
 cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* p, caee_fwd_stats* stats,
-                               cudaStream_t s);
+                               cudaStream_t s, const void* x_split = nullptr);
 // prune.cu
 void caee_launch_prune(caee_ctx* c, int mode, int flags, double theta, double eps, int T, const int32_t* idx,
                        const float* gate, cudaStream_t s);

@@ -21,6 +21,7 @@
 // (prefill) use the stand-alone kernels.
 #include <cooperative_groups.h>
 
+#include "act_split_dev.cuh"
 #include "caee_internal.cuh"
 #include "prune_dev.cuh"
 #include "warp_select.cuh"
@@ -71,6 +72,12 @@ struct DecideParams {
   unsigned char* acc_must;    // [E]
   uint32_t* M;                // [E, kWords]
   int* bar;                   // [4]: barrier 1, barrier 2, exit ticket
+  // e4m3 decode steps of <= 16 tokens: the one-CTA kernel also splits x into its two e4m3 terms (expert_fp8.cu),
+  // before it waits for the router GEMM — the split depends on x alone, so its launch and its time disappear
+  const __nv_bfloat16* split_x;   // NULL: not this step
+  uint8_t *split_hi, *split_lo;
+  float* split_scale;
+  int split_blocks;               // T * H / 128
 };
 
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
@@ -125,6 +132,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_decide(const DecideParams p) {
   if (p.has_prune && p.fast) caee_prune_preload(sm, E, p.D, p.w_eff, p.part, p.pl_experts, p.pl_start);
   if (kSingle) {
     for (int e = tid; e < E; e += kThreads) { sm.I[e] = 0; sm.act[e] = 0; sm.must[e] = 0; s_M[e] = 0; }
+    if (p.split_x)
+      for (int b = warp; b < p.split_blocks; b += kWarps) caee_act_split_block(p.split_x, p.split_hi, p.split_lo, p.split_scale, (size_t)b, lane);
     __syncthreads();
   }
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -240,8 +249,12 @@ size_t caee_decide_scratch_bytes(const caee_ctx* c) {
   return E * 8 + E + E + 16 /* align */ + E * kWords * 4 + 64;
 }
 
+bool caee_decide_splits_x(const caee_ctx* c, int T) {
+  return T <= kWarps && c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && c->xq != nullptr && c->d.H % 128 == 0;
+}
+
 cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const caee_prune_params* pp, caee_fwd_stats* stats,
-                               cudaStream_t st) {
+                               cudaStream_t st, const void* x_split) {
   const caee_layer_desc& d = c->d;
   DecideParams p;
   p.logits = scores_in ? nullptr : c->partial;
@@ -265,6 +278,12 @@ cudaError_t caee_launch_decide(caee_ctx* c, const float* scores_in, int T, const
   p.M = reinterpret_cast<uint32_t*>(z + m_off);
   p.bar = reinterpret_cast<int*>(z + m_off + E * kWords * 4);
   p.pl_experts = c->pl_experts; p.pl_start = c->pl_start; p.fast = c->part_max <= 32;
+  p.split_x = nullptr; p.split_hi = p.split_lo = nullptr; p.split_scale = nullptr; p.split_blocks = 0;
+  if (x_split && caee_decide_splits_x(c, T)) {
+    p.split_x = (const __nv_bfloat16*)x_split;
+    p.split_hi = c->xq; p.split_lo = c->xq + (size_t)d.max_tokens * d.H; p.split_scale = c->xs;
+    p.split_blocks = T * (d.H / 128);
+  }
   const int nv = caee_ceil_div(d.E, 32);
   void* args[] = {&p};
   ++c->n_launches;

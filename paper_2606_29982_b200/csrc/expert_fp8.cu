@@ -30,6 +30,7 @@
 #include <cstring>
 
 #include "umma_common.cuh"
+#include "act_split_dev.cuh"
 
 namespace {
 
@@ -62,47 +63,16 @@ struct Fp8Params {
   KSplit ksp;               // split k range of phase-1 tiles in steps of a few tokens (umma_common.cuh)
 };
 
-// two floats -> two e4m3 codes (low byte = a), round to nearest even, saturating
-__device__ __forceinline__ uint16_t cvt_e4m3x2(float a, float b) {
-  uint16_t r;
-  asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(b), "f"(a));
-  return r;
-}
-// two e4m3 codes -> two floats (exact)
-__device__ __forceinline__ float2 e4m3x2_to_float2(uint16_t v) {
-  uint32_t h2;
-  asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(v));
-  return __half22float2(*reinterpret_cast<__half2*>(&h2));
-}
-// a/s as hi + lo (both e4m3), for a pair of values
-__device__ __forceinline__ void split_pair(float a, float b, float inv_s, uint16_t& hi, uint16_t& lo) {
-  const float va = a * inv_s, vb = b * inv_s;
-  hi = cvt_e4m3x2(va, vb);
-  const float2 h = e4m3x2_to_float2(hi);
-  lo = cvt_e4m3x2(va - h.x, vb - h.y);
-}
+__device__ __forceinline__ uint16_t cvt_e4m3x2(float a, float b) { return caee_cvt_e4m3x2(a, b); }
+__device__ __forceinline__ float2 e4m3x2_to_float2(uint16_t v) { return caee_e4m3x2_to_float2(v); }
 
-// Once per step: x[T,H] bf16 -> hi/lo e4m3 terms and the (token, 128-block) scales.
-// One warp per block of 128 elements, 4 per lane.
+// Once per step: x[T,H] bf16 -> hi/lo e4m3 terms and the (token, 128-block) scales (act_split_dev.cuh).
+// One warp per block of 128 elements.  (Steps of <= 16 tokens: the decision kernel does this itself.)
 __global__ void __launch_bounds__(256) k_act_split(const __nv_bfloat16* __restrict__ x, uint8_t* __restrict__ hi,
                                                    uint8_t* __restrict__ lo, float* __restrict__ scale, size_t n_blocks) {
   const size_t b = (size_t)blockIdx.x * 8 + (threadIdx.x >> 5);
-  const int lane = threadIdx.x & 31;
   if (b >= n_blocks) return;
-  const uint2 u = *reinterpret_cast<const uint2*>(x + b * 128 + lane * 4);
-  const float v0 = __uint_as_float(u.x << 16), v1 = __uint_as_float(u.x & 0xffff0000u);
-  const float v2 = __uint_as_float(u.y << 16), v3 = __uint_as_float(u.y & 0xffff0000u);
-  float m = fmaxf(fmaxf(fabsf(v0), fabsf(v1)), fmaxf(fabsf(v2), fabsf(v3)));
-#pragma unroll
-  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  const float s = m > 0.f ? m * (1.0f / 448.0f) : 1.0f;
-  const float inv = 1.0f / s;
-  uint16_t h01, l01, h23, l23;
-  split_pair(v0, v1, inv, h01, l01);
-  split_pair(v2, v3, inv, h23, l23);
-  *reinterpret_cast<uint32_t*>(hi + b * 128 + lane * 4) = (uint32_t)h01 | ((uint32_t)h23 << 16);
-  *reinterpret_cast<uint32_t*>(lo + b * 128 + lane * 4) = (uint32_t)l01 | ((uint32_t)l23 << 16);
-  if (lane == 0) scale[b] = s;
+  caee_act_split_block(x, hi, lo, scale, b, threadIdx.x & 31);
 }
 
 // One thread per 16 codes: raw row-major [rows, cols] e4m3 -> stage images.

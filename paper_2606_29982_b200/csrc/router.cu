@@ -268,7 +268,7 @@ void caee_router_shape(const caee_ctx* c, int T, int* tt, int* ksplit, int* hs) 
   const bool small = T <= 4;
   *tt = small ? (T <= 1 ? 1 : (T <= 2 ? 2 : 4)) : (T <= 16 ? 16 : (T >= 1024 ? 64 : 32));   // prefill-size steps: 4 x 4 outputs per thread
   const int tiles = small ? caee_ceil_div(d.E, SE) : caee_ceil_div(d.E, TE) * caee_ceil_div(T, *tt);
-  const int want = caee_ceil_div((T <= 256 ? 1 : 2) * c->num_sms, tiles);
+  const int want = caee_ceil_div((small ? c->router_small_waves : (T <= 256 ? 1 : 2)) * c->num_sms, tiles);
   const int maxk = d.H / 128 > 0 ? d.H / 128 : 1;
   int ks = want < 1 ? 1 : (want > maxk ? maxk : want);
   const int kc = small ? SKC : KC;
