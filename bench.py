@@ -373,7 +373,7 @@ def run_caee(args, cfg, prune, eps):
                 "call": "caee_moe_forward_host: x from pinned host memory, y back to it, every step; copies double-buffered on two side streams",
                 "ms_per_step": ms_e2e},
         "gpu_launches": gpu_launches,
-        "roofline": {"bound": "hbm", "kernel": "k_expert_fp8" if fp8 else "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": ("k_expert_fp8_ts" if T > 128 else "k_expert_fp8") if fp8 else "k_expert_umma", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if achieved else None, "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": peak_src,
                      "bytes_per_launch": bytes_per_launch, "kernel_ms": k_ms,
@@ -405,12 +405,12 @@ def run_caee(args, cfg, prune, eps):
                            "peak_source": "caee_calibrate_cost H2D tier, measured in this run",
                            "bytes_per_launch": h2d, "kernel_ms": copy_ms}
     if fp8 and T > 256:
-        # prefill-size e4m3 step: k_expert_fp8_wide (fp16 MMAs) is bound by the tensor pipe / its
-        # shared-memory operand feed, not by HBM: report useful flops against the 16-bit tensor peak
+        # prefill-size e4m3 step: k_expert_fp8_ts (fp16 MMAs, weights widened into tensor memory) is bound by the tensor
+        # pipe and the board's power cap, not by HBM: report useful flops against the 16-bit tensor peak
         tpeak, tsrc = tensor_peak()
         flops = 6.0 * cfg.H * cfg.I * T * (cfg.k + cfg.S)      # every token keeps k routed slots + S shared
         tf = flops / (k_ms * 1e-3) / 1e12 if k_ms else None
-        out["roofline"].update({"bound": "tensor", "kernel": "k_expert_fp8_wide", "achieved": tf, "peak": tpeak,
+        out["roofline"].update({"bound": "tensor", "kernel": "k_expert_fp8_ts", "achieved": tf, "peak": tpeak,
                                 "unit": "TFLOP/s", "frac": tf / tpeak if tf else None, "peak_source": tsrc,
                                 "flops_per_launch": flops, "hbm_gbs": achieved})
         out["roofline"].pop("frac_of_8TBps_nominal", None)

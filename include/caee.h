@@ -193,10 +193,11 @@ caee_status caee_set_router(caee_ctx* ctx, const float* W_r, const float* b_logi
  * device memory.  The e4m3 UMMA kernel feeds the e4m3 codes to the tensor cores as they are and
  * carries each activation (x and the SwiGLU intermediate) as two e4m3 terms with one fp32 scale per
  * (token, 128-wide block): about 2^-8 relative error per activation, fp32 accumulation, the
- * 128x128 weight block scales applied in fp32.  Steps of more than 256 tokens take the e4m3
- * prefill kernel instead: weights widened to fp16 with the block scale folded in (one rounding
- * to 11 bits), x and the SwiGLU intermediate as fp16 (x exact for 6.1e-5 <= |x| <= 65504,
- * clamped above), fp32 accumulation over the whole k range.
+ * 128x128 weight block scales applied in fp32.  Steps of more than 128 tokens take the e4m3
+ * converter kernel instead: weights widened to fp16 with the block scale folded in (one rounding
+ * to 11 bits) and fed to the tensor cores from tensor memory, x and the SwiGLU intermediate as
+ * fp16 (x exact for 6.1e-5 <= |x| <= 65504, clamped above; h clamped likewise), fp32 accumulation
+ * over the whole k range.
  * Call caee_set_residency first when some experts live in host memory (changing the
  * residency afterwards invalidates the weights: set them again). */
 caee_status caee_set_weights(caee_ctx* ctx, const caee_expert_weights* w, int32_t pack);

@@ -28,7 +28,8 @@
 #define CAEE_RUN_TOKENS 128 /* most tokens per run: one UMMA N tile */
 #define CAEE_RUN_TOKENS_MIN 64
 #define CAEE_RUN_TOKENS_WIDE 256 /* e4m3 prefill kernel (expert_fp8_wide.cu): one N = 256 UMMA tile */
-#define CAEE_FP8_WIDE_MIN_TOKENS 257 /* steps of at least this many tokens take the e4m3 prefill kernel */
+#define CAEE_FP8_WIDE_MIN_TOKENS 129 /* e4m3 steps of at least this many tokens take the converter kernels (expert_fp8_ts.cu / _wide.cu):
+                                        measured on C4 against the decode kernel, T=192 -6%, T=256 -7%, T=128 +4% (the x gather) */
 #define CAEE_STAGE_RING 8  /* staging slots of the static offload path */
 #define CAEE_FETCH_GROUP 4 /* fetched experts per expert-kernel launch */
 #define CAEE_EP_MAX 8 /* most devices of an expert-parallel group (one NVSwitch domain) */
@@ -162,6 +163,8 @@ struct caee_ctx {
   unsigned attr_done = 0;            // bit i: this context's device has kernel i's MaxDynamicSharedMemorySize (a per-device attribute)
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
   bool pdl = true;                   // programmatic dependent launches on the decode path (env CAEE_NO_PDL=1 switches them off)
+  int step_prefill = 0;              // this step's e4m3 expert kernel: 0 decode (expert_fp8.cu), 1 expert_fp8_wide.cu, 2 expert_fp8_ts.cu
+  bool fp8_ts = true;                // prefill-size e4m3 steps take the A-from-TMEM kernel (expert_fp8_ts.cu); env CAEE_FP8_TS=0: expert_fp8_wide.cu
   bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
   float* ks_part = nullptr;          // UMMA decode kernels: partial sums of split phase-1 tiles (KSplit, umma_common.cuh)
   int32_t* ks_cnt = nullptr;         //   and their per-tile counters (zero between steps)
@@ -280,6 +283,8 @@ bool caee_fp8_wide_supported(const caee_ctx* c);
 size_t caee_fp8_wide_xg_bytes(const caee_ctx* c);
 void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t s);
 void caee_launch_expert_fp8_wide(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
+// expert_fp8_ts.cu
+void caee_launch_expert_fp8_ts(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t s);
 // cache.cu
 caee_status caee_cache_prepare_layer(caee_ctx* c, size_t slot_bytes);
 void caee_cache_detach(caee_ctx* c);

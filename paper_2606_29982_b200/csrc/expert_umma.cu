@@ -420,7 +420,7 @@ void caee_launch_pack_expert(caee_ctx* c, int e, uint8_t* dst, const void* g, co
 // Once per step, before the first expert launch (e4m3: x -> its two e4m3 terms, expert_fp8.cu).
 void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (c->d.w_dtype != CAEE_E4M3) return;
-  if (c->wl.run_cap == CAEE_RUN_TOKENS_WIDE) caee_launch_fp8_wide_prepare(c, x, T, st);
+  if (c->step_prefill) caee_launch_fp8_wide_prepare(c, x, T, st);
   else caee_launch_fp8_prepare(c, x, T, st);
 }
 
@@ -429,7 +429,8 @@ void caee_launch_umma_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st
 caee_status caee_launch_expert_umma(caee_ctx* c, const void* x, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
   const caee_layer_desc& d = c->d;
   if (d.w_dtype == CAEE_E4M3) {
-    if (c->wl.run_cap == CAEE_RUN_TOKENS_WIDE) caee_launch_expert_fp8_wide(c, T, run_begin, run_count, ticket, st);
+    if (c->step_prefill == 2) caee_launch_expert_fp8_ts(c, T, run_begin, run_count, ticket, st);
+    else if (c->step_prefill == 1) caee_launch_expert_fp8_wide(c, T, run_begin, run_count, ticket, st);
     else caee_launch_expert_fp8(c, T, run_begin, run_count, ticket, st);
     return CAEE_OK;
   }

@@ -505,12 +505,14 @@ def test_forward_small_fp8(H, kernel):
         L.close()
 
 
-@pytest.mark.parametrize("T", [24, 300])
-def test_forward_fp8_uneven_block_scales(H, T):
+@pytest.mark.parametrize("T,ts", [(24, 1), (130, 1), (300, 1), (300, 0)])
+def test_forward_fp8_uneven_block_scales(H, T, ts, monkeypatch):
     """Block scales spread over three decades inside one tile row: the per-block promotion of the
-    decode kernel (T = 24) and the scale x 2^J folding into fp16 weights of the prefill kernel
-    (T = 300) must still match the oracle's exact dequantisation."""
+    decode kernel (T = 24) and the scale x 2^J folding into fp16 weights of the converter kernels
+    (T >= 129: expert_fp8_ts.cu, A operand from tensor memory; ts = 0: expert_fp8_wide.cu, through shared
+    memory) must still match the oracle's exact dequantisation."""
     from paper_2606_29982_b200 import binding as B
+    monkeypatch.setenv("CAEE_FP8_TS", str(ts))
     cfg = C4S
     L = _layer(H, cfg, max_tokens=max(32, T), kernel=B.CAEE_KERNEL_UMMA)
     try:
@@ -669,19 +671,20 @@ def test_forward_c4_full_size_sampled(H, T, mode):
         L.close()
 
 
-@pytest.mark.parametrize("pairs", [0, 1])
-def test_forward_c4_prefill_4096_sampled(H, pairs, monkeypatch):
-    """pairs = 1: the same kernel on CTA pairs (cta_group::2 MMAs of M = 256, static tile schedule).
-    Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill,
-    256-token runs, the e4m3 prefill kernel expert_fp8_wide.cu): K_final and F_* for all 4096 tokens
-    bit-exact, y on sampled tokens."""
+@pytest.mark.parametrize("pairs,ts", [(0, 1), (0, 0), (1, 0)])
+def test_forward_c4_prefill_4096_sampled(H, pairs, ts, monkeypatch):
+    """Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill): K_final and
+    F_* for all 4096 tokens bit-exact, y on sampled tokens.  ts = 1: the default kernel, expert_fp8_ts.cu (128-token
+    runs, widened weights in tensor memory); ts = 0: expert_fp8_wide.cu (256-token runs, widened weights in shared
+    memory), alone or — pairs = 1 — on CTA pairs (cta_group::2 MMAs of M = 256, static tile schedule)."""
     monkeypatch.setenv("CAEE_FP8_WIDE_PAIRS", str(pairs))
+    monkeypatch.setenv("CAEE_FP8_TS", str(ts))
     L = H.GpuLayer(wl.C4, seed=0, max_tokens=4096, keep_raw=False)
     try:
         T = 4096
         # 64 tokens at a stride of 65: they sit in different 16-column groups of their 256-token runs and
         # touch several hundred (expert, run) pairs
-        r = _forward_case(H, L, T, "frac", tokens=_spread(T, 64 if pairs == 0 else 16), seed=100, chunk=8)
+        r = _forward_case(H, L, T, "frac", tokens=_spread(T, 64 if (pairs == 0 and ts == 1) else 16), seed=100, chunk=8)
         print(f"C4 T={T} frac: max|err|/RMS = {r:.3e}")
     finally:
         L.close()
