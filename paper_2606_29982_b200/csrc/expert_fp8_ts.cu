@@ -43,7 +43,6 @@ using namespace caee_umma;
 
 constexpr int kThreads = 640;
 constexpr int kKRaw = 128;                 // k per packed stage = one block-scale block
-constexpr int kKSub = 64;                  // k per converted / token stage
 constexpr int kAStagesT = 2, kTokStages = 4;                    // both rings in 128-k stages: one hand-over per block-scale block
 constexpr int kRunTokens = CAEE_RUN_TOKENS;                     // 128
 constexpr int kTokBytes = kRunTokens * kKRaw * 2;               // 32 KB: two 64-k images of 128 rows x 128 bytes
@@ -83,11 +82,6 @@ __device__ __forceinline__ void widen16_ts(const uint4 v, const __half2 s2, uint
     o[2 * i + 1] = *reinterpret_cast<const uint32_t*>(&p1);
   }
 }
-__device__ __forceinline__ uint4 ldg_stream(const uint8_t* p) {
-  uint4 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-  return v;
-}
 // 32 consecutive 32-bit columns of this thread's TMEM lane
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
   asm volatile(
@@ -113,7 +107,7 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, ui
 #ifdef CAEE_WIDE_STATS
 #define WAIT_T(acc, ...) do { long long _t0 = clock64(); __VA_ARGS__; acc += clock64() - _t0; } while (0)
 #else
-#define WAIT_T(acc, ...) do { __VA_ARGS__; } while (0)
+#define WAIT_T(acc, ...) do { __VA_ARGS__; } while (0)      /* acc is not even named in the product build */
 #endif
 
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_constant__ TsParams p) {
@@ -164,9 +158,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_cons
   const uint32_t tmem_base = tmem_base_s;
   TileQueue tq{qfull0, qempty0, tq_slots, 0, 0};
   Tile t;
-  long long w_a = 0, w_b = 0, w_c = 0, w_d = 0;   // wait cycles (CAEE_WIDE_STATS builds print them)
+#ifdef CAEE_WIDE_STATS
+  long long w_a = 0, w_b = 0, w_c = 0, w_d = 0;   // wait cycles of this thread, printed at the end
   const long long t_start = clock64();
-  (void)t_start; (void)w_a; (void)w_b; (void)w_c; (void)w_d;
+#endif
 
   if (warp == 0) {
     // ===== tile claimer and weight producer: one atomic ticket per tile, broadcast through the shared-memory queue;

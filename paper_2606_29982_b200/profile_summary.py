@@ -65,7 +65,7 @@ def git_head():
 
 # SASS mnemonics of the Blackwell tensor / TMEM / bulk-copy paths (B200_PROFILING.md) and what they are
 SASS_OPS = [("UTCHMMA", "tcgen05.mma kind::f16"), ("UTCQMMA", "tcgen05.mma kind::f8f6f4"), ("UTCBAR", "tcgen05.commit"),
-            ("LDTM", "tcgen05.ld (TMEM -> registers)"), ("UTCATOMSWS", "tcgen05.alloc / dealloc"),
+            ("LDTM", "tcgen05.ld (TMEM -> registers)"), ("STTM", "tcgen05.st (registers -> TMEM)"), ("UTCATOMSWS", "tcgen05.alloc / dealloc"),
             ("UBLKCP", "cp.async.bulk (bulk copy global -> shared)"), ("UTMALDG", "cp.async.bulk.tensor (TMA, incl. tile::gather4)"),
             ("SYNCS", "mbarrier ops"), ("HMMA", "mma.sync (legacy tensor path)"), ("ACQBULK", "griddepcontrol.wait"),
             ("ELECT", "elect.sync")]
