@@ -28,8 +28,11 @@
 //                 at no register cost, and shared memory has room here (80 KB of traffic per 64 k at N = 128)
 //   warps 8-15    converters: warp w owns TMEM lane quadrant w % 4 of tile half (w - 8) / 4; thread = one
 //                 weight row: 128 codes per 128-k stage shared -> registers -> fp16 -> 2 x tcgen05.st (A ring)
-//   warp 2        token-operand loader: one bulk copy per 64-k stage from the run's stage image (tok ring,
-//                 8 x 16 KB; x images by k_gather_x, h images by the phase-1 epilogue: expert_fp8_wide.cu)
+//   warp 2        token-operand loader: one bulk copy per 128-k stage from the run's stage image (tok ring,
+//                 4 x 32 KB; x images by k_gather_x, h images by the phase-1 epilogue: expert_fp8_wide.cu).
+//                 (Tried: writing the x images inside this kernel with the idle warp 3 of every CTA, row b of every
+//                 run by CTA b, phase-1 tiles waiting on a per-run counter — parity green, but one warp per SM moves a
+//                 14 KB row in ~20 us and the step went from 3.55 to 8.45 ms; k_gather_x stays.)
 //   warp 1        MMA issuer: 16 tcgen05.mma (A from TMEM, M 128, N = padded tokens, K 16) per 128-k stage
 //   warps 4-7, 16-19   epilogue: TMEM -> SwiGLU -> h (fp16 stage image), or -> o rows (fp32)
 #include <cstdio>
