@@ -196,6 +196,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_cons
     const uint32_t d0 = tmem_base, d1 = tmem_base + kAccCols;
     for (int it = 0; tm.at(tq.pop(), t); ++it) {
       const int npad = (__shfl_sync(0xffffffffu, p.wl.run_n[t.run], 0) + 15) & ~15;
+      CAEE_DEV_ASSERT(npad >= 16 && npad <= kRunTokens && p.wl.run_hrow[t.run] + npad <= p.wl.hrow_cap);
       const uint32_t idesc = (1u << 4) | ((uint32_t)(npad >> 3) << 17) | ((uint32_t)(kTileRows >> 4) << 24);   // fp16 x fp16 -> fp32
       const int nkb = t.phase == 1 ? p.KB1 : p.KB2;
       const uint32_t sub_bytes = (uint32_t)npad * 128u;       // one 64-k image of the run inside a token stage
