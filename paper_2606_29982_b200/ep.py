@@ -54,9 +54,16 @@ def gather_tokens(x_local, T, group=None):
     assert x_local.shape[0] == hi - lo, (x_local.shape, lo, hi)
     pad = torch.zeros((per,) + tuple(x_local.shape[1:]), dtype=x_local.dtype, device=x_local.device)
     pad[: hi - lo] = x_local
-    out = torch.empty((world * per,) + tuple(x_local.shape[1:]), dtype=x_local.dtype, device=x_local.device)
-    dist.all_gather_into_tensor(out, pad, group=group) if x_local.is_cuda else dist.all_gather(list(out.split(per)), pad, group=group)
-    return out[:T]
+    if x_local.is_cuda and dist.get_backend(group) == "nccl":
+        out = torch.empty((world * per,) + tuple(x_local.shape[1:]), dtype=x_local.dtype, device=x_local.device)
+        dist.all_gather_into_tensor(out, pad, group=group)
+        return out[:T]
+    # gloo (CPU tensors, or CUDA tensors staged through the host: gloo gathers host memory only)
+    host = pad.cpu().contiguous().view(torch.uint8)      # gloo knows few element types: bytes always work
+    parts = [torch.empty_like(host) for _ in range(world)]
+    dist.all_gather(parts, host, group=group)
+    out = torch.cat(parts).view(x_local.dtype)[:T]
+    return out.to(x_local.device)
 
 
 def exchange_bytes(payload: bytes, group=None):
@@ -89,11 +96,20 @@ class EpGroup:
         if y is None:
             y = torch.empty_like(x)
         B.caee_moe_forward(self.ctx, x, T, params, None, stats)
-        dist.barrier(group=self.group)        # every rank's expert kernel (and its peer stores) is complete
+        self._group_barrier()                 # every rank's expert kernel (and its peer stores) is complete
         B.caee_ep_combine(self.ctx, T, y)
-        dist.barrier(group=self.group)        # nobody overwrites a peer's o rows before they are combined
+        self._group_barrier()                 # nobody overwrites a peer's o rows before they are combined
         lo, hi = home_range(T, self.rank, self.world)
         return y, (lo, hi)
+
+    def _group_barrier(self):
+        """All ranks' enqueued work is complete.  NCCL's barrier is ordered on the stream; any other backend synchronises
+        the device first and then meets on the host."""
+        if dist.get_backend(self.group) != "nccl":
+            torch.cuda.synchronize()
+        dist.barrier(group=self.group)
+        if dist.get_backend(self.group) == "nccl":
+            torch.cuda.synchronize()
 
     def close(self):
         for r, p in enumerate(self.peers):
