@@ -44,6 +44,8 @@ def _worker(rank, world, port, T, out):
     # 1. the ranks' own tokens -> the step's x, on every rank
     xg = ep.gather_tokens(torch.from_numpy(x[lo:hi].copy()), T).numpy()
     ok_gather = np.array_equal(xg, x)
+    xb = torch.from_numpy(x).to(torch.bfloat16)                       # the activation dtype of the UMMA paths
+    ok_gather = ok_gather and torch.equal(ep.gather_tokens(xb[lo:hi].contiguous(), T), xb)
     # the handle exchange used for the o buffers
     hs = ep.exchange_bytes(bytes([rank]) * 64)
     ok_handles = [h[0] for h in hs] == list(range(world)) and all(len(h) == 64 for h in hs)
