@@ -317,10 +317,13 @@ def test_forward_small_bf16(H, cfg, kernel):
         L.close()
 
 
-def test_forward_hot_expert_spans_several_runs(H):
-    """All tokens on the same experts: one expert gets T > 128 tokens (two runs, ragged tail)."""
+@pytest.mark.parametrize("fp8", [False, True])
+def test_forward_hot_expert_spans_several_runs(H, fp8):
+    """All tokens on the same experts: one expert gets T > 128 tokens (several runs, ragged tail).  fp8: the same on the
+    e4m3 layer, i.e. on the tensor-memory converter kernel (128-token runs: three runs per hot expert, one of 27 tokens;
+    a nearly idle expert with one 16-column tile; experts without tokens)."""
     from paper_2606_29982_b200 import binding as B
-    cfg = C2S
+    cfg = wl.scaled(C4S, name="C4-small-ungrouped", n_group=1, topk_group=1, k=3) if fp8 else C2S
     L = _layer(H, cfg, max_tokens=300, kernel=B.CAEE_KERNEL_UMMA)
     try:
         T = 283
