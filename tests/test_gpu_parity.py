@@ -756,10 +756,11 @@ def test_forward_is_cuda_graph_capturable(H):
 
 
 # ---------------------------------------------------------------- NEXT-2: expert parallelism
-@pytest.mark.parametrize("cfg_name,world,mode,scattered,partial", [
-    ("C1", 2, "rank", False, False), ("R1S", 2, "dense", False, True), ("R1S", 4, "thresh", True, True),
-    ("C2S", 4, "cir", False, False), ("C4S", 2, "frac", True, True), ("R1S", 8, "cir", False, True)])
-def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered, partial):
+@pytest.mark.parametrize("cfg_name,world,mode,scattered,partial,T", [
+    ("C1", 2, "rank", False, False, 16), ("R1S", 2, "dense", False, True, 29), ("R1S", 4, "thresh", True, True, 29),
+    ("C2S", 4, "cir", False, False, 29), ("C4S", 2, "frac", True, True, 29), ("R1S", 8, "cir", False, True, 29),
+    ("C4S", 4, "cir", False, True, 300), ("R1S", 2, "thresh", True, False, 300)])
+def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered, partial, T):
     """`world` contexts in one process stand for the ranks of an expert-parallel group: each owns a
     subset of the experts and runs ITS slice of the step (the runs of its experts, the shared experts of its
     home tokens), storing every o row into the home rank's o buffer (here: plain pointers instead of IPC
@@ -771,14 +772,14 @@ def test_expert_parallel_ranks_on_one_gpu(H, cfg_name, world, mode, scattered, p
     from paper_2606_29982_b200 import binding as B
     from paper_2606_29982_b200 import ep
     cfg = {"C1": wl.C1, "R1S": R1S, "C2S": C2S, "C4S": C4S}[cfg_name]
-    T = 29 if cfg_name != "C1" else 16
+    mt = max(32, T)          # T = 300: the prefill-size paths (stand-alone decision kernels, tensor-core router, e4m3 converter kernel)
     rng = np.random.default_rng(5)
     owner = rng.integers(0, world, size=cfg.E).astype(np.int32) if scattered else ep.owner_table(cfg.E, world)
-    single = _layer(H, cfg, max_tokens=32)
+    single = _layer(H, cfg, max_tokens=mt)
     if partial:      # the peers' buffers do not exist yet: the rank's own buffer stands in until they do
-        ranks = [_layer(H, cfg, max_tokens=32, ep=(r, world, owner, lambda ctx: [B.caee_ep_obuf(ctx)[0]] * world)) for r in range(world)]
+        ranks = [_layer(H, cfg, max_tokens=mt, ep=(r, world, owner, lambda ctx: [B.caee_ep_obuf(ctx)[0]] * world)) for r in range(world)]
     else:
-        ranks = [_layer(H, cfg, max_tokens=32) for _ in range(world)]
+        ranks = [_layer(H, cfg, max_tokens=mt) for _ in range(world)]
     try:
         peers = [B.caee_ep_obuf(L.ctx)[0] for L in ranks]
         for r, L in enumerate(ranks):
