@@ -404,16 +404,20 @@ def run_caee(args, cfg, prune, eps):
                            "achieved": gbs, "peak": calib["h2d_gbs"], "unit": "GB/s", "frac": gbs / calib["h2d_gbs"] if gbs else None, "traffic": None,
                            "peak_source": "caee_calibrate_cost H2D tier, measured in this run",
                            "bytes_per_launch": h2d, "kernel_ms": copy_ms}
-    if fp8 and T > 256:
-        # prefill-size e4m3 step: k_expert_fp8_ts (fp16 MMAs, weights widened into tensor memory) is bound by the tensor
-        # pipe and the board's power cap, not by HBM: report useful flops against the 16-bit tensor peak
+    if fp8 and T > 128 and k_ms:
+        # e4m3 steps of more than 128 tokens run k_expert_fp8_ts (fp16 MMAs on weights widened into tensor memory).  Which
+        # roofline bounds the step follows from its arithmetic intensity: useful flops per weight byte streamed against the
+        # ridge point of this box (sustained 16-bit tensor rate / measured HBM rate); below it the HBM figures above stand
         tpeak, tsrc = tensor_peak()
         flops = 6.0 * cfg.H * cfg.I * T * (cfg.k + cfg.S)      # every token keeps k routed slots + S shared
-        tf = flops / (k_ms * 1e-3) / 1e12 if k_ms else None
-        out["roofline"].update({"bound": "tensor", "kernel": "k_expert_fp8_ts", "achieved": tf, "peak": tpeak,
-                                "unit": "TFLOP/s", "frac": tf / tpeak if tf else None, "peak_source": tsrc,
-                                "flops_per_launch": flops, "hbm_gbs": achieved})
-        out["roofline"].pop("frac_of_8TBps_nominal", None)
+        intensity = flops / bytes_per_launch if bytes_per_launch else 0.0
+        ridge = tpeak * 1e12 / (peak * 1e9)
+        out["roofline"].update({"flops_per_launch": flops, "flop_per_byte": intensity, "ridge_flop_per_byte": ridge})
+        if intensity > ridge:
+            tf = flops / (k_ms * 1e-3) / 1e12
+            out["roofline"].update({"bound": "tensor", "achieved": tf, "peak": tpeak, "unit": "TFLOP/s", "frac": tf / tpeak,
+                                    "peak_source": tsrc, "hbm_gbs": achieved})
+            out["roofline"].pop("frac_of_8TBps_nominal", None)
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores: the whole T-token layer step, a few repetitions
         o = OracleLayer(cfg, T, prune, eps, 0, dev, layer=L)
