@@ -613,7 +613,6 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   // decode steps (T <= 128) use 64-token runs: the smaller token operand leaves room for a deeper
   // weight ring (only the shared experts and the few hottest experts are split and streamed twice),
   // and the e4m3 kernel's hi/lo terms share one MMA (expert_fp8.cu); larger steps keep 128 for weight reuse
-  // e4m3 prefill-size steps: 256-token runs for the converter kernel (expert_fp8_wide.cu)
   c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
   // e4m3 prefill-size steps: the A-from-TMEM kernel on 128-token runs (expert_fp8_ts.cu), or the shared-memory converter
   // kernel on 256-token runs (expert_fp8_wide.cu; also for CTA pairs)

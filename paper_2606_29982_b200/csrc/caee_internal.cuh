@@ -157,7 +157,7 @@ struct caee_ctx {
   uint8_t* hq = nullptr;             // UMMA e4m3: hi | lo terms of h, [rows, I] each
   float* hs = nullptr;               //   and its scales [rows, I/128]
   alignas(64) unsigned char tm_x[128] = {0}, tm_h[128] = {0};  // CUtensorMap of xq / hq (row gathers), see expert_fp8.cu
-  uint8_t* xg = nullptr;             // e4m3 prefill kernel (expert_fp8_wide.cu): per-run stage images of the gathered x rows
+  uint8_t* xg = nullptr;             // e4m3 converter kernels (expert_fp8_ts.cu, expert_fp8_wide.cu): per-run stage images of the gathered x rows
   bool tm_ready = false;
   int wide_max_pairs = -1;           // co-resident CTA pairs of the e4m3 prefill kernel on this device (-1: not asked yet)
   unsigned attr_done = 0;            // bit i: this context's device has kernel i's MaxDynamicSharedMemorySize (a per-device attribute)

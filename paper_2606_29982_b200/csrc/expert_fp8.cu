@@ -111,8 +111,8 @@ __global__ void k_scale_table(const float* __restrict__ sg, const float* __restr
   }
 }
 
-// Per-expert power of two 2^J with max |scale| 2^J in [64, 128): the prefill kernel
-// (expert_fp8_wide.cu) folds scale 2^J into fp16 weights (|code| <= 448, so products stay below
+// Per-expert power of two 2^J with max |scale| 2^J in [64, 128): the converter kernels
+// (expert_fp8_ts.cu, expert_fp8_wide.cu) fold scale 2^J into fp16 weights (|code| <= 448, so products stay below
 // 65504) and multiplies its accumulators by 2^-J.  norm[0] = 2^J, norm[1] = 2^-J.
 __global__ void __launch_bounds__(256) k_scale_norm(const float* __restrict__ tab, int n, float* __restrict__ norm) {
   __shared__ float red[8];
