@@ -25,7 +25,7 @@
 // version of this kernel.  So both token operands are kept as per-run STAGE IMAGES: for run r
 // (rows padded to 16) stage s = the 64 k of every row, 128 bytes each, in 128-byte-swizzled
 // 8-row atoms — ONE contiguous bulk copy per stage.  x's images are written once per step by
-// k_gather_x (0.19 ms at 4096 tokens, bound by HBM writes: 0.59 GB); h's images are written in place by
+// k_gather_x (0.15 ms at 4096 tokens, bound by HBM writes: 0.5 GB at 3.2 TB/s, where a memset reaches 3.8); h's images are written in place by
 // the phase-1 epilogue.  (Round 2 tried to drop k_gather_x by gathering the x rows inside this kernel with
 // 16-byte cp.async copies from an fp16 copy of x — two loader warps, 2048 copies per stage, swizzled on the
 // way in, cp.async.mbarrier.arrive on the stage barrier: correct, but the expert kernel went from 4.15 to
@@ -490,34 +490,52 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_wide(const __grid_co
   }
 }
 
-// x rows of every run -> the run's token-operand stage images (fp16).  CTA (r, y): run r; eight
-// threads share a row (one 16-byte chunk of every 128-byte piece each) and walk its 64-k stages in
-// order, so a row's 2H bytes are read front to back; rows >= n are written as zeros.
+// bf16 pair -> fp16 pair, clamped to fp16's range
+__device__ __forceinline__ uint4 bf16x8_to_f16x8(uint4 v) {
+  uint32_t* w = reinterpret_cast<uint32_t*>(&v);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const float lo = __uint_as_float(w[q] << 16), hi = __uint_as_float(w[q] & 0xffff0000u);
+    const __half2 h2 = __floats2half2_rn(fminf(fmaxf(lo, -65504.f), 65504.f), fminf(fmaxf(hi, -65504.f), 65504.f));
+    w[q] = *reinterpret_cast<const uint32_t*>(&h2);
+  }
+  return v;
+}
+
+// x rows of every run -> the run's token-operand stage images (fp16).  CTA (r, y): run r, the y-th
+// share of its 64-k stages, ALL rows: eight threads share a row's 128-byte piece (one 16-byte chunk
+// each), the CTA covers 32 rows per pass, so a stage image (npad x 128 bytes) and the stages after it
+// are written front to back — one contiguous region per CTA; rows >= n are written as zeros.
+constexpr int kGatherY = 8, kGatherPass = CAEE_RUN_TOKENS_WIDE / 32;
 __global__ void __launch_bounds__(256) k_gather_x(caee_worklist wl, const uint4* __restrict__ x, uint8_t* __restrict__ xg, int H,
                                                   int n_runs_arg) {
   const int n_runs = n_runs_arg >= 0 ? n_runs_arg : wl.meta[1];
   const int run = blockIdx.x;
   if (run >= n_runs) return;
   const int n = wl.run_n[run], start = wl.run_start[run], npad = (n + 15) & ~15;
-  const int nsub = H / kKSub, j = threadIdx.x & 7;
+  const int nsub = H / kKSub, j = threadIdx.x & 7, r0 = threadIdx.x >> 3;
+  const int per = (nsub + gridDim.y - 1) / gridDim.y, s_lo = blockIdx.y * per, s_hi = min(nsub, s_lo + per);
   uint8_t* img = xg + (size_t)wl.run_hrow[run] * H * 2;
-  for (int rr = blockIdx.y * 32 + (threadIdx.x >> 3); rr < npad; rr += gridDim.y * 32) {
-    const uint4* src = rr < n ? x + (size_t)wl.ent_tok[start + rr] * (H / 8) + j : nullptr;
-    uint8_t* dst = img + (rr >> 3) * 1024 + (rr & 7) * 128 + ((j ^ (rr & 7)) << 4);
-    const size_t sstride = (size_t)npad * 128;
-#pragma unroll 4
-    for (int s = 0; s < nsub; ++s) {
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (src) v = __ldg(src + s * 8);
-      uint32_t* w = reinterpret_cast<uint32_t*>(&v);
+  const size_t sstride = (size_t)npad * 128;
+  const uint4* src[kGatherPass];
+  uint32_t doff[kGatherPass];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {   // bf16 pair -> fp16 pair, clamped to fp16's range
-        const float lo = __uint_as_float(w[q] << 16), hi = __uint_as_float(w[q] & 0xffff0000u);
-        const __half2 h2 = __floats2half2_rn(fminf(fmaxf(lo, -65504.f), 65504.f), fminf(fmaxf(hi, -65504.f), 65504.f));
-        w[q] = *reinterpret_cast<const uint32_t*>(&h2);
-      }
-      *reinterpret_cast<uint4*>(dst + s * sstride) = v;
+  for (int q = 0; q < kGatherPass; ++q) {
+    const int rr = q * 32 + r0;
+    src[q] = rr < n ? x + (size_t)wl.ent_tok[start + rr] * (H / 8) + j : nullptr;
+    doff[q] = (uint32_t)((rr >> 3) * 1024 + (rr & 7) * 128 + ((j ^ (rr & 7)) << 4));
+  }
+  const int npass = (npad + 31) >> 5;
+  for (int s = s_lo; s < s_hi; ++s) {
+    uint4 v[kGatherPass];
+#pragma unroll
+    for (int q = 0; q < kGatherPass; ++q) {
+      v[q] = make_uint4(0, 0, 0, 0);
+      if (q < npass && src[q]) v[q] = __ldg(src[q] + s * 8);
     }
+#pragma unroll
+    for (int q = 0; q < kGatherPass; ++q)
+      if (q < npass && q * 32 + r0 < npad) *reinterpret_cast<uint4*>(img + s * sstride + doff[q]) = bf16x8_to_f16x8(v[q]);
   }
 }
 
@@ -531,7 +549,7 @@ size_t caee_fp8_wide_xg_bytes(const caee_ctx* c) { return c->h_rows_cap * (size_
 void caee_launch_fp8_wide_prepare(caee_ctx* c, const void* x, int T, cudaStream_t st) {
   if (T <= 0) return;
   ++c->n_launches;
-  k_gather_x<<<dim3((unsigned)c->wl.max_runs, 8), 256, 0, st>>>(c->wl, (const uint4*)x, c->xg, c->d.H, -1);
+  k_gather_x<<<dim3((unsigned)c->wl.max_runs, kGatherY), 256, 0, st>>>(c->wl, (const uint4*)x, c->xg, c->d.H, -1);
 }
 
 // runs [run_begin, run_begin + run_count) (run_count < 0: every run of the work list), tile
