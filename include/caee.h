@@ -231,6 +231,31 @@ caee_status caee_get_cost_table(const caee_ctx* ctx, int64_t* ticks_resident, in
  * selection score; gate dev [T,k] fp32. */
 caee_status caee_route(caee_ctx* ctx, const void* x, int32_t T, float* scores, int32_t* idx, float* gate,
                        void* stream);
+/* caee_route WITHOUT a context and without any allocation (S0+S1): for callers that cannot call
+ * cudaMalloc — code under CUDA graph capture, tight serving loops, harnesses that forbid it.  caee_create allocates
+ * the router's split-K scratch (ks x T x E fp32 partial logits) with cudaMalloc; this call runs the same router GEMM
+ * (the fp32-FMA kernels of router.cu at every T: the tensor-core router needs a packed image of W_r) and the same
+ * top-k kernel with that scratch in ONE file-scope device array of CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS floats
+ * (2 MiB, held by every GPU that loads the library until the process exits).  It calls no cudaMalloc / cudaFree
+ * and no allocating library routine, only enqueues work on `stream`, and never synchronises.
+ *   device: CUDA ordinal, -1 = the current device.  x dev [T,H] act_dtype (CAEE_F32 or CAEE_BF16), Wr dev [E,H]
+ *   fp32, both 16-byte aligned; b_logit, corr_bias dev [E] fp32 or NULL; scores dev [T,E] fp32 or NULL; idx dev [T,k]
+ *   int32; gate dev [T,k] fp32.  H a positive multiple of 8; E, k, n_group, topk_group, score_fn, norm_topk as in
+ *   caee_layer_desc.  Results are bit-identical to caee_route on a context of the same shape while that one uses the
+ *   FMA router (T < 64); from 64 tokens on caee_route's tensor-core scores agree to 1e-5 relative.
+ * Limits: T <= CAEE_ROUTE_NOALLOC_MAX_TOKENS and ks * T * E <= CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS (ks = the split
+ * the router picks for T, at most H/128) — beyond either the call returns CAEE_ESHAPE and enqueues nothing;
+ * caee_last_error(NULL) gives the reason, as for caee_create.
+ * Sharing: every call on a device uses the same array, which keeps the last call's contents.  Nothing in it has to
+ * start at zero (the GEMM writes every partial the top-k kernel reads), but calls that OVERLAP on the GPU — two
+ * streams, or two host threads enqueueing on different streams — race on it: keep them on one stream or order them
+ * with events.  Contexts are not affected (they own their scratch). */
+#define CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS (1 << 19)
+#define CAEE_ROUTE_NOALLOC_MAX_TOKENS 128
+caee_status caee_route_noalloc(int32_t device, const void* x, int32_t act_dtype, const float* Wr, const float* b_logit,
+                               const float* corr_bias, int32_t T, int32_t H, int32_t E, int32_t k, int32_t n_group,
+                               int32_t topk_group, int32_t score_fn, int32_t norm_topk, float* scores, int32_t* idx,
+                               float* gate, void* stream);
 /* S1 only, on caller-supplied scores (parity entry point). */
 caee_status caee_route_from_scores(caee_ctx* ctx, const float* scores, int32_t T, int32_t* idx, float* gate,
                                    void* stream);

@@ -26,7 +26,7 @@ CAEE_KERNEL_AUTO, CAEE_KERNEL_SIMT, CAEE_KERNEL_UMMA = 0, 1, 2
 
 EXPORTS = ["caee_create", "caee_destroy", "caee_last_error", "caee_set_router", "caee_set_weights",
            "caee_set_partitions", "caee_set_residency", "caee_set_cost_table", "caee_calibrate_cost", "caee_calibrate_points",
-           "caee_get_cost_table", "caee_launch_count", "caee_route",
+           "caee_get_cost_table", "caee_launch_count", "caee_route", "caee_route_noalloc",
            "caee_route_from_scores", "caee_prune", "caee_moe_forward", "caee_moe_forward_from_scores",
            "caee_moe_forward_host", "caee_host_flush", "caee_last_routing", "caee_profile", "caee_profile_read", "caee_profile_read_offload", "caee_version",
            "caee_cache_create", "caee_cache_destroy", "caee_cache_attach", "caee_cache_read_stats", "caee_cache_snapshot",
@@ -96,6 +96,8 @@ _lib.caee_calibrate_points.argtypes = [_ctx_p, C.c_int32, C.c_int32, C.c_void_p,
 _lib.caee_get_cost_table.argtypes = [_ctx_p, C.c_void_p, C.c_void_p]
 _lib.caee_launch_count.argtypes = [_ctx_p, C.c_void_p]
 _lib.caee_route.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.caee_route_noalloc.argtypes = ([C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int32] * 8 +
+                                    [C.c_void_p] * 4)
 _lib.caee_route_from_scores.argtypes = [_ctx_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.caee_prune.argtypes = [_ctx_p, C.POINTER(caee_prune_params), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
                             C.POINTER(caee_prune_out), C.c_void_p]
@@ -232,6 +234,13 @@ def caee_launch_count(ctx):
 
 def caee_route(ctx, x, T, scores, idx, gate, stream=None):
     _check(_lib.caee_route(ctx, _ptr(x), int(T), _ptr(scores), _ptr(idx), _ptr(gate), _stream(stream)), ctx)
+
+
+def caee_route_noalloc(device, x, act_dtype, Wr, b_logit, corr_bias, T, H, E, k, n_group, topk_group, score_fn, norm_topk,
+                       scores, idx, gate, stream=None):
+    _check(_lib.caee_route_noalloc(int(device), _ptr(x), int(act_dtype), _ptr(Wr), _ptr(b_logit), _ptr(corr_bias), int(T), int(H),
+                                   int(E), int(k), int(n_group), int(topk_group), int(score_fn), int(norm_topk), _ptr(scores),
+                                   _ptr(idx), _ptr(gate), _stream(stream)))
 
 
 def caee_route_from_scores(ctx, scores, T, idx, gate, stream=None):

@@ -6,6 +6,9 @@
 //                    in ascending ks: deterministic scores, no reduction tail in this kernel
 //  k_route_topk    : one warp per token: activation, selection, gates (steps > 256 tokens and
 //                    caee_route; decode-size steps run the same code inside k_decide, decide.cu).
+#include <cstring>
+#include <mutex>
+
 #include "caee_internal.cuh"
 #include "warp_select.cuh"
 
@@ -293,4 +296,105 @@ void caee_launch_route_topk(caee_ctx* c, const float* scores_in, int T, float* s
   else if (nv <= 4) launch_topk<4>(c, scores_in, T, scores_out, idx, gate, st);
   else if (nv <= 8) launch_topk<8>(c, scores_in, T, scores_out, idx, gate, st);
   else launch_topk<16>(c, scores_in, T, scores_out, idx, gate, st);
+}
+
+// ------------------------------------------------------------------ caee_route_noalloc (include/caee.h)
+// The split-K scratch of the router GEMM for callers that cannot allocate: one file-scope device array per GPU that
+// loads the library.  In HOST code the name below is a host-side stand-in, not a device address: its device address
+// is taken once per device with cudaGetSymbolAddress (that device current) and passed to the kernels as `partial`.
+static __device__ __align__(256) float g_route_noalloc_partial[CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+struct NoAllocDevice {
+  float* partial = nullptr;   // device address of g_route_noalloc_partial on this device
+  int num_sms = 0;
+  bool ready = false;
+};
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mu;
+
+struct CurrentDevice {   // makes `dev` current for the scope
+  int prev = -1;
+  explicit CurrentDevice(int dev) {
+    cudaGetDevice(&prev);
+    if (prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~CurrentDevice() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+// set-up, once per device, with that device current; no allocation (the array came with the module)
+caee_status noalloc_device(int dev, NoAllocDevice* out) {
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  NoAllocDevice& nd = g_noalloc_dev[dev];
+  if (!nd.ready) {
+    int major = 0, sms = 0;
+    CAEE_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return caee_fail(nullptr, CAEE_EUNSUPPORTED, "caee_route_noalloc: device %d is not an sm_100 device", dev);
+    CAEE_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* ptr = nullptr;
+    CAEE_CUDA(nullptr, cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_route_noalloc_partial));
+    if (!ptr) return caee_fail(nullptr, CAEE_ECUDA, "caee_route_noalloc: cudaGetSymbolAddress returned NULL");
+    nd.partial = ptr;
+    nd.num_sms = sms;
+    nd.ready = true;
+  }
+  *out = nd;
+  return CAEE_OK;
+}
+
+}  // namespace
+
+caee_status caee_route_noalloc(int32_t device, const void* x, int32_t act_dtype, const float* Wr, const float* b_logit,
+                               const float* corr_bias, int32_t T, int32_t H, int32_t E, int32_t k, int32_t n_group,
+                               int32_t topk_group, int32_t score_fn, int32_t norm_topk, float* scores, int32_t* idx,
+                               float* gate, void* stream) {
+  const char* me = "caee_route_noalloc";
+  if (H < 8 || H % 8) return caee_fail(nullptr, CAEE_ESHAPE, "%s: H must be a positive multiple of 8", me);
+  if (E < 1 || E > CAEE_MAX_E) return caee_fail(nullptr, CAEE_EINVAL, "%s: E must be in 1..%d", me, CAEE_MAX_E);
+  if (k < 1 || k > E || k > 32) return caee_fail(nullptr, CAEE_EINVAL, "%s: k must be in 1..min(E,32)", me);
+  if (n_group < 1 || n_group > 32 || E % n_group) return caee_fail(nullptr, CAEE_EINVAL, "%s: n_group must divide E and be <= 32", me);
+  if (topk_group < 1 || topk_group > n_group) return caee_fail(nullptr, CAEE_EINVAL, "%s: topk_group must be in 1..n_group", me);
+  if ((long long)topk_group * (E / n_group) < k) return caee_fail(nullptr, CAEE_EINVAL, "%s: topk_group*(E/n_group) < k", me);
+  if (score_fn != CAEE_SCORE_SOFTMAX && score_fn != CAEE_SCORE_SIGMOID) return caee_fail(nullptr, CAEE_EINVAL, "%s: unknown score_fn", me);
+  if (act_dtype != CAEE_F32 && act_dtype != CAEE_BF16) return caee_fail(nullptr, CAEE_EDTYPE, "%s: act_dtype must be F32 or BF16", me);
+  if (T < 0) return caee_fail(nullptr, CAEE_EINVAL, "%s: T is negative", me);
+  if (T > CAEE_ROUTE_NOALLOC_MAX_TOKENS)
+    return caee_fail(nullptr, CAEE_ESHAPE, "%s: T=%d exceeds the no-allocation limit of %d tokens", me, T, CAEE_ROUTE_NOALLOC_MAX_TOKENS);
+  if (T == 0) return CAEE_OK;
+  if (!x || !Wr || !idx || !gate) return caee_fail(nullptr, CAEE_EINVAL, "%s: x, Wr, idx or gate is NULL", me);
+  if (((uintptr_t)x | (uintptr_t)Wr) & 15) return caee_fail(nullptr, CAEE_EINVAL, "%s: x and Wr must be 16-byte aligned", me);
+  int dev = device;
+  if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return caee_fail(nullptr, CAEE_ECUDA, "%s: no current device", me);
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return caee_fail(nullptr, CAEE_EINVAL, "%s: device %d out of range", me, dev);
+  CurrentDevice cur(dev);
+  NoAllocDevice nd;
+  caee_status rc = noalloc_device(dev, &nd);
+  if (rc != CAEE_OK) return rc;
+
+  // a host-only stand-in for the context the launchers read their shapes and pointers from (nothing is allocated;
+  // wr_img stays NULL, so caee_router_shape picks the FMA kernels at every T)
+  caee_ctx view;
+  memset(&view.d, 0, sizeof view.d);
+  view.d.H = H; view.d.E = E; view.d.k = k; view.d.n_group = n_group; view.d.topk_group = topk_group;
+  view.d.score_fn = score_fn; view.d.norm_topk = norm_topk; view.d.act_dtype = act_dtype; view.d.device = dev;
+  view.device = dev; view.num_sms = nd.num_sms;
+  view.Wr = Wr; view.b_logit = b_logit; view.corr_bias = corr_bias;
+  view.partial = nd.partial;
+  int tt, ks;
+  caee_router_shape(&view, T, &tt, &ks, nullptr);
+  const size_t need = (size_t)ks * (size_t)T * (size_t)E;
+  if (need > (size_t)CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS)
+    return caee_fail(nullptr, CAEE_ESHAPE, "%s: T=%d, E=%d with a %d-way split needs %zu scratch floats, the static array holds %d", me, T,
+                     E, ks, need, CAEE_ROUTE_NOALLOC_SCRATCH_FLOATS);
+  cudaStream_t st = (cudaStream_t)stream;
+  if ((rc = caee_launch_router_logits(&view, x, T, st)) != CAEE_OK) return caee_fail(nullptr, rc, "%s: %s", me, view.err.c_str());
+  caee_launch_route_topk(&view, nullptr, T, scores, idx, gate, st);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return caee_fail(nullptr, CAEE_ECUDA, "%s: launch failed: %s", me, cudaGetErrorString(e));
+  return CAEE_OK;
 }
