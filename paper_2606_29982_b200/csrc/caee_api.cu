@@ -210,6 +210,7 @@ caee_status create_impl(caee_ctx* c) {
     if ((rc = caee_fp8_make_tensor_maps(c)) != CAEE_OK) return rc;
     if (const char* v = getenv("CAEE_FP8_WIDE_MIN_TOKENS")) c->fp8_wide_min_tokens = std::max(1, atoi(v));   // tuning aid
     if (const char* v = getenv("CAEE_FP8_WIDE_PAIRS")) c->fp8_wide_pairs = atoi(v) != 0;                      // tuning aid
+    if (const char* v = getenv("CAEE_TS_RUN_TOKENS")) c->ts_run_tokens = atoi(v) > CAEE_RUN_TOKENS ? CAEE_RUN_TOKENS_TS : CAEE_RUN_TOKENS;   // tuning aid
     if (const char* v = getenv("CAEE_FP8_TS")) c->fp8_ts = atoi(v) != 0;                                      // tuning aid
     if (!caee_fp8_wide_supported(c)) c->fp8_wide_min_tokens = 1 << 30;   // k range too long for its scale registers
     if (d.max_tokens >= c->fp8_wide_min_tokens) { A(c->xg, caee_fp8_wide_xg_bytes(c)); }
@@ -614,12 +615,12 @@ static caee_status forward_impl(caee_ctx* c, const void* x, const float* scores,
   // weight ring (only the shared experts and the few hottest experts are split and streamed twice),
   // and the e4m3 kernel's hi/lo terms share one MMA (expert_fp8.cu); larger steps keep 128 for weight reuse
   c->wl.run_cap = (c->kernel == CAEE_KERNEL_UMMA && T <= 128) ? CAEE_RUN_TOKENS_MIN : CAEE_RUN_TOKENS;
-  // e4m3 prefill-size steps: the A-from-TMEM kernel on 128-token runs (expert_fp8_ts.cu), or the shared-memory converter
+  // e4m3 prefill-size steps: the A-from-TMEM kernel on 192-token runs (expert_fp8_ts.cu), or the shared-memory converter
   // kernel on 256-token runs (expert_fp8_wide.cu; also for CTA pairs)
   c->step_prefill = 0;
   if (c->kernel == CAEE_KERNEL_UMMA && c->d.w_dtype == CAEE_E4M3 && T >= c->fp8_wide_min_tokens) {
     c->step_prefill = (c->fp8_ts && !c->fp8_wide_pairs) ? 2 : 1;
-    c->wl.run_cap = c->step_prefill == 2 ? CAEE_RUN_TOKENS : CAEE_RUN_TOKENS_WIDE;
+    c->wl.run_cap = c->step_prefill == 2 ? c->ts_run_tokens : CAEE_RUN_TOKENS_WIDE;
   }
   if (c->cache) {
     // R33: the step's cost model and run order see the cache as it is now (other layers' misses

@@ -27,6 +27,7 @@
 #define CAEE_MAX_D 64
 #define CAEE_RUN_TOKENS 128 /* most tokens per run: one UMMA N tile */
 #define CAEE_RUN_TOKENS_MIN 64
+#define CAEE_RUN_TOKENS_TS 192 /* e4m3 prefill kernel with the weights in tensor memory (expert_fp8_ts.cu), its wider shape */
 #define CAEE_RUN_TOKENS_WIDE 256 /* e4m3 prefill kernel (expert_fp8_wide.cu): one N = 256 UMMA tile */
 #define CAEE_FP8_WIDE_MIN_TOKENS 129 /* e4m3 steps of at least this many tokens take the converter kernels (expert_fp8_ts.cu / _wide.cu):
                                         measured on C4 against the decode kernel, T=192 -6%, T=256 -7%, T=128 +4% (the x gather) */
@@ -164,6 +165,7 @@ struct caee_ctx {
   int fp8_wide_min_tokens = CAEE_FP8_WIDE_MIN_TOKENS;
   bool pdl = true;                   // programmatic dependent launches on the decode path (env CAEE_NO_PDL=1 switches them off)
   int step_prefill = 0;              // this step's e4m3 expert kernel: 0 decode (expert_fp8.cu), 1 expert_fp8_wide.cu, 2 expert_fp8_ts.cu
+  int ts_run_tokens = CAEE_RUN_TOKENS_TS;   // run cap of expert_fp8_ts.cu steps: CAEE_RUN_TOKENS_TS (192) or 128 (env CAEE_TS_RUN_TOKENS=128)
   bool fp8_ts = true;                // prefill-size e4m3 steps take the A-from-TMEM kernel (expert_fp8_ts.cu); env CAEE_FP8_TS=0: expert_fp8_wide.cu
   bool fp8_wide_pairs = false;       // e4m3 prefill kernel on CTA pairs (cta_group::2); env CAEE_FP8_WIDE_PAIRS=1 at caee_create
   float* ks_part = nullptr;          // UMMA decode kernels: partial sums of split phase-1 tiles (KSplit, umma_common.cuh)

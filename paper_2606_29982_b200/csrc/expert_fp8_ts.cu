@@ -13,11 +13,14 @@
 // K-major A fragment has there) and the MMAs read them on the tensor datapath: shared memory carries
 // only the token operand (48 KB per 64 k at N = 128, 375 cycles against 512 of MMAs).
 //
-// TMEM budget (512 columns).  Two fp32 accumulators of N <= 128 columns (gate | up of 128 features, or
-// 256 down rows): 256 columns.  A ring of 2 stages x (2 tiles x 64 columns = 128 k of 128 rows each):
-// 256 columns.  Hence runs of at most 128 tokens here (256 in expert_fp8_wide.cu): a hot expert's
-// weights are converted once per 128-token run — conversion is cheap (F2FP + HMUL2 per code pair at
-// full ALU rate), it was its shared-memory traffic that cost.
+// TMEM budget (512 columns), two shapes (TsCfg below).  192-token runs, the default: two fp32 accumulators of
+// N <= 192 columns (gate | up of 128 features, or 256 down rows) = 384 columns, and an A ring of 2 stages x (2 tiles
+// x 32 columns = 64 k of 128 rows each) = 128 columns.  128-token runs (CAEE_TS_RUN_TOKENS=128; round 2's first
+// version): accumulators 256 columns, A ring 2 stages x 128 k = 256 columns.  A hot expert's weights are streamed
+// (from L2) and converted once per run — conversion is cheap (F2FP + HMUL2 per code pair at full ALU rate), it was
+// its shared-memory traffic that cost in expert_fp8_wide.cu — but a run costs 2.4-3.4 us whatever its length, so the
+// longer runs win: config 4's 4096-token step has 354 runs instead of 433 and the kernel takes 3.41-3.45 instead of
+// 3.57-3.62 ms (0.67-0.68 instead of 0.64-0.65 of the sustained tensor rate; same box, interleaved).
 //
 // Pipeline (640 threads, 1 CTA per SM; all rings are mbarrier full/empty pairs):
 //   warp 0        tile claimer (atomic ticket, shared-memory queue; see umma_common.cuh) and weight producer: one
@@ -27,13 +30,14 @@
 //                 the MMA warp waited 25% of the time for converted weights; the copy engine prefetches deeper
 //                 at no register cost, and shared memory has room here (80 KB of traffic per 64 k at N = 128)
 //   warps 8-15    converters: warp w owns TMEM lane quadrant w % 4 of tile half (w - 8) / 4; thread = one
-//                 weight row: 128 codes per 128-k stage shared -> registers -> fp16 -> 2 x tcgen05.st (A ring)
-//   warp 2        token-operand loader: one bulk copy per 128-k stage from the run's stage image (tok ring,
-//                 4 x 32 KB; x images by k_gather_x, h images by the phase-1 epilogue: expert_fp8_wide.cu).
+//                 weight row: 128 codes per 128-k raw stage shared -> registers -> fp16 -> 2 x tcgen05.st (one A stage each,
+//                 or both into one 128-k A stage)
+//   warp 2        token-operand loader: one bulk copy per token stage from the run's stage image (tok ring, 5 x 24 KB
+//                 of 64 k, or 4 x 32 KB of 128 k in the 128-token shape; x images by k_gather_x, h images by the phase-1 epilogue: expert_fp8_wide.cu).
 //                 (Tried: writing the x images inside this kernel with the idle warp 3 of every CTA, row b of every
 //                 run by CTA b, phase-1 tiles waiting on a per-run counter — parity green, but one warp per SM moves a
 //                 14 KB row in ~20 us and the step went from 3.55 to 8.45 ms; k_gather_x stays.)
-//   warp 1        MMA issuer: 16 tcgen05.mma (A from TMEM, M 128, N = padded tokens, K 16) per 128-k stage
+//   warp 1        MMA issuer: 8 tcgen05.mma (A from TMEM, M 128, N = padded tokens, K 16) per 64-k stage (16 per 128-k stage)
 //   warps 4-7, 16-19   epilogue: TMEM -> SwiGLU -> h (fp16 stage image), or -> o rows (fp32)
 #include <cstdio>
 #include <cstring>
@@ -46,17 +50,29 @@ using namespace caee_umma;
 
 constexpr int kThreads = 640;
 constexpr int kKRaw = 128;                 // k per packed stage = one block-scale block
-constexpr int kAStagesT = 2, kTokStages = 4;                    // both rings in 128-k stages: one hand-over per block-scale block
-constexpr int kRunTokens = CAEE_RUN_TOKENS;                     // 128
-constexpr int kTokBytes = kRunTokens * kKRaw * 2;               // 32 KB: two 64-k images of 128 rows x 128 bytes
 constexpr int kRawStages = 3;
-constexpr int kRawOff = kTokStages * kTokBytes;                 // raw ring behind the token ring
-constexpr int kSmemBytes = kRawOff + kRawStages * kAStageBytes; // 128 + 96 = 224 KB
 constexpr int kConvWarps = 8, kEpiWarps = 8;
-constexpr int kAccCols = 128;              // TMEM columns per accumulator
-constexpr int kACol0 = 2 * kAccCols;       // first column of the A ring
-constexpr int kAStageCols = 128;           // two tiles x 64 columns (128 fp16 per row)
 constexpr int kMaxKb = 64;
+// Two shapes of the same kernel, by the most tokens of a run (= the MMAs' N, = TMEM columns per accumulator):
+//   kRun 128: accumulators 2 x 128 columns, A ring 2 stages x 128 columns (128 k: one hand-over per block-scale block),
+//             token ring 4 x 32 KB (128-k stages);
+//   kRun 192: accumulators 2 x 192 columns, A ring 2 stages x 64 columns (64 k), token ring 5 x 24 KB (64-k stages).
+//             A hot expert's image is streamed from L2 and converted once per 192 instead of once per 128 tokens
+//             (config 4's 4096-token step: 354 runs instead of 433; a run costs 2.4-3.4 us whatever its length).
+template <int kRun>
+struct TsCfg {
+  static constexpr int kSubK = kRun <= 128 ? 128 : 64;            // k per A stage and per token stage
+  static constexpr int kAStagesT = 2;
+  static constexpr int kTokStages = kRun <= 128 ? 4 : 5;
+  static constexpr int kTokBytes = kRun * kSubK * 2;              // kSubK / 64 images of kRun rows x 128 bytes
+  static constexpr int kRawOff = kTokStages * kTokBytes;          // raw ring behind the token ring
+  static constexpr int kSmemBytes = kRawOff + kRawStages * kAStageBytes;   // 224 KB / 216 KB
+  static constexpr int kAccCols = kRun;                           // TMEM columns per accumulator
+  static constexpr int kACol0 = 2 * kAccCols;                     // first column of the A ring
+  static constexpr int kAStageCols = kSubK;                       // two tiles x kSubK / 2 columns (two fp16 per column)
+  static_assert(kACol0 + kAStagesT * kAStageCols <= kTmemCols, "TMEM budget");
+  static_assert(kSmemBytes + 1024 <= 227 * 1024, "shared memory budget");
+};
 
 struct TsParams {
   caee_worklist wl;
@@ -113,7 +129,12 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, ui
 #define WAIT_T(acc, ...) do { __VA_ARGS__; } while (0)      /* acc is not even named in the product build */
 #endif
 
+template <int kRun>
 __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_constant__ TsParams p) {
+  using C = TsCfg<kRun>;
+  constexpr int kSubK = C::kSubK, kAStagesT = C::kAStagesT, kTokStages = C::kTokStages, kTokBytes = C::kTokBytes;
+  constexpr int kRawOff = C::kRawOff, kAccCols = C::kAccCols, kACol0 = C::kACol0, kAStageCols = C::kAStageCols;
+  constexpr int kRunTokens = kRun;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   constexpr int kBars = 2 * (kAStagesT + kTokStages + kRawStages) + 2 + 2 * kQueue;
@@ -202,44 +223,75 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_cons
       const uint32_t sub_bytes = (uint32_t)npad * 128u;       // one 64-k image of the run inside a token stage
       WAIT_T(w_a, mbar_wait(tempty, (it & 1) ^ 1));
       tc_fence_after();
-      for (int s = 0; s < nkb; ++s) {
-        WAIT_T(w_b, mbar_wait(cfull0 + 8 * cs, cph));
-        WAIT_T(w_c, mbar_wait(kfull0 + 8 * ks, kph));
-        tc_fence_after();
-        const uint32_t a0 = tmem_base + kACol0 + cs * kAStageCols, a1 = a0 + kAStageCols / 2;
-        const uint64_t b0 = make_desc_sw128(smem_base + ks * kTokBytes), b1 = make_desc_sw128(smem_base + ks * kTokBytes + sub_bytes);
-        if (elect_one()) {
-          if (s == 0) {
-            umma_f16_ts<false>(d0, a0, b0, idesc);
-            umma_f16_ts<false>(d1, a1, b0, idesc);
-          } else {
-            umma_f16_ts<true>(d0, a0, b0, idesc);
-            umma_f16_ts<true>(d1, a1, b0, idesc);
-          }
+      if constexpr (kSubK == 128) {
+        for (int s = 0; s < nkb; ++s) {
+          WAIT_T(w_b, mbar_wait(cfull0 + 8 * cs, cph));
+          WAIT_T(w_c, mbar_wait(kfull0 + 8 * ks, kph));
+          tc_fence_after();
+          const uint32_t a0 = tmem_base + kACol0 + cs * kAStageCols, a1 = a0 + kAStageCols / 2;
+          const uint64_t b0 = make_desc_sw128(smem_base + ks * kTokBytes), b1 = make_desc_sw128(smem_base + ks * kTokBytes + sub_bytes);
+          if (elect_one()) {
+            if (s == 0) {
+              umma_f16_ts<false>(d0, a0, b0, idesc);
+              umma_f16_ts<false>(d1, a1, b0, idesc);
+            } else {
+              umma_f16_ts<true>(d0, a0, b0, idesc);
+              umma_f16_ts<true>(d1, a1, b0, idesc);
+            }
 #pragma unroll
-          for (int k16 = 1; k16 < kKRaw / 16; ++k16) {   // per 16-k step: weights +8 TMEM columns, tokens +32 B (>> 4) inside a 64-k image
-            const uint64_t b = (k16 < 4 ? b0 : b1) + (uint64_t)((k16 & 3) * 2);
-            umma_f16_ts<true>(d0, a0 + k16 * 8, b, idesc);
-            umma_f16_ts<true>(d1, a1 + k16 * 8, b, idesc);
+            for (int k16 = 1; k16 < kKRaw / 16; ++k16) {   // per 16-k step: weights +8 TMEM columns, tokens +32 B (>> 4) inside a 64-k image
+              const uint64_t b = (k16 < 4 ? b0 : b1) + (uint64_t)((k16 & 3) * 2);
+              umma_f16_ts<true>(d0, a0 + k16 * 8, b, idesc);
+              umma_f16_ts<true>(d1, a1 + k16 * 8, b, idesc);
+            }
+            tc_commit(cempty0 + 8 * cs);
+            tc_commit(kempty0 + 8 * ks);
+            if (s == nkb - 1) tc_commit(tfull);
           }
-          tc_commit(cempty0 + 8 * cs);
-          tc_commit(kempty0 + 8 * ks);
-          if (s == nkb - 1) tc_commit(tfull);
+          __syncwarp();
+          if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
+          if (++ks == kTokStages) { ks = 0; kph ^= 1; }
         }
-        __syncwarp();
-        if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
-        if (++ks == kTokStages) { ks = 0; kph ^= 1; }
+      } else {
+        // 64-k stages on both rings: 2 nkb hand-overs of 8 MMAs each
+        for (int s = 0; s < 2 * nkb; ++s) {
+          WAIT_T(w_b, mbar_wait(cfull0 + 8 * cs, cph));
+          WAIT_T(w_c, mbar_wait(kfull0 + 8 * ks, kph));
+          tc_fence_after();
+          const uint32_t a0 = tmem_base + kACol0 + cs * kAStageCols, a1 = a0 + kAStageCols / 2;
+          const uint64_t b0 = make_desc_sw128(smem_base + ks * kTokBytes);
+          if (elect_one()) {
+            if (s == 0) {
+              umma_f16_ts<false>(d0, a0, b0, idesc);
+              umma_f16_ts<false>(d1, a1, b0, idesc);
+            } else {
+              umma_f16_ts<true>(d0, a0, b0, idesc);
+              umma_f16_ts<true>(d1, a1, b0, idesc);
+            }
+#pragma unroll
+            for (int k16 = 1; k16 < 4; ++k16) {
+              umma_f16_ts<true>(d0, a0 + k16 * 8, b0 + (uint64_t)(k16 * 2), idesc);
+              umma_f16_ts<true>(d1, a1 + k16 * 8, b0 + (uint64_t)(k16 * 2), idesc);
+            }
+            tc_commit(cempty0 + 8 * cs);
+            tc_commit(kempty0 + 8 * ks);
+            if (s == 2 * nkb - 1) tc_commit(tfull);
+          }
+          __syncwarp();
+          if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
+          if (++ks == kTokStages) { ks = 0; kph ^= 1; }
+        }
       }
     }
   } else if (warp == 2) {
-    // ===== token-operand loader: ONE bulk copy per 128-k stage (two consecutive 64-k images) from the run's stage images
+    // ===== token-operand loader: ONE bulk copy per token stage (kSubK k: one or two consecutive 64-k images) from the run's stage images
     if (lane == 0) {
       int stage = 0, ph = 0;
       while (tm.at(tq.pop1(), t)) {
         const int npad = (p.wl.run_n[t.run] + 15) & ~15;
-        const int nsub = t.phase == 1 ? p.KB1 : p.KB2;
+        const int nsub = (t.phase == 1 ? p.KB1 : p.KB2) * (kKRaw / kSubK);
         const size_t row_bytes = (size_t)(t.phase == 1 ? p.H : p.I) * 2;
-        const uint32_t stage_bytes = (uint32_t)npad * 256u;      // two consecutive 64-k images of the run: one copy
+        const uint32_t stage_bytes = (uint32_t)npad * (uint32_t)(kSubK * 2);   // kSubK / 64 consecutive 64-k images of the run: one copy
         const uint8_t* src = (t.phase == 1 ? p.xg : p.hbuf) + (size_t)p.wl.run_hrow[t.run] * row_bytes;
         if (t.phase == 2) {
           const int* flag = p.wl.ready + t.run;
@@ -359,22 +411,44 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_cons
         const __half2 w2 = __float2half2_rn(__shfl_sync(0xffffffffu, s0, kb & 31));
         WAIT_T(w_c, mbar_wait(rfull0 + 8 * rs, rph));          // the stage's codes have landed (bulk copy)
         const uint8_t* raw = smem + kRawOff + rs * kAStageBytes + row_off;
-        WAIT_T(w_a, mbar_wait(cempty0 + 8 * cs, cph ^ 1));     // the MMAs that read this A stage are done
-        tc_fence_after();
+        if constexpr (kSubK == 128) {
+          WAIT_T(w_a, mbar_wait(cempty0 + 8 * cs, cph ^ 1));     // the MMAs that read this A stage are done
+          tc_fence_after();
 #pragma unroll
-        for (int hh = 0; hh < 2; ++hh) {
-          uint32_t o[32];
+          for (int hh = 0; hh < 2; ++hh) {
+            uint32_t o[32];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) widen16_ts(*reinterpret_cast<const uint4*>(raw + hh * 512 + i * 128), w2, o + 8 * i);
-          tmem_st32(trow + cs * kAStageCols + hh * 32, o);
+            for (int i = 0; i < 4; ++i) widen16_ts(*reinterpret_cast<const uint4*>(raw + hh * 512 + i * 128), w2, o + 8 * i);
+            tmem_st32(trow + cs * kAStageCols + hh * 32, o);
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(rempty0 + 8 * rs);      // this warp has read its rows of the stage
+          WAIT_T(w_b, tmem_st_wait());
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(cfull0 + 8 * cs);
+          if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
+        } else {
+          // 64-k A stages: each half of the raw stage is its own hand-over
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            uint32_t o[32];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) widen16_ts(*reinterpret_cast<const uint4*>(raw + hh * 512 + i * 128), w2, o + 8 * i);
+            if (hh == 1) {
+              __syncwarp();
+              if (lane == 0) mbar_arrive(rempty0 + 8 * rs);    // both halves of this warp's rows are in registers
+            }
+            WAIT_T(w_a, mbar_wait(cempty0 + 8 * cs, cph ^ 1));
+            tc_fence_after();
+            tmem_st32(trow + cs * kAStageCols, o);
+            WAIT_T(w_b, tmem_st_wait());
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cfull0 + 8 * cs);
+            if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
+          }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(rempty0 + 8 * rs);      // this warp has read its rows of the stage
-        WAIT_T(w_b, tmem_st_wait());
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(cfull0 + 8 * cs);
-        if (++cs == kAStagesT) { cs = 0; cph ^= 1; }
         if (++rs == kRawStages) { rs = 0; rph ^= 1; }
       }
     }
@@ -395,7 +469,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_expert_fp8_ts(const __grid_cons
 }  // namespace
 
 // runs [run_begin, run_begin + run_count) (run_count < 0: every run of the work list), tile tickets from
-// wl.sched[ticket].  Runs hold up to CAEE_RUN_TOKENS (128) tokens; x images by caee_launch_fp8_wide_prepare.
+// wl.sched[ticket].  Runs hold up to wl.run_cap = CAEE_RUN_TOKENS_TS (192) or CAEE_RUN_TOKENS (128) tokens; x images by
+// caee_launch_fp8_wide_prepare.
 void caee_launch_expert_fp8_ts(caee_ctx* c, int T, int run_begin, int run_count, int ticket, cudaStream_t st) {
   (void)T;
   ++c->n_launches;
@@ -414,9 +489,17 @@ void caee_launch_expert_fp8_ts(caee_ctx* c, int T, int run_begin, int run_count,
   p.t2_off = p.P1 * p.KB1 * 2;
   p.norm_off = (int)caee_fp8_norm_offset(c);
   p.slots = d.k + d.S;
+  if (c->wl.run_cap > CAEE_RUN_TOKENS) {
+    if (!(c->attr_done & 32u)) {
+      cudaFuncSetAttribute(k_expert_fp8_ts<CAEE_RUN_TOKENS_TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, TsCfg<CAEE_RUN_TOKENS_TS>::kSmemBytes + 1024);
+      c->attr_done |= 32u;
+    }
+    k_expert_fp8_ts<CAEE_RUN_TOKENS_TS><<<c->num_sms, kThreads, TsCfg<CAEE_RUN_TOKENS_TS>::kSmemBytes + 1024, st>>>(p);
+    return;
+  }
   if (!(c->attr_done & 16u)) {
-    cudaFuncSetAttribute(k_expert_fp8_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes + 1024);
+    cudaFuncSetAttribute(k_expert_fp8_ts<CAEE_RUN_TOKENS>, cudaFuncAttributeMaxDynamicSharedMemorySize, TsCfg<CAEE_RUN_TOKENS>::kSmemBytes + 1024);
     c->attr_done |= 16u;
   }
-  k_expert_fp8_ts<<<c->num_sms, kThreads, kSmemBytes + 1024, st>>>(p);
+  k_expert_fp8_ts<CAEE_RUN_TOKENS><<<c->num_sms, kThreads, TsCfg<CAEE_RUN_TOKENS>::kSmemBytes + 1024, st>>>(p);
 }

@@ -508,14 +508,16 @@ def test_forward_small_fp8(H, kernel):
         L.close()
 
 
-@pytest.mark.parametrize("T,ts", [(24, 1), (130, 1), (300, 1), (300, 0)])
+@pytest.mark.parametrize("T,ts", [(24, 1), (130, 1), (300, 1), (300, 128), (300, 0)])
 def test_forward_fp8_uneven_block_scales(H, T, ts, monkeypatch):
     """Block scales spread over three decades inside one tile row: the per-block promotion of the
     decode kernel (T = 24) and the scale x 2^J folding into fp16 weights of the converter kernels
-    (T >= 129: expert_fp8_ts.cu, A operand from tensor memory; ts = 0: expert_fp8_wide.cu, through shared
-    memory) must still match the oracle's exact dequantisation."""
+    (T >= 129: expert_fp8_ts.cu, A operand from tensor memory, in its default 192-token shape or — ts = 128 — its
+    128-token one; ts = 0: expert_fp8_wide.cu, through shared memory) must still match the oracle's exact dequantisation."""
     from paper_2606_29982_b200 import binding as B
-    monkeypatch.setenv("CAEE_FP8_TS", str(ts))
+    monkeypatch.setenv("CAEE_FP8_TS", str(int(ts != 0)))
+    if ts > 1:
+        monkeypatch.setenv("CAEE_TS_RUN_TOKENS", str(ts))
     cfg = C4S
     L = _layer(H, cfg, max_tokens=max(32, T), kernel=B.CAEE_KERNEL_UMMA)
     try:
@@ -674,14 +676,16 @@ def test_forward_c4_full_size_sampled(H, T, mode):
         L.close()
 
 
-@pytest.mark.parametrize("pairs,ts", [(0, 1), (0, 0), (1, 0)])
+@pytest.mark.parametrize("pairs,ts", [(0, 1), (0, 128), (0, 0), (1, 0)])
 def test_forward_c4_prefill_4096_sampled(H, pairs, ts, monkeypatch):
     """Config 4's 4096-token prefill batch (stand-alone decision kernels, segmented work-list fill): K_final and
-    F_* for all 4096 tokens bit-exact, y on sampled tokens.  ts = 1: the default kernel, expert_fp8_ts.cu (128-token
-    runs, widened weights in tensor memory); ts = 0: expert_fp8_wide.cu (256-token runs, widened weights in shared
-    memory), alone or — pairs = 1 — on CTA pairs (cta_group::2 MMAs of M = 256, static tile schedule)."""
+    F_* for all 4096 tokens bit-exact, y on sampled tokens.  ts = 1: the default kernel, expert_fp8_ts.cu (192-token
+    runs, widened weights in tensor memory; ts = 128: its 128-token shape); ts = 0: expert_fp8_wide.cu (256-token runs,
+    widened weights in shared memory), alone or — pairs = 1 — on CTA pairs (cta_group::2 MMAs of M = 256, static tile schedule)."""
     monkeypatch.setenv("CAEE_FP8_WIDE_PAIRS", str(pairs))
-    monkeypatch.setenv("CAEE_FP8_TS", str(ts))
+    monkeypatch.setenv("CAEE_FP8_TS", str(int(ts != 0)))
+    if ts > 1:
+        monkeypatch.setenv("CAEE_TS_RUN_TOKENS", str(ts))
     L = H.GpuLayer(wl.C4, seed=0, max_tokens=4096, keep_raw=False)
     try:
         T = 4096
